@@ -1,0 +1,727 @@
+"""Pins for the fp64 CPU oracle (oracle/ahs_oracle.c): what the paper and the mathematics fix.
+
+None of these compare the oracle with the CUDA path; all run with -m "not gpu".  Each test says what a
+plausible mistake it would catch.  Independent evaluations in this file use a different formulation
+from the oracle's (vectorised complex numpy with np.roll, or literal per-term Python complex loops).
+Citations are PAPER.md line numbers / equation numbers; readings R1.. are listed in DESIGN.md.
+"""
+import cmath
+import math
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+TWO_PI = 2.0 * math.pi
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers (independent formulation: arrays are [z, y, x]; direction i <-> numpy axis 2 - i)
+# ------------------------------------------------------------------------------------------------
+def sh(f, i, d):
+    """f evaluated at x + d*k_i (periodic)."""
+    return np.roll(f, -d, axis=2 - i)
+
+
+def unpack(f10):
+    phi = f10[0] + 1j * f10[1]
+    Pi = f10[2] + 1j * f10[3]
+    th = [f10[4], f10[5], f10[6]]
+    eps = [f10[7], f10[8], f10[9]]
+    return phi, Pi, th, eps
+
+
+def pack(phi, Pi, th, eps):
+    return np.ascontiguousarray(np.stack([phi.real, phi.imag, Pi.real, Pi.imag, *th, *eps]).astype(np.float64))
+
+
+def a_of(p, tau):
+    tref = p.tau_ref if p.tau_ref else p.tau0
+    return (tau / tref) ** p.m
+
+
+def np_gauss(p, f10, n):
+    """Gauss residual (R4) with np.roll."""
+    phi, Pi, th, eps = unpack(f10)
+    ah = a_of(p, p.tau0 + n * p.dt - 0.5 * p.dt)
+    div = sum(eps[i] - sh(eps[i], i, -1) for i in range(3))
+    rhs = 2 * p.q * p.dx ** 2 * p.e0 ** 2 * ah ** (2 * p.s) * np.imag(np.conj(phi) * Pi)
+    return np.abs(div - rhs).max(), np.sqrt(np.mean(rhs ** 2))
+
+
+def np_plaq(th, i, j):
+    return th[i] + sh(th[j], i, 1) - sh(th[i], j, 1) - th[j]
+
+
+def np_site_fields(p, f10, n):
+    """K, G, Lag of Eq. 2 / Eq. 10 in vectorised complex form."""
+    phi, Pi, th, eps = unpack(f10)
+    a = a_of(p, p.tau0 + n * p.dt)
+    U = [np.exp(-1j * p.q * th[i]) for i in range(3)]
+    G = sum(np.abs(U[i] * sh(phi, i, 1) - phi) ** 2 for i in range(3)) / p.dx ** 2
+    K = np.abs(Pi) ** 2
+    ea2 = (p.e0 * a ** (p.s - 1)) ** 2 * a ** 2
+    la2 = p.lambda0 * a ** (2 * (p.s - 1)) * a ** 2
+    mag = sum(1 - np.cos(np_plaq(th, i, j)) for i in range(3) for j in range(3) if i != j)
+    gauge = (sum(e ** 2 for e in eps) - p.c_B / p.dx ** 2 * mag) / (2 * ea2 * p.dx ** 2)
+    Lag = gauge + K - G - la2 / 4 * (np.abs(phi) ** 2 - p.sigma ** 2) ** 2
+    return K, G, Lag
+
+
+def random_state(N, rng, amp=0.3):
+    phi = (1 + amp * rng.standard_normal((N, N, N))) * np.exp(1j * rng.uniform(0, TWO_PI, (N, N, N)))
+    Pi = amp * (rng.standard_normal((N, N, N)) + 1j * rng.standard_normal((N, N, N)))
+    th = [amp * rng.standard_normal((N, N, N)) for _ in range(3)]
+    eps = [amp * rng.standard_normal((N, N, N)) for _ in range(3)]
+    return pack(phi, Pi, th, eps)
+
+
+# ------------------------------------------------------------------------------------------------
+# P14  Philox4x32-10
+# ------------------------------------------------------------------------------------------------
+def test_philox_known_answers(oracle):
+    """Catches: wrong multiplier/Weyl constant, hi/lo swapped, wrong lane permutation, 7 vs 10 rounds."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        assert oracle.philox4x32_10(v[0:4], v[4:6]) == tuple(v[6:10])
+
+
+def test_philox_matches_aten_engine(oracle, tmp_path):
+    """Independent implementation: ATen's CPU-usable philox_engine header (10 rounds, same key/counter
+    packing as cuRAND: key = seed, counter = (offset, subsequence)).  Catches a wrong KAT memory."""
+    import torch
+    inc = os.path.join(os.path.dirname(torch.__file__), "include")
+    hdr = os.path.join(inc, "ATen", "core", "PhiloxRNGEngine.h")
+    if not os.path.exists(hdr):
+        pytest.skip("ATen philox header not in this torch build")
+    src = tmp_path / "aten_philox.cpp"
+    src.write_text(
+        '#include <cstdio>\n#include <cstdint>\n#include <cstdlib>\n#include <ATen/core/PhiloxRNGEngine.h>\n'
+        'int main(int argc, char** argv) {\n'
+        '  uint64_t seed = strtoull(argv[1], 0, 0), sub = strtoull(argv[2], 0, 0), off = strtoull(argv[3], 0, 0);\n'
+        '  at::Philox4_32 g(seed, sub, off);\n'
+        '  for (int i = 0; i < 4; ++i) printf("%u\\n", (unsigned)g());\n  return 0; }\n')
+    exe = tmp_path / "aten_philox"
+    r = subprocess.run(["g++", "-O1", "-std=c++17", "-I", inc, "-o", str(exe), str(src)], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip("ATen philox header does not compile standalone here: " + r.stderr[-300:])
+    for seed, site in [(0, 0), (180900995, 12345), (0xDEADBEEF12345678, (1 << 33) + 17), (7, 1 << 30)]:
+        out = subprocess.check_output([str(exe), str(seed), "0", str(site)], text=True).split()
+        got = tuple(int(v) for v in out)
+        # ours: counter = (site_lo, site_hi, 0, 0), key = (seed_lo, seed_hi)
+        mine = oracle.philox4x32_10((site & 0xFFFFFFFF, site >> 32, 0, 0), (seed & 0xFFFFFFFF, seed >> 32))
+        assert got == mine
+
+
+# ------------------------------------------------------------------------------------------------
+# P15  initial condition
+# ------------------------------------------------------------------------------------------------
+def test_ic_random_phase(oracle):
+    p = oracle.Params(N=32, sigma=1.3)
+    f = oracle.initial_condition(p, seed=180900995)
+    phi, Pi, th, eps = unpack(f)
+    np.testing.assert_allclose(np.abs(phi), 1.3, rtol=0, atol=7e-16)      # |phi| = sigma (L72)
+    assert not f[2:].any()                                                # all other variables zero (L72)
+    # phase from Philox word pair (r0, r1) of counter = site: check two sites by hand
+    for site in (0, 31 * 32 * 32 + 5):
+        r = oracle.philox4x32_10((site, 0, 0, 0), (180900995, 0))
+        u = ((r[0] << 32 | r[1]) >> 11) * 2.0 ** -53
+        z = 1.3 * cmath.exp(1j * TWO_PI * u)
+        assert abs(phi.reshape(-1)[site] - z) < 1e-15
+    # phases uniform: mean of exp(i theta) ~ 0 within 5 sigma/sqrt(N^3)
+    assert abs(np.mean(phi / 1.3)) < 5.0 / math.sqrt(32 ** 3)
+    # different seeds differ, same seed repeats
+    assert np.array_equal(f, oracle.initial_condition(p, seed=180900995))
+    assert not np.array_equal(f, oracle.initial_condition(p, seed=180900996))
+
+
+def test_ic_obeys_gauss_and_third_of_plaquettes_pierced(oracle):
+    """L72: the IC 'obeys the discretized form of Gauss's law'.  Four i.i.d. uniform corner phases pierce
+    a plaquette with probability 1/3 (Vachaspati-Vilenkin): pins the winding count on random data."""
+    p = oracle.Params(N=48)
+    f = oracle.initial_condition(p, seed=3)
+    d = oracle.diagnostics(p, f, 0)
+    assert d["gauss_max"] == 0.0 and d["gauss_rhs_rms"] == 0.0
+    frac = d["n_pierced"] / (3 * 48 ** 3)
+    assert abs(frac - 1.0 / 3.0) < 0.01, frac
+    assert d["sum_abs_w"] == d["n_pierced"]          # theta = 0: |W| <= 1
+    assert d["L"] == pytest.approx(math.pi / 6 * p.dx * d["n_pierced"], rel=1e-15)     # L93
+    assert d["xi"] == pytest.approx(math.sqrt((48 * p.dx) ** 3 / d["L"]), rel=1e-15)  # L88
+
+
+def test_ic_gaussian_moments(oracle):
+    """BASELINE config 3: re, im each N(0, sigma^2/2) i.i.d.  Catches sigma vs sigma/sqrt2, log base, u1=0."""
+    p = oracle.Params(N=32, sigma=1.0)
+    f = oracle.initial_condition(p, seed=11, kind=oracle.IC_GAUSSIAN)
+    re, im = f[0].ravel(), f[1].ravel()
+    n = re.size
+    assert np.isfinite(f).all() and not f[2:].any()
+    for v in (re, im):
+        assert abs(v.mean()) < 5 * math.sqrt(0.5 / n)
+        assert abs(v.var() - 0.5) < 5 * 0.5 * math.sqrt(2.0 / n)
+        assert abs(np.mean(v ** 4) - 3 * 0.25) < 0.05           # Gaussian kurtosis
+    assert abs(np.mean(re * im)) < 5 * 0.5 / math.sqrt(n)
+
+
+# ------------------------------------------------------------------------------------------------
+# P1  Gauss's law preserved to machine precision
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("m,s", [(1, 1), (2, 0), (1, 0), (2, 1), (0, 1), (1, 0.5)])
+def test_gauss_law_at_roundoff(oracle, m, s):
+    """Ties the current coefficient d2 to the Laplacian coefficient c2 and the dampings c1, d1, and the
+    a^(2s) dx^2 e0^2 of the residual.  Catches: wrong sign/coefficient of the current, a_n vs a_{n+1/2},
+    curl not divergence-free (index error), Pi/eps time level mix-up."""
+    p = oracle.Params(N=12, m=m, s=s, e0=0.9, lambda0=1.7, dx=0.6)
+    f = oracle.initial_condition(p, seed=5)
+    oracle.step(p, f, 0, 20)
+    res, scale = np_gauss(p, f, 20)
+    assert scale > 0.005                           # the charge density is not trivially zero
+    assert res < 2e-13 * max(1.0, scale), (res, scale)
+    d = oracle.diagnostics(p, f, 20)
+    assert abs(d["gauss_max"] - res) < 1e-13 * max(1.0, scale)      # both at roundoff; sums ordered differently
+    assert d["gauss_rhs_rms"] == pytest.approx(scale, rel=1e-12)
+    # a deliberately wrong half-step level must show an O(dt) violation: the test has teeth
+    p_bad = oracle.Params(**{**oracle.params_dict(p), "tau0": p.tau0 + 0.5 * p.dt})
+    if m != 0 and s != 0:
+        assert np_gauss(p_bad, f, 20)[0] > 1e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# P3  brute-force per-term evaluation of Eqs. 4-7 on 4^3 (north_star)
+# ------------------------------------------------------------------------------------------------
+def brute_force_step(p, f10, n):
+    """Eqs. 4-7 literally, site by site, with Python complex numbers and explicit (x+-1)%N indices.
+    No shared sub-expressions, no arrays of intermediate products."""
+    N = p.N
+    phi, Pi, th, eps = unpack(f10)
+    q = p.q
+    tau = p.tau0 + n * p.dt
+    am, a0, ap = a_of(p, tau - p.dt / 2), a_of(p, tau), a_of(p, tau + p.dt / 2)
+    e_ = lambda a: p.e0 * a ** (p.s - 1)          # Eq. 8
+    lam_ = lambda a: p.lambda0 * a ** (2 * (p.s - 1))
+    new = np.array(f10, copy=True)
+
+    def idx(x, y, z, i, d):
+        c = [x, y, z]
+        c[i] = (c[i] + d) % N
+        return (c[2], c[1], c[0])
+
+    def plaq(x, y, z, i, j):
+        return (th[i][z, y, x] + th[j][idx(x, y, z, i, 1)] - th[i][idx(x, y, z, j, 1)] - th[j][z, y, x])
+
+    for z in range(N):
+        for y in range(N):
+            for x in range(N):
+                f0 = complex(phi[z, y, x])
+                lap = 0j
+                for j in range(3):
+                    lap += (complex(phi[idx(x, y, z, j, 1)]) * cmath.exp(-1j * q * th[j][z, y, x]) - 2 * f0
+                            + complex(phi[idx(x, y, z, j, -1)]) * cmath.exp(+1j * q * th[j][idx(x, y, z, j, -1)]))
+                Pn = ((am / ap) ** 2 * complex(Pi[z, y, x])
+                      - p.dt * (a0 ** 2 / ap) ** 2 * lam_(a0) / 2 * (abs(f0) ** 2 - p.sigma ** 2) * f0
+                      + p.dt / p.dx ** 2 * (a0 / ap) ** 2 * lap)
+                new[2][z, y, x], new[3][z, y, x] = Pn.real, Pn.imag
+                for i in range(3):
+                    cur = q * (f0.conjugate() * cmath.exp(-1j * q * th[i][z, y, x]) * complex(phi[idx(x, y, z, i, 1)])).imag
+                    curl = 0.0
+                    for j in range(3):
+                        if j == i:
+                            continue
+                        xm = [x, y, z]
+                        xm[j] = (xm[j] - 1) % N
+                        curl += math.sin(plaq(x, y, z, i, j)) - math.sin(plaq(xm[0], xm[1], xm[2], i, j))
+                    En = ((e_(ap) / e_(am)) ** 2 * eps[i][z, y, x] + 2 * p.dt * a0 ** 2 * e_(ap) ** 2 * cur
+                          - p.dt / p.dx ** 2 * (e_(ap) / e_(a0)) ** 2 * curl)
+                    new[7 + i][z, y, x] = En
+    new[0] += p.dt * new[2]
+    new[1] += p.dt * new[3]
+    for i in range(3):
+        new[4 + i] += p.dt * new[7 + i]
+    return new
+
+
+@pytest.mark.parametrize("m,s,q", [(1, 1, 1), (2, 0, 1), (1, 0.3, 1), (0, 1, 1), (1, 1, -1)])
+def test_step_against_brute_force_4cubed(oracle, m, s, q):
+    p = oracle.Params(N=4, m=m, s=s, q=q, dx=0.7, dt=0.05, lambda0=1.3, e0=0.8, sigma=1.1, tau0=2.0)
+    rng = np.random.default_rng(42)
+    f = random_state(4, rng)
+    want = f
+    for n in range(3, 6):
+        want = brute_force_step(p, want, n)
+    got = oracle.step(p, f.copy(), 3, 3)
+    for k in range(10):
+        scale = np.abs(want[k]).max()
+        assert np.abs(got[k] - want[k]).max() <= 2e-15 * max(scale, 1.0), oracle.FIELD_NAMES[k]
+
+
+def test_coeff_closed_forms(oracle):
+    """s = 1: the gauge sector is conformally invariant -> d1 = 1, d3 = dt/dx^2 for any a(tau).
+    m = 0: a = 1 -> c1 = d1 = 1, c2 = d3 = dt/dx^2, c3 = dt lambda0/2, d2 = 2 dt e0^2.
+    s = 0: lambda a^2 and e^2 a^2 are constant -> c3 = c2 dx^2 lambda0/2, d2 = 2 dt e0^2 (a_n/a_{n+1/2})^2."""
+    p = oracle.Params(N=4, m=2, s=1, dx=0.5, dt=0.1, e0=0.9, lambda0=1.7)
+    for n in (0, 7, 100):
+        c = oracle.coeffs(p, n)
+        assert c[3] == pytest.approx(1.0, abs=1e-15) and c[5] == pytest.approx(0.1 / 0.25, rel=1e-15)
+    p = oracle.Params(N=4, m=0, s=0.4, dx=0.5, dt=0.1, e0=0.9, lambda0=1.7)
+    c = oracle.coeffs(p, 13)
+    np.testing.assert_allclose(c, [1, 0.4, 0.1 * 1.7 / 2, 1, 2 * 0.1 * 0.81, 0.4], rtol=1e-15)
+    p = oracle.Params(N=4, m=1, s=0, dx=0.5, dt=0.1, e0=0.9, lambda0=1.7, tau0=1.0)
+    c = oracle.coeffs(p, 10)
+    a0, ap, am = 2.0, 2.05, 1.95
+    np.testing.assert_allclose(c[2], c[1] * 0.25 * 1.7 / 2, rtol=1e-14)
+    np.testing.assert_allclose(c[4], 2 * 0.1 * 0.81 * (a0 / ap) ** 2, rtol=1e-14)
+    np.testing.assert_allclose(c[0], (am / ap) ** 2, rtol=1e-14)
+    np.testing.assert_allclose(c[3], (am / ap) ** 2, rtol=1e-14)   # e ~ 1/a at s=0
+    # the normalisation of a drops out of every coefficient when s = 0 (R3)
+    p2 = oracle.Params(N=4, m=1, s=0, dx=0.5, dt=0.1, e0=0.9, lambda0=1.7, tau0=1.0, tau_ref=37.0)
+    np.testing.assert_allclose(oracle.coeffs(p2, 10), c, rtol=1e-13)
+
+
+# ------------------------------------------------------------------------------------------------
+# P2  "through variational principles" (L53): the kicks are minus the gradient of the potential part
+#     of the oracle's own Eq. 2, i.e. step and Lagrangian are tied together by calculus.
+# ------------------------------------------------------------------------------------------------
+def test_force_is_gradient_of_lagrangian(oracle):
+    """With Pi = eps = 0, -sum_x Lag = potential energy U(phi, theta) (Eq. 2).  At a = 1 one step from rest gives
+    Pi = dt * F_phi, eps = dt * F_theta with F_phi = -dU/dconj(phi), F_theta_i = -e^2 dx^2 dU/dtheta_i.
+    Catches: any wrong term/sign/index in the Laplacian, Higgs force, current or curl; c_B = 1/2 (Eq. 2's
+    stray factor, R2) fails this by a factor 2 in the curl."""
+    p = oracle.Params(N=4, m=0, s=1, dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0)
+    rng = np.random.default_rng(7)
+    f = random_state(4, rng, amp=0.4)
+    f[2:4] = 0.0
+    f[7:10] = 0.0
+
+    def U(g):
+        return -oracle.site_fields(p, np.ascontiguousarray(g), 0)[2].sum()
+
+    stepped = oracle.step(p, f.copy(), 0, 1)
+    F_phi = (stepped[2] + 1j * stepped[3]) / p.dt
+    F_th = [stepped[7 + i] / p.dt for i in range(3)]
+    h = 1e-5
+    for (z, y, x) in [(0, 0, 0), (1, 2, 3), (3, 3, 3), (2, 0, 1)]:
+        gp, gm = f.copy(), f.copy(); gp[0][z, y, x] += h; gm[0][z, y, x] -= h
+        dU_du = (U(gp) - U(gm)) / (2 * h)
+        gp, gm = f.copy(), f.copy(); gp[1][z, y, x] += h; gm[1][z, y, x] -= h
+        dU_dv = (U(gp) - U(gm)) / (2 * h)
+        want = -0.5 * (dU_du + 1j * dU_dv)
+        assert abs(F_phi[z, y, x] - want) < 1e-7 * max(1, abs(want))
+        for i in range(3):
+            gp, gm = f.copy(), f.copy(); gp[4 + i][z, y, x] += h; gm[4 + i][z, y, x] -= h
+            want = -(p.e0 * p.dx) ** 2 * (U(gp) - U(gm)) / (2 * h)
+            assert abs(F_th[i][z, y, x] - want) < 1e-7 * max(1, abs(want))
+    # teeth: Eq. 2 as printed (c_B = 1/2) is not the potential of Eq. 5
+    p_half = oracle.Params(**{**oracle.params_dict(p), "c_B": 0.5})
+    gp, gm = f.copy(), f.copy(); gp[4][1, 2, 3] += h; gm[4][1, 2, 3] -= h
+    Uh = lambda g: -oracle.site_fields(p_half, g, 0)[2].sum()
+    bad = -(p.e0 * p.dx) ** 2 * (Uh(gp) - Uh(gm)) / (2 * h)
+    assert abs(F_th[0][1, 2, 3] - bad) > 1e-3
+
+
+# ------------------------------------------------------------------------------------------------
+# P4  vacuum and pure gauge stay put
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("m,s", [(1, 1), (2, 0)])
+def test_vacuum_stays_vacuum(oracle, m, s):
+    p = oracle.Params(N=6, m=m, s=s)
+    f = np.zeros((10, 6, 6, 6)); f[0] = p.sigma
+    g = oracle.step(p, f.copy(), 0, 25)
+    assert np.array_equal(g, f)                    # bitwise
+    d = oracle.diagnostics(p, g, 25)
+    assert d["n_pierced"] == 0 and math.isinf(d["xi"]) and d["gauss_max"] == 0.0
+
+
+def test_pure_gauge_is_static(oracle):
+    """phi = sigma e^{i alpha}, theta_i = q (alpha^{x+k_i} - alpha^x): U phi^{x+k} = phi^x and every Xi = 0."""
+    for q in (+1, -1):
+        p = oracle.Params(N=6, m=1, s=1, q=q)
+        rng = np.random.default_rng(1)
+        al = rng.uniform(-3, 3, (6, 6, 6))
+        phi = p.sigma * np.exp(1j * al)
+        th = [q * (sh(al, i, 1) - al) for i in range(3)]
+        z = np.zeros((6, 6, 6))
+        f = pack(phi, z + 0j, th, [z, z, z])
+        g = oracle.step(p, f.copy(), 0, 10)
+        assert np.abs(g - f).max() < 5e-15
+        assert oracle.diagnostics(p, g, 10)["n_pierced"] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# P5 / P6  symplectic structure at a = 1: energy and time reversal
+# ------------------------------------------------------------------------------------------------
+def staggered_energy(oracle, p, f_prev, f_next):
+    """H at level n with the staggered-product kinetic terms Re[conj(Pi^{n-1/2}) Pi^{n+1/2}] and
+    eps^{n-1/2} eps^{n+1/2} / (2 e^2 dx^2); potential part from the oracle's Eq. 2 with Pi = eps = 0."""
+    pot = f_prev.copy(); pot[2:4] = 0; pot[7:10] = 0
+    U = -oracle.site_fields(p, pot, 0)[2].sum()
+    kin = (f_prev[2] * f_next[2] + f_prev[3] * f_next[3]).sum()
+    kin += sum((f_prev[7 + i] * f_next[7 + i]).sum() for i in range(3)) / (2 * p.e0 ** 2 * p.dx ** 2)
+    return U + kin
+
+
+def energy_spread(oracle, dt, nsteps):
+    p = oracle.Params(N=8, m=0, s=1, dt=dt)
+    f = oracle.initial_condition(p, seed=2)
+    hs = []
+    for n in range(nsteps):
+        prev = f.copy()
+        oracle.step(p, f, n, 1)
+        hs.append(staggered_energy(oracle, p, prev, f))
+    hs = np.array(hs)
+    drift = (hs[-nsteps // 4:].mean() - hs[: nsteps // 4].mean()) / hs.mean()
+    return (hs.max() - hs.min()) / hs.mean(), drift
+
+
+def test_energy_conserved_in_undamped_limit(oracle):
+    """north_star: 'Energy must be conserved in the a=1 undamped limit'.  A leapfrog conserves a shadow
+    Hamiltonian: bounded O(dt^2) oscillation, no secular drift.  Catches a kick/drift ordering error and any
+    force that is not a gradient."""
+    s1, _ = energy_spread(oracle, 0.1, 200)
+    s2, _ = energy_spread(oracle, 0.05, 400)
+    s3, _ = energy_spread(oracle, 0.025, 800)
+    assert s1 < 2e-2
+    assert 3.0 < s1 / s2 < 5.0 and 3.0 < s2 / s3 < 5.0, (s1, s2, s3)     # error of the shadow Hamiltonian ~ dt^2
+
+
+def test_time_reversal(oracle):
+    p = oracle.Params(N=6, m=0, s=1)
+    f0 = oracle.initial_condition(p, seed=9)
+    f = oracle.step(p, f0.copy(), 0, 30)
+    # snapshot holds phi^30, Pi^{29.5}: step phi, theta back by one drift so that they sit at level 29,
+    # negate the momenta (now "Pi^{29 + 1/2}" seen backwards) and run 29 more steps.
+    f[0] -= p.dt * f[2]; f[1] -= p.dt * f[3]
+    for i in range(3):
+        f[4 + i] -= p.dt * f[7 + i]
+    f[2:4] *= -1; f[7:10] *= -1
+    oracle.step(p, f, 0, 29)
+    assert np.abs(f[0:2] - f0[0:2]).max() < 1e-12 and np.abs(f[4:7] - f0[4:7]).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# P7  lattice symmetries
+# ------------------------------------------------------------------------------------------------
+def test_translation_and_axis_swap(oracle):
+    """Catches direction bookkeeping errors in curl/plaquettes and periodic wrap errors."""
+    p = oracle.Params(N=6, m=1, s=1)
+    rng = np.random.default_rng(3)
+    f = random_state(6, rng)
+    ref = oracle.step(p, f.copy(), 0, 5)
+    # translation by (dx,dy,dz) = (2,5,1)
+    tr = lambda a: np.roll(a, (1, 5, 2), axis=(-3, -2, -1))
+    got = oracle.step(p, np.ascontiguousarray(tr(f)), 0, 5)
+    assert np.array_equal(got, tr(ref))
+    # swap x <-> y: arrays transpose, theta_0 <-> theta_1, eps_0 <-> eps_1
+    def swap(a):
+        b = np.swapaxes(a, -1, -2).copy()
+        b[[4, 5]] = b[[5, 4]]; b[[7, 8]] = b[[8, 7]]
+        return np.ascontiguousarray(b)
+    got = oracle.step(p, swap(f), 0, 5)
+    assert np.abs(got - swap(ref)).max() < 1e-14       # the j-sum runs in a different order
+    # swap x <-> z
+    def swapz(a):
+        b = np.swapaxes(a, -1, -3).copy()
+        b[[4, 6]] = b[[6, 4]]; b[[7, 9]] = b[[9, 7]]
+        return np.ascontiguousarray(b)
+    got = oracle.step(p, swapz(f), 0, 5)
+    assert np.abs(got - swapz(ref)).max() < 1e-14
+    d0, d1 = oracle.diagnostics(p, ref, 5), oracle.diagnostics(p, swapz(ref), 5)
+    assert d0["n_pierced"] == d1["n_pierced"]
+    assert d0["v2_num"] == pytest.approx(d1["v2_num"], rel=1e-12) and d0["v2_den"] == pytest.approx(d1["v2_den"], rel=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# P8  linear dispersion at a = 1
+# ------------------------------------------------------------------------------------------------
+def test_dispersion_relation_static_background(oracle):
+    """Around phi = sigma: a transverse gauge wave theta_1 ~ sin(k x) and a radial wave phi = sigma(1 + d sin(k x))
+    obey theta^{n+1} - 2 theta^n + theta^{n-1} = -dt^2 (khat^2 + M^2) theta^n with khat = (2/dx) sin(k dx/2),
+    M^2 = 2 e0^2 sigma^2 (gauge) or lambda0 sigma^2 (radial).  Pins the 2 e^2 of d2, the lambda/2 of c3 and the
+    1/dx^2 of c2, d3."""
+    N = 8
+    p = oracle.Params(N=N, m=0, s=1, dx=0.5, dt=0.1, lambda0=1.7, e0=0.9, sigma=1.2)
+    k = TWO_PI * 2 / (N * p.dx)
+    khat2 = (2 / p.dx * math.sin(k * p.dx / 2)) ** 2
+    x = np.arange(N)[None, None, :] * np.ones((N, N, 1))
+    wave = 1e-7 * np.sin(k * p.dx * x)
+    for which, M2 in (("gauge", 2 * p.e0 ** 2 * p.sigma ** 2), ("radial", p.lambda0 * p.sigma ** 2)):
+        f = np.zeros((10, N, N, N)); f[0] = p.sigma
+        if which == "gauge":
+            f[5] = wave; probe = lambda g: g[5][0, 0, 1]
+        else:
+            f[0] = p.sigma * (1 + wave); probe = lambda g: g[0][0, 0, 1] - p.sigma
+        hist = []
+        for n in range(12):
+            oracle.step(p, f, n, 1); hist.append(probe(f))
+        for n in range(2, 11):
+            lhs = (hist[n + 1] - 2 * hist[n] + hist[n - 1]) / hist[n]
+            assert lhs == pytest.approx(-p.dt ** 2 * (khat2 + M2), rel=2e-6), which
+
+
+# ------------------------------------------------------------------------------------------------
+# P18  linear modes in the radiation era against the closed form [A sin(W tau) + B cos(W tau)] / tau
+# ------------------------------------------------------------------------------------------------
+def test_linear_modes_in_radiation_era_closed_form(oracle):
+    """a ~ tau (m = 1), s = 0: chi = tau * delta is a free oscillator, chi'' + W^2 chi = 0, for the radial mode
+    (W^2 = khat^2 + lambda0 sigma^2) and the transverse gauge mode (W^2 = khat^2 + 2 e0^2 sigma^2), because
+    a^2 lambda(a) and a^2 e(a)^2 are constant at s = 0 and a''/a = 0.  The leapfrog is 2nd order, so with dt = 0.01
+    it must follow the closed form to ~1e-4; putting a scale factor at the wrong half-step (e.g. (a_n/a_{n-1/2})^2 in
+    c2 or d3, or a_{n+1/2} for a_{n-1/2} in c1 or d1) is a 1st-order error ~1e-2 and fails."""
+    N = 8
+    p = oracle.Params(N=N, m=1, s=0, dx=0.5, dt=0.01, lambda0=2.0, e0=1.0, sigma=1.0, tau0=1.0)
+    k = TWO_PI / (N * p.dx)
+    khat2 = (2 / p.dx * math.sin(k * p.dx / 2)) ** 2
+    x = np.arange(N)[None, None, :] * np.ones((N, N, 1))
+    shape = np.sin(k * p.dx * x)
+    amp = 1e-7
+    nsteps = 300
+    for which, M2 in (("radial", p.lambda0 * p.sigma ** 2), ("gauge", 2 * p.e0 ** 2 * p.sigma ** 2)):
+        W = math.sqrt(khat2 + M2)
+        A, B = 0.7, -0.4
+        delta = lambda t: (A * math.sin(W * t) + B * math.cos(W * t)) / t
+        ddelta = lambda t: (W * (A * math.cos(W * t) - B * math.sin(W * t))) / t - delta(t) / t
+        f = np.zeros((10, N, N, N)); f[0] = p.sigma
+        th = p.tau0 - p.dt / 2
+        if which == "radial":
+            f[0] += amp * delta(p.tau0) * shape; f[2] = amp * ddelta(th) * shape
+            probe = lambda g: (g[0][0, 0, 2] - p.sigma) / (amp * shape[0, 0, 2])
+        else:
+            f[5] = amp * delta(p.tau0) * shape; f[8] = amp * ddelta(th) * shape
+            probe = lambda g: g[5][0, 0, 2] / (amp * shape[0, 0, 2])
+        err = 0.0
+        for n in range(nsteps):
+            oracle.step(p, f, n, 1)
+            err = max(err, abs(probe(f) - delta(p.tau0 + (n + 1) * p.dt)))
+        assert err < 3e-4, (which, err)
+
+
+def test_homogeneous_mode_with_physical_width_bessel(oracle):
+    """m = 1, s = 1: a^2 lambda(a) = lambda0 tau^2 / tau_ref^2.  Small homogeneous radial oscillation:
+    chi = tau * delta obeys chi'' + M^2 tau^2 chi = 0, M = sqrt(lambda0) sigma / tau_ref, solved by
+    sqrt(tau) J_{+-1/4}(M tau^2 / 2).  Pins the power of a in c3 (a_n^4 / a_{n+1/2}^2) at s = 1."""
+    from scipy.special import jv
+    N = 4
+    p = oracle.Params(N=N, m=1, s=1, dx=0.5, dt=0.005, lambda0=2.0, sigma=1.0, tau0=1.0, tau_ref=1.0)
+    M = math.sqrt(p.lambda0) * p.sigma
+    A, B = 0.6, 0.8
+    chi = lambda t: math.sqrt(t) * (A * jv(0.25, M * t * t / 2) + B * jv(-0.25, M * t * t / 2))
+    delta = lambda t: chi(t) / t
+    h = 1e-5
+    ddelta = lambda t: (delta(t + h) - delta(t - h)) / (2 * h)
+    amp = 1e-7
+    f = np.zeros((10, N, N, N))
+    f[0] = p.sigma * (1 + amp * delta(p.tau0)); f[2] = p.sigma * amp * ddelta(p.tau0 - p.dt / 2)
+    err = 0.0
+    for n in range(400):
+        oracle.step(p, f, n, 1)
+        err = max(err, abs((f[0][0, 0, 0] / p.sigma - 1) / amp - delta(p.tau0 + (n + 1) * p.dt)))
+    assert err < 3e-4, err
+
+
+# ------------------------------------------------------------------------------------------------
+# P9  homogeneous mode = scalar recurrence (non-linear; pins c1, c3 and the schedule for all (m, s))
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("m,s", [(1, 0), (1, 1), (2, 0), (2, 1)])
+def test_homogeneous_mode_scalar_recurrence(oracle, m, s):
+    p = oracle.Params(N=4, m=m, s=s, lambda0=1.9, sigma=1.1, tau0=1.5)
+    f = np.zeros((10, 4, 4, 4)); f[0] = 0.3
+    fs, ps = 0.3, 0.0
+    for n in range(40):
+        oracle.step(p, f, n, 1)
+        tau = p.tau0 + n * p.dt
+        am, a0, ap = (tau - p.dt / 2) ** m, tau ** m, (tau + p.dt / 2) ** m    # tau_ref-independent ratios:
+        norm = p.tau0 ** m                                                   # a = (tau/tau0)^m
+        am, a0, ap = am / norm, a0 / norm, ap / norm
+        lam = p.lambda0 * a0 ** (2 * (s - 1))
+        ps = (am / ap) ** 2 * ps - p.dt * (a0 ** 2 / ap) ** 2 * lam / 2 * (fs * fs - p.sigma ** 2) * fs
+        fs = fs + p.dt * ps
+        assert np.ptp(f[0]) == 0.0 and not f[1].any() and not f[4:].any()
+        assert f[0][0, 0, 0] == pytest.approx(fs, rel=1e-13) and f[2][0, 0, 0] == pytest.approx(ps, rel=1e-12, abs=1e-15)
+
+
+# ------------------------------------------------------------------------------------------------
+# P10  hand-built straight string-antistring pair on 16^3 (north_star)
+# ------------------------------------------------------------------------------------------------
+def string_pair(N=16):
+    z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    th = np.arctan2(y - 7.5, x - 3.5) - np.arctan2(y - 7.5, x - 11.5)
+    zero = np.zeros((N, N, N))
+    return pack(np.exp(1j * th), zero + 0j, [zero] * 3, [zero] * 3)
+
+
+def test_string_antistring_pair_gives_exactly_2N_pierced_plaquettes(oracle):
+    N = 16
+    p = oracle.Params(N=N)
+    f = string_pair(N)
+    cnt, tot, W = oracle.winding(p, f, want_w=True)
+    assert cnt == 2 * N and tot == 2 * N
+    assert not W[1].any() and not W[2].any()                 # only xy-plaquettes are pierced
+    # one string of each orientation per z-slice, at the plaquettes based at (3,7) and (11,7)
+    for z in range(N):
+        nz = np.argwhere(W[0][z] != 0)
+        assert sorted(map(tuple, nz)) == [(7, 3), (7, 11)]
+        assert W[0][z][7, 3] == -W[0][z][7, 11] and abs(W[0][z][7, 3]) == 1
+    # orientation: phase winds by +2 pi counter-clockwise around (3.5, 7.5) -> W_xy = +1 there
+    assert W[0][0][7, 3] == +1
+    d = oracle.diagnostics(p, f, 0)
+    assert d["L"] == pytest.approx(math.pi / 6 * 0.5 * 32)
+    # the same pair along x instead of z: pierces yz-plaquettes
+    g = np.ascontiguousarray(np.swapaxes(f, -1, -3))
+    cnt, tot, W = oracle.winding(p, g, want_w=True)
+    assert cnt == 2 * N and not W[0].any() and not W[1].any()
+
+
+# ------------------------------------------------------------------------------------------------
+# P11  random lattice gauge transformation (north_star)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("q", [+1, -1])
+def test_gauge_invariance_of_diagnostics(oracle, q):
+    p = oracle.Params(N=10, m=1, s=0, q=q)
+    f = oracle.initial_condition(p, seed=21)
+    oracle.step(p, f, 0, 40)
+    phi, Pi, th, eps = unpack(f)
+    rng = np.random.default_rng(0)
+    al = rng.uniform(-10, 10, (10, 10, 10))
+    g = pack(phi * np.exp(1j * al), Pi * np.exp(1j * al), [th[i] + q * (sh(al, i, 1) - al) for i in range(3)], eps)
+    c0, t0, W0 = oracle.winding(p, f, want_w=True)
+    c1, t1, W1 = oracle.winding(p, g, want_w=True)
+    assert c0 > 0 and np.array_equal(W0, W1) and (c0, t0) == (c1, t1)
+    d0, d1 = oracle.diagnostics(p, f, 40), oracle.diagnostics(p, g, 40)
+    for key in ("v2_num", "v2_den", "v2", "mean_lagrangian"):
+        assert d1[key] == pytest.approx(d0[key], rel=1e-11), key
+    assert abs(d1["gauss_max"] - d0["gauss_max"]) < 1e-13
+    # and the evolution commutes with the transformation
+    fa = oracle.step(p, f.copy(), 40, 5); ga = oracle.step(p, g.copy(), 40, 5)
+    pa, _, tha, _ = unpack(fa); pg, _, thg, _ = unpack(ga)
+    assert np.abs(pg - pa * np.exp(1j * al)).max() < 1e-12
+    assert max(np.abs(thg[i] - tha[i] - q * (sh(al, i, 1) - al)).max() for i in range(3)) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# P12  charge conjugation: the printed Eqs. 4-5 (q = -1) and the pinned form (q = +1) are one dynamics
+# ------------------------------------------------------------------------------------------------
+def test_charge_conjugation(oracle):
+    pp = oracle.Params(N=6, m=1, s=1, q=+1)
+    pm = oracle.Params(N=6, m=1, s=1, q=-1)
+    f = oracle.initial_condition(pp, seed=4)
+    a = oracle.step(pp, f.copy(), 0, 15)
+    b = oracle.step(pm, f.copy(), 0, 15)                 # same IC, other convention
+    assert np.array_equal(a[0:4], b[0:4])                # phi, Pi identical
+    assert np.array_equal(a[4:], -b[4:])                 # theta, eps sign-flipped
+    fc = f.copy(); fc[1] *= -1                           # conj(phi) IC
+    c = oracle.step(pm, fc, 0, 15)
+    assert np.array_equal(c[0], a[0]) and np.array_equal(c[1], -a[1]) and np.array_equal(c[4:], a[4:])
+    assert oracle.winding(pp, a) == oracle.winding(pm, b)
+    da, db = oracle.diagnostics(pp, a, 15), oracle.diagnostics(pm, b, 15)
+    assert da["v2_num"] == db["v2_num"] and da["gauss_max"] == db["gauss_max"]
+
+
+# ------------------------------------------------------------------------------------------------
+# P13  Eq. 11 literally, in floating point
+# ------------------------------------------------------------------------------------------------
+def test_winding_literal_equation_11(oracle):
+    """Y_i = [arg(phi^{x+k_i}) - arg(phi^x) - q theta_i]_pi + q theta_i ; W = (Y_i^x + Y_j^{x+k_i} - Y_i^{x+k_j} - Y_j^x)/2pi."""
+    for q in (+1, -1):
+        p = oracle.Params(N=10, m=1, s=0, q=q)
+        f = oracle.initial_condition(p, seed=33)
+        oracle.step(p, f, 0, 30)
+        phi, _, th, _ = unpack(f)
+        arg = np.angle(phi)
+        wrap = lambda d: d - TWO_PI * np.rint(d / TWO_PI)
+        Y = [wrap(sh(arg, i, 1) - arg - q * th[i]) + q * th[i] for i in range(3)]
+        _, _, W = oracle.winding(p, f, want_w=True)
+        assert np.count_nonzero(W) > 50
+        for pl, (i, j) in enumerate([(0, 1), (0, 2), (1, 2)]):
+            lit = (Y[i] + sh(Y[j], i, 1) - sh(Y[i], j, 1) - Y[j]) / TWO_PI
+            assert np.abs(lit - W[pl]).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# P17  Eq. 2 / Eq. 10: closed forms and an independent vectorised evaluation
+# ------------------------------------------------------------------------------------------------
+def test_lagrangian_closed_forms(oracle):
+    N = 6
+    p = oracle.Params(N=N, m=1, s=0.5, dx=0.5, lambda0=1.7, e0=0.9, sigma=1.1, tau0=1.0, tau_ref=0.5)
+    n = 10
+    a = ((p.tau0 + n * p.dt) / 0.5) ** 1
+    e2a2 = p.e0 ** 2 * a ** (2 * p.s)                       # e(a)^2 a^2 = e0^2 a^(2s)
+    one = np.ones((N, N, N))
+    # (a) uniform fields: Lag = sum eps^2/(2 e^2 a^2 dx^2) + |Pi|^2 - (lambda0 a^(2s)/4)(f^2 - sigma^2)^2, G = 0
+    f = pack(0.7 * one + 0j, (0.2 - 0.3j) * one, [0 * one] * 3, [0.1 * one, -0.2 * one, 0.3 * one])
+    K, G, L = oracle.site_fields(p, f, n)
+    want = 0.14 / (2 * e2a2 * 0.25) + 0.13 - p.lambda0 * a ** (2 * p.s) / 4 * (0.49 - 1.21) ** 2
+    assert np.allclose(G, 0, atol=1e-30) and np.allclose(K, 0.13, rtol=1e-15) and np.allclose(L, want, rtol=1e-14)
+    # (b) plane wave phi = sigma e^{i k x}: G = khat^2 sigma^2
+    k = TWO_PI * 2 / N
+    x = np.arange(N)[None, None, :] * one
+    f = pack(p.sigma * np.exp(1j * k * x), 0j * one, [0 * one] * 3, [0 * one] * 3)
+    K, G, L = oracle.site_fields(p, f, n)
+    khat2 = (2 / p.dx * math.sin(k / 2)) ** 2
+    assert np.allclose(G, khat2 * p.sigma ** 2, rtol=1e-13) and np.allclose(L, -G, rtol=1e-13)
+    # ... and the same wave is gradient-free if the link carries the phase: theta_0 = q k  => U phi^{x+1} = phi^x
+    f = pack(p.sigma * np.exp(1j * k * x), 0j * one, [k * one, 0 * one, 0 * one], [0 * one] * 3)
+    assert np.allclose(oracle.site_fields(p, f, n)[1], 0, atol=1e-28)
+    # (c) uniform magnetic flux through xy plaquettes: theta_1 = B x with B = 2 pi / N (seam consistent mod 2 pi)
+    B = TWO_PI / N
+    f = pack(p.sigma * one + 0j, 0j * one, [0 * one, B * x, 0 * one], [0 * one] * 3)
+    K, G, L = oracle.site_fields(p, f, n)
+    Gw = (2 - 2 * np.cos(B * x)) * p.sigma ** 2 / p.dx ** 2          # |e^{-i B x} - 1|^2 sigma^2 / dx^2
+    mag = 2 * (1 - math.cos(B)) / (p.dx ** 2 * 2 * e2a2 * p.dx ** 2)  # ordered pairs (0,1),(1,0); c_B = 1
+    assert np.allclose(G, Gw, rtol=1e-13, atol=1e-15) and np.allclose(L, -mag - Gw, rtol=1e-13)
+
+
+def test_diagnostics_against_vectorised_numpy(oracle):
+    p = oracle.Params(N=12, m=2, s=0.5, e0=0.9, lambda0=1.7, dx=0.6)
+    f = oracle.initial_condition(p, seed=8)
+    oracle.step(p, f, 0, 25)
+    K, G, L = np_site_fields(p, f, 25)
+    Ko, Go, Lo = oracle.site_fields(p, f, 25)
+    assert np.abs(K - Ko).max() < 1e-13 and np.abs(G - Go).max() < 1e-12 and np.abs(L - Lo).max() < 1e-11
+    d = oracle.diagnostics(p, f, 25)
+    assert d["v2_num"] == pytest.approx((K * L).sum(), rel=1e-11)
+    assert d["v2_den"] == pytest.approx((G * L).sum(), rel=1e-11)
+    R = (K * L).sum() / (G * L).sum()
+    assert d["v2"] == pytest.approx(2 * R / (1 + R), rel=1e-10)
+    assert d["mean_lagrangian"] == pytest.approx(L.mean(), rel=1e-11)
+    assert d["nonfinite"] == 0
+    f[3][1, 2, 3] = np.nan
+    assert oracle.diagnostics(p, f, 25)["nonfinite"] == 1
+
+
+def test_v2_of_a_boosted_field_is_v_squared(oracle):
+    """Eq. 9-10: for a field translating rigidly, phi(x - v t), with |phi-dot|^2 = v^2 |d_x phi|^2 pointwise,
+    R = v^2 <(d_x phi)^2 X>/<(D phi)^2 X> ; with gradients only along x, R = v^2 and <v^2> = 2 v^2/(1 + v^2)
+    for ANY weight X.  Pins the estimator's ratio and the 2R/(1+R) map."""
+    N = 16
+    p = oracle.Params(N=N, m=0, s=1)
+    x = np.arange(N)[None, None, :] * np.ones((N, N, 1))
+    k = TWO_PI / N
+    phi = 1.0 + 0.3 * np.sin(k * x) + 0.2j * np.cos(2 * k * x)
+    v = 0.37
+    Pi = -v * (sh(phi, 0, 1) - phi) / p.dx            # -v * forward difference: same stencil as D_0 phi
+    zero = np.zeros((N, N, N))
+    d = oracle.diagnostics(p, pack(phi, Pi, [zero] * 3, [zero] * 3), 0)
+    assert d["v2_num"] / d["v2_den"] == pytest.approx(v * v, rel=1e-12)
+    assert d["v2"] == pytest.approx(2 * v * v / (1 + v * v), rel=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# G3 / R3: the documented stability window of the literal a = (tau/tau0)^m reading
+# ------------------------------------------------------------------------------------------------
+def test_config1_literal_reading_leaves_stability_region(oracle):
+    """DESIGN.md R3: dt^2 (12/dx^2 + lambda0 sigma^2 a^(2s)) < 4 fails for a > 13.3 at s = 1 (dx=.5, dt=.1): config 1 run
+    literally (tau_ref = tau0 = 1, a = tau) is finite at step 60 and not at step 100; with s = 0 it is stable."""
+    p = oracle.Params(N=8, m=1, s=1)
+    f = oracle.initial_condition(p, seed=1)
+    oracle.step(p, f, 0, 60)
+    assert np.isfinite(f).all() and np.abs(f[0:2]).max() < 3
+    oracle.step(p, f, 60, 60)
+    assert (not np.isfinite(f).all()) or np.abs(f[0:2]).max() > 1e3
+    p0 = oracle.Params(N=8, m=1, s=0)
+    f = oracle.initial_condition(p0, seed=1)
+    oracle.step(p0, f, 0, 200)
+    assert np.isfinite(f).all() and np.abs(f[0:2]).max() < 3
