@@ -1,0 +1,176 @@
+/*
+ * ahs.h -- C ABI of libahs: the data-parallel hot path of arXiv 1809.00995 (Correia & Martins,
+ * "Abelian-Higgs Cosmic String Evolution with CUDA") on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations are PAPER.md line numbers; "R<n>" = readings in DESIGN.md):
+ *   - the damped staggered-leapfrog update, Eqs. 4-7 (L55-L62), of a complex scalar phi and its
+ *     momentum Pi on the sites and of the U(1) link angles theta_i and their conjugates eps_i on the
+ *     links of a periodic N^3 comoving lattice, with a(tau) = (tau/tau_ref)^m (L224, R3) and the
+ *     core-width parameter s of Eq. 8 (L68): e(a) = e0 a^(s-1), lambda(a) = lambda0 a^(2(s-1));
+ *   - the network diagnostics: plaquette winding, Eq. 11 (L88-L93), giving the string length
+ *     L = (pi/6) dx n_pierced and xi = sqrt((N dx)^3 / L); the Lagrangian-weighted mean square velocity,
+ *     Eqs. 9-10 with the weight of Eq. 2 (L40, L78-L86); and the residual of the discrete Gauss law
+ *     (L72, L181; R4).
+ *
+ * Variables.  The stored "A" and "E" are the paper's rescaled link variables (L44, R5):
+ *     theta_i = e0 * dx * A_i   (dimensionless link angle, U_i^x = exp(-i theta_i^x), R1)
+ *     eps_i   = d theta_i / d eta.
+ * A field snapshot "after n steps" is { phi^n, theta^n at tau_n = tau0 + n dt ; Pi^(n-1/2), eps^(n-1/2) }.
+ * Fields cross this boundary as 10 contiguous arrays of N^3 values in the order
+ *     phi_re, phi_im, Pi_re, Pi_im, theta_0, theta_1, theta_2, eps_0, eps_1, eps_2
+ * with site index  x + N*(y + N*z)  (x fastest; direction 0,1,2 = x,y,z; theta_i^x sits on the link
+ * from x to x + k_i).
+ *
+ * Pointers.  Every pointer argument says HOST or DEVICE.  The caller owns every host pointer it passes.
+ * The library owns the device memory it allocates; if ahs_params.device_buffer is given the caller owns
+ * it and frees it after ahs_destroy.  All work of a handle is issued on the handle's CUDA stream;
+ * ahs_step is asynchronous, every function that returns data to the host synchronises that stream.
+ * A handle is not thread-safe; distinct handles are independent (replicas).
+ *
+ * Errors.  Functions returning int return AHS_OK (0) or a negative code; ahs_last_error() returns a
+ * thread-local, statically stored, human readable message for the last failure on the calling thread.
+ * There is no CPU fallback and no other backend: without a CUDA device every call that needs one fails
+ * with AHS_ERR_CUDA.
+ */
+#ifndef AHS_H_
+#define AHS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define AHS_API __attribute__((visibility("default")))
+#else
+#define AHS_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ahs_sim ahs_sim; /* opaque handle */
+
+enum { AHS_OK = 0, AHS_ERR_INVALID_ARG = -1, AHS_ERR_OOM = -2, AHS_ERR_CUDA = -3, AHS_ERR_NONFINITE = -4, AHS_ERR_STATE = -5 };
+enum { AHS_F32 = 0, AHS_F64 = 1 };                                   /* storage AND arithmetic type of the step */
+enum { AHS_IC_RANDOM_PHASE = 0, AHS_IC_GAUSSIAN = 1, AHS_IC_NONE = 2 /* all fields zero; set them with ahs_set_fields */ };
+enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
+
+/*
+ * Parameters of a simulation (L36: lambda, e, sigma; L51: dx, dt; L68-70: s; L224: a ~ eta^m; L72: IC).
+ *   N               lattice is N^3, periodic.  N >= 4 (ahs_create_ex); the z-marching kernel needs N % 128 == 0
+ *                   (fp32) or N % 64 == 0 (fp64) and is chosen automatically when it applies.
+ *   dx, dt          lattice spacing and conformal time step, > 0.
+ *   lambda, e, sigma  lambda_0, e_0 of Eq. 8 and the vacuum expectation value, > 0.
+ *   m               a(tau) = (tau/tau_ref)^m : 0 static, 1 radiation, 2 matter.
+ *   s               Eq. 8: 0 = constant comoving core width, 1 = true equations of motion.
+ *   tau0            conformal time of step 0; tau0 - dt/2 > 0 is required when m != 0.
+ *   tau_ref         normalisation of a (R3); 0 means tau0, i.e. a(tau0) = 1.
+ *   seed            Philox4x32-10 key (lo 32 bits, hi 32 bits); counter = (site lo, site hi, 0, 0)  (R9).
+ *   precision       AHS_F32 or AHS_F64.
+ *   ic_kind         AHS_IC_RANDOM_PHASE: phi = sigma exp(2 pi i u), Pi = theta = eps = 0 (L72);
+ *                   AHS_IC_GAUSSIAN: re, im ~ N(0, sigma^2/2) by Box-Muller; AHS_IC_NONE: zeros.
+ *   kernel          AHS_KERNEL_AUTO, or force one of the two step/diagnostics implementations.
+ *   device_buffer   DEVICE pointer, optional (NULL => the library calls cudaMalloc).  Must hold
+ *                   ahs_required_bytes(N, precision) bytes, 256-byte aligned (e.g. torch.empty(...).data_ptr()).
+ *   stream          cudaStream_t as void*, optional (NULL => the legacy default stream).
+ */
+typedef struct {
+    int32_t N;
+    int32_t precision;
+    int32_t ic_kind;
+    int32_t kernel;
+    double dx, dt, lambda, e, sigma, m, s, tau0, tau_ref;
+    uint64_t seed;
+    void* device_buffer;
+    size_t device_buffer_bytes;
+    void* stream;
+} ahs_params;
+
+/* Result of one diagnostics pass on the current snapshot (after `step` steps). */
+typedef struct {
+    int64_t step;             /* n                                                                         */
+    double tau;               /* tau_n = tau0 + n dt                                                       */
+    uint64_t n_pierced;       /* plaquettes with W != 0, Eq. 11 (L88-93), bit-exact integer                */
+    uint64_t sum_abs_w;       /* sum |W| over the 3 N^3 plaquettes                                         */
+    double L;                 /* (pi/6) dx n_pierced (L93)                                                 */
+    double xi;                /* sqrt((N dx)^3 / L); +inf if n_pierced == 0                                */
+    double v2_num;            /* sum_x |Pi|^2 Lag^x     (Eq. 10, weight = Eq. 2 with c_B = 1, R2)          */
+    double v2_den;            /* sum_x |D phi|^2 Lag^x                                                     */
+    double v2;                /* 2R/(1+R), R = v2_num / v2_den (Eq. 9)                                     */
+    double mean_lagrangian;   /* sum_x Lag^x / N^3                                                         */
+    double gauss_max;         /* max_x |sum_i (eps_i^x - eps_i^{x-k_i}) - 2 dx^2 e0^2 a_h^(2s) Im[conj(phi) Pi]|,
+                                 a_h = a(tau_n - dt/2)  (R4)                                               */
+    double gauss_rhs_rms;     /* rms_x of the second term: the scale gauss_max is to be compared with      */
+    int32_t nonfinite;        /* 1 if any stored field value is NaN or +-inf                               */
+    int32_t reserved;
+} ahs_diag;
+
+/* Bytes of device memory a simulation needs: 15 arrays of N^3 values (10 live + the phi', theta' shadow
+ * buffers of the double-buffered drift) plus reduction scratch.  0 if N or precision is invalid. */
+AHS_API size_t ahs_required_bytes(int32_t N, int32_t precision);
+
+/* north_star signature: fp32, random-phase IC (L72), a = (tau/tau0)^m, default stream, library-owned
+ * memory on the current device.  Returns NULL on failure (see ahs_last_error). */
+AHS_API ahs_sim* ahs_create(int32_t N, double dx, double dt, double lambda, double e, double sigma,
+                    double m, double s, double tau0, uint64_t seed);
+
+/* General constructor.  params: HOST pointer.  Returns NULL on failure. */
+AHS_API ahs_sim* ahs_create_ex(const ahs_params* params);
+
+/* n >= 0 leapfrog steps (Eqs. 4-7), one fused kernel launch per step, asynchronous on the handle's
+ * stream; the six coefficients of Eqs. 4-5 are computed on the host in fp64 from tau_n and passed as
+ * kernel arguments. */
+AHS_API int32_t ahs_step(ahs_sim* sim, int32_t n);
+
+/* Diagnostics of the current snapshot.  L, v2, gauss: HOST pointers, any may be NULL.
+ * L = (pi/6) dx n_pierced; v2 = <v^2>_L; gauss = max |Gauss residual| (absolute).
+ * Synchronises.  Returns AHS_ERR_NONFINITE (outputs still filled) if a field value is not finite. */
+AHS_API int32_t ahs_diagnostics(ahs_sim* sim, double* L, double* v2, double* gauss);
+AHS_API int32_t ahs_diagnostics_ex(ahs_sim* sim, ahs_diag* out /* HOST */);
+
+/* Launch the diagnostics kernels without reading the result back (asynchronous; for timing). The result
+ * is fetched by the next ahs_diagnostics_fetch.  */
+AHS_API int32_t ahs_diagnostics_launch(ahs_sim* sim);
+AHS_API int32_t ahs_diagnostics_fetch(ahs_sim* sim, ahs_diag* out /* HOST */);
+
+/* Copy the snapshot to / from HOST memory as doubles: host10 holds 10*N^3 doubles in the field order above.
+ * ahs_set_fields rounds to the storage precision and sets the step counter (tau = tau0 + step*dt). Synchronise. */
+AHS_API int32_t ahs_get_fields(ahs_sim* sim, double* host10);
+AHS_API int32_t ahs_set_fields(ahs_sim* sim, const double* host10, int64_t step);
+
+/* The same in the storage type (float for AHS_F32, double for AHS_F64): 10*N^3 values, no conversion, one
+ * cudaMemcpyAsync per field on the handle's stream followed by a synchronise. Pinned host memory makes
+ * the copies run at PCIe speed. */
+AHS_API int32_t ahs_get_fields_native(ahs_sim* sim, void* host10);
+AHS_API int32_t ahs_set_fields_native(ahs_sim* sim, const void* host10, int64_t step);
+
+/* DEVICE pointer to live field k (0..9, order above) in the storage type; valid until the next ahs_step
+ * (phi and theta alternate between two buffers).  For zero-copy views from PyTorch. */
+AHS_API int32_t ahs_field_device_ptr(ahs_sim* sim, int32_t k, void** dev_ptr /* HOST pointer to a DEVICE pointer */);
+
+/* Counters: step n, tau_n, and the number of kernels launched by this handle so far. */
+AHS_API int32_t ahs_get_state(ahs_sim* sim, int64_t* step, double* tau, int64_t* kernel_launches);
+
+/* Which implementation the handle uses: AHS_KERNEL_GENERIC or AHS_KERNEL_MARCH. */
+AHS_API int32_t ahs_kernel_kind(ahs_sim* sim);
+
+/* The six coefficients (c1, c2, c3, d1, d2, d3) of Eqs. 4-5 for the step n -> n+1, as the host computes
+ * them. out6: HOST. */
+AHS_API int32_t ahs_coefficients(ahs_sim* sim, int64_t n, double* out6);
+
+/* Block until all work of the handle has finished. */
+AHS_API int32_t ahs_synchronize(ahs_sim* sim);
+
+/* Free the handle and the device memory the library allocated. NULL is allowed. */
+AHS_API int32_t ahs_destroy(ahs_sim* sim);
+
+/* Message of the last failure on this thread ("" if none). Never NULL. */
+AHS_API const char* ahs_last_error(void);
+
+/* Library version string, e.g. "ahs 0.1 sm_100a". */
+AHS_API const char* ahs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AHS_H_ */

@@ -1,0 +1,441 @@
+// ahs_api.cu -- the C ABI of include/ahs.h: handle, SoA lattice store in HBM, per-step coefficient
+// schedule (host, fp64), kernel dispatch, host<->device field transfer.  No torch types here: PyTorch (if the
+// caller uses it) only supplies a device buffer and a stream through ahs_params.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ahs_internal.cuh"
+
+using namespace ahs;
+
+struct ahs_sim {
+    ahs_params p;
+    int64_t nsites;
+    size_t elem;             // sizeof storage type
+    size_t array_bytes;      // bytes of one field array, rounded up to 256
+    char* base;              // device buffer
+    bool owns_buffer;
+    cudaStream_t stream;
+    int cur;                 // which (phi, theta) buffer holds level n
+    int64_t step;
+    int64_t launches;
+    int kernel;              // AHS_KERNEL_GENERIC or AHS_KERNEL_MARCH
+    DiagPartial* partials;   // device, kMaxDiagPartials records
+    DiagPartial* result;     // device, 1 record
+    DiagPartial* result_host;  // pinned host, 1 record
+    int64_t diag_step;       // step the pending diagnostics launch refers to (-1: none)
+    int device;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define AHS_CUDA(call)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) return fail(AHS_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+size_t round256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+bool valid_N(int32_t N) { return N >= 4 && N <= 2048; }
+
+size_t scratch_bytes() { return round256(sizeof(DiagPartial) * (size_t)(kMaxDiagPartials + 1)); }
+
+template <typename T> T* slot(const ahs_sim* s, int k) { return reinterpret_cast<T*>(s->base + (size_t)k * s->array_bytes); }
+
+// live slot of user-facing field k (0..9: phi_re, phi_im, Pi_re, Pi_im, theta_0..2, eps_0..2)
+int live_slot(const ahs_sim* s, int k)
+{
+    const int b = s->cur ? PHI_RE1 : PHI_RE0;
+    switch (k) {
+        case 0: return b + 0;
+        case 1: return b + 1;
+        case 2: return PI_RE;
+        case 3: return PI_IM;
+        case 4: case 5: case 6: return b + 2 + (k - 4);
+        default: return EPS0 + (k - 7);
+    }
+}
+
+// ---- the scale factor and couplings (Eq. 8; R3) --------------------------------------------
+double tau_of(const ahs_params& p, int64_t n) { return p.tau0 + (double)n * p.dt; }
+double scale_factor(const ahs_params& p, double tau)
+{
+    const double tref = (p.tau_ref != 0.0) ? p.tau_ref : p.tau0;
+    return std::pow(tau / tref, p.m);
+}
+double e_of(const ahs_params& p, double a) { return p.e * std::pow(a, p.s - 1.0); }
+double lambda_of(const ahs_params& p, double a) { return p.lambda * std::pow(a, 2.0 * (p.s - 1.0)); }
+
+// Coefficients of Eqs. 4-5 for the step n -> n+1 (L55-57): scale factors at tau_n -+ dt/2 and tau_n.
+StepCoef step_coefficients(const ahs_params& p, int64_t n)
+{
+    const double tau = tau_of(p, n);
+    const double a_m = scale_factor(p, tau - 0.5 * p.dt), a_0 = scale_factor(p, tau), a_p = scale_factor(p, tau + 0.5 * p.dt);
+    const double e_m = e_of(p, a_m), e_0 = e_of(p, a_0), e_p = e_of(p, a_p);
+    StepCoef c;
+    const double r_mp = a_m / a_p, r_0p = a_0 / a_p, q_0p = a_0 * a_0 / a_p;
+    c.c1 = r_mp * r_mp;                                       // (a_{n-1/2}/a_{n+1/2})^2
+    c.c2 = p.dt / (p.dx * p.dx) * r_0p * r_0p;                // dt/dx^2 (a_n/a_{n+1/2})^2
+    c.c3 = p.dt * q_0p * q_0p * lambda_of(p, a_0) * 0.5;      // dt (a_n^2/a_{n+1/2})^2 lambda_n/2
+    c.d1 = (e_p / e_m) * (e_p / e_m);                         // (e_{n+1/2}/e_{n-1/2})^2
+    c.d2 = 2.0 * p.dt * a_0 * a_0 * e_p * e_p;                // 2 dt a_n^2 e_{n+1/2}^2
+    c.d3 = p.dt / (p.dx * p.dx) * (e_p / e_0) * (e_p / e_0);  // dt/dx^2 (e_{n+1/2}/e_n)^2
+    c.dt = p.dt;
+    c.sigma2 = p.sigma * p.sigma;
+    return c;
+}
+
+DiagCoef diag_coefficients(const ahs_params& p, int64_t n)
+{
+    const double tau = tau_of(p, n);
+    const double a = scale_factor(p, tau), a_h = scale_factor(p, tau - 0.5 * p.dt);
+    const double ea = e_of(p, a);
+    DiagCoef c;
+    c.inv_dx2 = 1.0 / (p.dx * p.dx);
+    c.gauge_norm = 1.0 / (2.0 * ea * ea * a * a * p.dx * p.dx);
+    c.cB_inv_dx2 = 1.0 / (p.dx * p.dx);
+    c.pot_coef = 0.25 * a * a * lambda_of(p, a);
+    c.sigma2 = p.sigma * p.sigma;
+    c.gauss_rhs = 2.0 * p.dx * p.dx * p.e * p.e * std::pow(a_h, 2.0 * p.s);
+    return c;
+}
+
+template <typename T>
+int do_step(ahs_sim* s)
+{
+    FieldPtrs<T> f;
+    const int in = s->cur ? PHI_RE1 : PHI_RE0, out = s->cur ? PHI_RE0 : PHI_RE1;
+    f.phi_re = slot<T>(s, in); f.phi_im = slot<T>(s, in + 1);
+    f.phi_re_out = slot<T>(s, out); f.phi_im_out = slot<T>(s, out + 1);
+    for (int i = 0; i < 3; ++i) {
+        f.th[i] = slot<T>(s, in + 2 + i);
+        f.th_out[i] = slot<T>(s, out + 2 + i);
+        f.eps[i] = slot<T>(s, EPS0 + i);
+    }
+    f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
+    const StepCoef c = step_coefficients(s->p, s->step);
+    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->stream)
+                                         : launch_step_generic<T>(f, s->p.N, c, s->stream);
+}
+
+template <typename T>
+int do_diag(ahs_sim* s)
+{
+    DiagPtrs<T> f;
+    const int in = s->cur ? PHI_RE1 : PHI_RE0;
+    f.phi_re = slot<T>(s, in); f.phi_im = slot<T>(s, in + 1);
+    for (int i = 0; i < 3; ++i) { f.th[i] = slot<T>(s, in + 2 + i); f.eps[i] = slot<T>(s, EPS0 + i); }
+    f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
+    const DiagCoef c = diag_coefficients(s->p, s->step);
+    return s->kernel == AHS_KERNEL_MARCH
+               ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream)
+               : launch_diag_generic<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream);
+}
+
+int check_sim(const ahs_sim* s)
+{
+    if (!s) return fail(AHS_ERR_INVALID_ARG, "null handle");
+    return AHS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ahs_last_error(void) { return g_err; }
+const char* ahs_version(void) { return "ahs 0.1 sm_100a"; }
+
+size_t ahs_required_bytes(int32_t N, int32_t precision)
+{
+    if (!valid_N(N) || (precision != AHS_F32 && precision != AHS_F64)) return 0;
+    const size_t elem = precision == AHS_F32 ? 4 : 8;
+    const size_t nsites = (size_t)N * N * N;
+    return (size_t)NUM_SLOTS * round256(nsites * elem) + scratch_bytes();
+}
+
+ahs_sim* ahs_create_ex(const ahs_params* params)
+{
+    g_err[0] = 0;
+    if (!params) { fail(AHS_ERR_INVALID_ARG, "params is NULL"); return nullptr; }
+    const ahs_params& p = *params;
+    if (!valid_N(p.N)) { fail(AHS_ERR_INVALID_ARG, "N = %d out of range [4, 2048]", p.N); return nullptr; }
+    if (p.precision != AHS_F32 && p.precision != AHS_F64) { fail(AHS_ERR_INVALID_ARG, "precision must be AHS_F32 or AHS_F64"); return nullptr; }
+    if (p.ic_kind < AHS_IC_RANDOM_PHASE || p.ic_kind > AHS_IC_NONE) { fail(AHS_ERR_INVALID_ARG, "unknown ic_kind %d", p.ic_kind); return nullptr; }
+    if (!(p.dx > 0) || !(p.dt > 0) || !(p.lambda > 0) || !(p.e > 0) || !(p.sigma > 0)) {
+        fail(AHS_ERR_INVALID_ARG, "dx, dt, lambda, e, sigma must be > 0"); return nullptr;
+    }
+    if (!std::isfinite(p.m) || !std::isfinite(p.s) || !std::isfinite(p.tau0) || !std::isfinite(p.tau_ref) || p.tau_ref < 0) {
+        fail(AHS_ERR_INVALID_ARG, "m, s, tau0 must be finite and tau_ref >= 0"); return nullptr;
+    }
+    if (p.m != 0.0 && !(p.tau0 - 0.5 * p.dt > 0)) { fail(AHS_ERR_INVALID_ARG, "tau0 - dt/2 must be > 0 when m != 0"); return nullptr; }
+    if (p.kernel < AHS_KERNEL_AUTO || p.kernel > AHS_KERNEL_MARCH) { fail(AHS_ERR_INVALID_ARG, "unknown kernel %d", p.kernel); return nullptr; }
+    const bool march_ok = p.precision == AHS_F32 ? march_supported<float>(p.N) : march_supported<double>(p.N);
+    if (p.kernel == AHS_KERNEL_MARCH && !march_ok) {
+        fail(AHS_ERR_INVALID_ARG, "the z-marching kernel needs N %% %d == 0 (N = %d)", p.precision == AHS_F32 ? 128 : 64, p.N);
+        return nullptr;
+    }
+
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "no CUDA device: %s (libahs has no CPU fallback)", cudaGetErrorString(ce)); return nullptr; }
+
+    ahs_sim* s = new (std::nothrow) ahs_sim();
+    if (!s) { fail(AHS_ERR_OOM, "host allocation failed"); return nullptr; }
+    s->p = p;
+    s->nsites = (int64_t)p.N * p.N * p.N;
+    s->elem = p.precision == AHS_F32 ? 4 : 8;
+    s->array_bytes = round256((size_t)s->nsites * s->elem);
+    s->stream = (cudaStream_t)p.stream;
+    s->cur = 0; s->step = 0; s->launches = 0; s->diag_step = -1; s->device = dev;
+    s->kernel = (p.kernel == AHS_KERNEL_AUTO) ? (march_ok ? AHS_KERNEL_MARCH : AHS_KERNEL_GENERIC) : p.kernel;
+    s->result_host = nullptr;
+
+    const size_t need = ahs_required_bytes(p.N, p.precision);
+    if (p.device_buffer) {
+        if (p.device_buffer_bytes < need || ((uintptr_t)p.device_buffer & 255)) {
+            fail(AHS_ERR_INVALID_ARG, "device_buffer must hold %zu bytes and be 256-byte aligned", need);
+            delete s; return nullptr;
+        }
+        s->base = (char*)p.device_buffer; s->owns_buffer = false;
+    } else {
+        size_t free_b = 0, total_b = 0;
+        ce = cudaMemGetInfo(&free_b, &total_b);
+        if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMemGetInfo: %s", cudaGetErrorString(ce)); delete s; return nullptr; }
+        if (need > free_b) { fail(AHS_ERR_OOM, "need %zu bytes of device memory, %zu free", need, free_b); delete s; return nullptr; }
+        void* ptr = nullptr;
+        ce = cudaMalloc(&ptr, need);
+        if (ce != cudaSuccess) { cudaGetLastError(); fail(AHS_ERR_OOM, "cudaMalloc(%zu): %s", need, cudaGetErrorString(ce)); delete s; return nullptr; }
+        s->base = (char*)ptr; s->owns_buffer = true;
+    }
+    s->partials = reinterpret_cast<DiagPartial*>(s->base + (size_t)NUM_SLOTS * s->array_bytes);
+    s->result = s->partials + kMaxDiagPartials;
+    ce = cudaMallocHost((void**)&s->result_host, sizeof(DiagPartial));
+    if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMallocHost: %s", cudaGetErrorString(ce)); ahs_destroy(s); return nullptr; }
+
+    // initial condition (L72): everything zero, then phi from Philox
+    ce = cudaMemsetAsync(s->base, 0, (size_t)NUM_SLOTS * s->array_bytes, s->stream);
+    if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(ce)); ahs_destroy(s); return nullptr; }
+    if (p.ic_kind != AHS_IC_NONE) {
+        const int r = p.precision == AHS_F32
+                          ? launch_ic<float>(slot<float>(s, PHI_RE0), slot<float>(s, PHI_IM0), p.N, p.sigma, p.seed, p.ic_kind, s->stream)
+                          : launch_ic<double>(slot<double>(s, PHI_RE0), slot<double>(s, PHI_IM0), p.N, p.sigma, p.seed, p.ic_kind, s->stream);
+        if (r < 0) { fail(AHS_ERR_CUDA, "IC kernel launch: %s", cudaGetErrorString(cudaGetLastError())); ahs_destroy(s); return nullptr; }
+        s->launches += r;
+    }
+    return s;
+}
+
+ahs_sim* ahs_create(int32_t N, double dx, double dt, double lambda, double e, double sigma, double m, double s, double tau0, uint64_t seed)
+{
+    ahs_params p;
+    std::memset(&p, 0, sizeof(p));
+    p.N = N; p.precision = AHS_F32; p.ic_kind = AHS_IC_RANDOM_PHASE; p.kernel = AHS_KERNEL_AUTO;
+    p.dx = dx; p.dt = dt; p.lambda = lambda; p.e = e; p.sigma = sigma; p.m = m; p.s = s; p.tau0 = tau0; p.tau_ref = 0.0;
+    p.seed = seed;
+    return ahs_create_ex(&p);
+}
+
+int32_t ahs_step(ahs_sim* s, int32_t n)
+{
+    if (int r = check_sim(s)) return r;
+    if (n < 0) return fail(AHS_ERR_INVALID_ARG, "n must be >= 0");
+    for (int32_t k = 0; k < n; ++k) {
+        const int r = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
+        if (r < 0) return fail(r, "step kernel launch failed at step %lld: %s", (long long)s->step, cudaGetErrorString(cudaGetLastError()));
+        s->launches += r;
+        s->cur ^= 1;
+        s->step += 1;
+    }
+    return AHS_OK;
+}
+
+int32_t ahs_diagnostics_launch(ahs_sim* s)
+{
+    if (int r = check_sim(s)) return r;
+    const int r = s->p.precision == AHS_F32 ? do_diag<float>(s) : do_diag<double>(s);
+    if (r < 0) return fail(r, "diagnostics kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    s->launches += r;
+    s->diag_step = s->step;
+    return AHS_OK;
+}
+
+int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
+{
+    if (int r = check_sim(s)) return r;
+    if (!out) return fail(AHS_ERR_INVALID_ARG, "out is NULL");
+    if (s->diag_step < 0) return fail(AHS_ERR_STATE, "no diagnostics launch is pending");
+    AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    const DiagPartial& r = *s->result_host;
+    const ahs_params& p = s->p;
+    std::memset(out, 0, sizeof(*out));
+    out->step = s->diag_step;
+    out->tau = tau_of(p, s->diag_step);
+    out->n_pierced = r.n_pierced;
+    out->sum_abs_w = r.sum_abs_w;
+    out->L = (M_PI / 6.0) * p.dx * (double)r.n_pierced;                     // L93
+    const double box = (double)p.N * p.dx;
+    out->xi = r.n_pierced ? std::sqrt(box * box * box / out->L) : INFINITY; // L88
+    out->v2_num = r.num;
+    out->v2_den = r.den;
+    const double R = r.num / r.den;                                          // Eq. 10
+    out->v2 = 2.0 * R / (1.0 + R);                                           // Eq. 9
+    out->mean_lagrangian = r.lsum / (double)s->nsites;
+    out->gauss_max = r.gmax;
+    out->gauss_rhs_rms = std::sqrt(r.rhs2 / (double)s->nsites);
+    out->nonfinite = r.nonfinite ? 1 : 0;
+    s->diag_step = -1;
+    if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "%llu sites hold a non-finite field value at step %lld",
+                                    (unsigned long long)r.nonfinite, (long long)out->step);
+    return AHS_OK;
+}
+
+int32_t ahs_diagnostics_ex(ahs_sim* s, ahs_diag* out)
+{
+    if (!out) return fail(AHS_ERR_INVALID_ARG, "out is NULL");
+    if (int r = ahs_diagnostics_launch(s)) return r;
+    return ahs_diagnostics_fetch(s, out);
+}
+
+int32_t ahs_diagnostics(ahs_sim* s, double* L, double* v2, double* gauss)
+{
+    ahs_diag d;
+    const int r = ahs_diagnostics_ex(s, &d);
+    if (r != AHS_OK && r != AHS_ERR_NONFINITE) return r;
+    if (L) *L = d.L;
+    if (v2) *v2 = d.v2;
+    if (gauss) *gauss = d.gauss_max;
+    return r;
+}
+
+int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
+{
+    if (int r = check_sim(s)) return r;
+    if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
+    const size_t bytes = (size_t)s->nsites * s->elem;
+    for (int k = 0; k < 10; ++k)
+        AHS_CUDA(cudaMemcpyAsync((char*)host10 + (size_t)k * bytes, s->base + (size_t)live_slot(s, k) * s->array_bytes, bytes,
+                                 cudaMemcpyDeviceToHost, s->stream));
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    return AHS_OK;
+}
+
+int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
+{
+    if (int r = check_sim(s)) return r;
+    if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
+    if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
+    const size_t bytes = (size_t)s->nsites * s->elem;
+    for (int k = 0; k < 10; ++k)
+        AHS_CUDA(cudaMemcpyAsync(s->base + (size_t)live_slot(s, k) * s->array_bytes, (const char*)host10 + (size_t)k * bytes, bytes,
+                                 cudaMemcpyHostToDevice, s->stream));
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    s->step = step;
+    return AHS_OK;
+}
+
+// fp64 host interface: for AHS_F64 a straight copy; for AHS_F32 each field is converted on the device through
+// the (currently dead) shadow buffer of phi/theta, two arrays of which hold one N^3 array of doubles.
+int32_t ahs_get_fields(ahs_sim* s, double* host10)
+{
+    if (int r = check_sim(s)) return r;
+    if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
+    if (s->p.precision == AHS_F64) return ahs_get_fields_native(s, host10);
+    const int shadow = s->cur ? PHI_RE0 : PHI_RE1;   // 5 dead float arrays = room for 2 double arrays
+    double* stage = reinterpret_cast<double*>(s->base + (size_t)shadow * s->array_bytes);
+    const size_t bytes = (size_t)s->nsites * sizeof(double);
+    for (int k = 0; k < 10; ++k) {
+        const int r = launch_convert_to_double<float>(slot<float>(s, live_slot(s, k)), stage, s->nsites, s->stream);
+        if (r < 0) return fail(AHS_ERR_CUDA, "convert kernel: %s", cudaGetErrorString(cudaGetLastError()));
+        s->launches += r;
+        AHS_CUDA(cudaMemcpyAsync(host10 + (size_t)k * s->nsites, stage, bytes, cudaMemcpyDeviceToHost, s->stream));
+    }
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    return AHS_OK;
+}
+
+int32_t ahs_set_fields(ahs_sim* s, const double* host10, int64_t step)
+{
+    if (int r = check_sim(s)) return r;
+    if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
+    if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
+    if (s->p.precision == AHS_F64) return ahs_set_fields_native(s, host10, step);
+    const int shadow = s->cur ? PHI_RE0 : PHI_RE1;
+    double* stage = reinterpret_cast<double*>(s->base + (size_t)shadow * s->array_bytes);
+    const size_t bytes = (size_t)s->nsites * sizeof(double);
+    for (int k = 0; k < 10; ++k) {
+        AHS_CUDA(cudaMemcpyAsync(stage, host10 + (size_t)k * s->nsites, bytes, cudaMemcpyHostToDevice, s->stream));
+        const int r = launch_convert_from_double<float>(stage, slot<float>(s, live_slot(s, k)), s->nsites, s->stream);
+        if (r < 0) return fail(AHS_ERR_CUDA, "convert kernel: %s", cudaGetErrorString(cudaGetLastError()));
+        s->launches += r;
+    }
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    s->step = step;
+    return AHS_OK;
+}
+
+int32_t ahs_field_device_ptr(ahs_sim* s, int32_t k, void** dev_ptr)
+{
+    if (int r = check_sim(s)) return r;
+    if (k < 0 || k > 9 || !dev_ptr) return fail(AHS_ERR_INVALID_ARG, "field index must be 0..9 and dev_ptr non-NULL");
+    *dev_ptr = s->base + (size_t)live_slot(s, k) * s->array_bytes;
+    return AHS_OK;
+}
+
+int32_t ahs_get_state(ahs_sim* s, int64_t* step, double* tau, int64_t* kernel_launches)
+{
+    if (int r = check_sim(s)) return r;
+    if (step) *step = s->step;
+    if (tau) *tau = tau_of(s->p, s->step);
+    if (kernel_launches) *kernel_launches = s->launches;
+    return AHS_OK;
+}
+
+int32_t ahs_kernel_kind(ahs_sim* s)
+{
+    if (int r = check_sim(s)) return r;
+    return s->kernel;
+}
+
+int32_t ahs_coefficients(ahs_sim* s, int64_t n, double* out6)
+{
+    if (int r = check_sim(s)) return r;
+    if (!out6 || n < 0) return fail(AHS_ERR_INVALID_ARG, "out6 is NULL or n < 0");
+    const StepCoef c = step_coefficients(s->p, n);
+    out6[0] = c.c1; out6[1] = c.c2; out6[2] = c.c3; out6[3] = c.d1; out6[4] = c.d2; out6[5] = c.d3;
+    return AHS_OK;
+}
+
+int32_t ahs_synchronize(ahs_sim* s)
+{
+    if (int r = check_sim(s)) return r;
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
+    return AHS_OK;
+}
+
+int32_t ahs_destroy(ahs_sim* s)
+{
+    if (!s) return AHS_OK;
+    cudaStreamSynchronize(s->stream);
+    if (s->result_host) cudaFreeHost(s->result_host);
+    if (s->owns_buffer && s->base) cudaFree(s->base);
+    delete s;
+    return AHS_OK;
+}
+
+}  // extern "C"

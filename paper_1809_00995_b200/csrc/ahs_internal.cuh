@@ -1,0 +1,77 @@
+// ahs_internal.cuh -- private declarations shared by the translation units of libahs (CUDA, sm_100a).
+// Nothing here is shared with oracle/ (test infrastructure): the two paths have no common code.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ahs.h"
+
+namespace ahs {
+
+// Field slots inside the device buffer.  phi and theta are double-buffered ("cur" = 0/1) so that one
+// fused kernel can kick Pi, eps in place and write the drifted phi', theta' without a race
+// (Eqs. 4-7 need phi^n, theta^n of the neighbours while phi^{n+1} is being produced).
+enum Slot {
+    PHI_RE0 = 0, PHI_IM0, TH0_0, TH1_0, TH2_0,   // buffer 0 of (phi, theta)
+    PHI_RE1, PHI_IM1, TH0_1, TH1_1, TH2_1,       // buffer 1
+    PI_RE, PI_IM, EPS0, EPS1, EPS2,              // single-buffered momenta
+    NUM_SLOTS
+};
+
+// The six per-step scalars of Eqs. 4-5 (host, fp64) plus constants, passed by value to the kernels.
+struct StepCoef {
+    double c1, c2, c3, d1, d2, d3;   // Eq. 4: c1 damping, c2 Laplacian, c3 Higgs force; Eq. 5: d1, d2 current, d3 curl
+    double dt;                        // Eqs. 6-7
+    double sigma2;                    // sigma^2
+};
+
+// Constants of the diagnostics pass for the snapshot after n steps.
+struct DiagCoef {
+    double inv_dx2;        // 1/dx^2
+    double gauge_norm;     // 1 / (2 e(a)^2 a^2 dx^2) with a = a(tau_n)     (Eq. 2 prefactor)
+    double cB_inv_dx2;     // c_B / dx^2, c_B = 1 (R2)
+    double pot_coef;       // a^2 lambda(a) / 4
+    double sigma2;
+    double gauss_rhs;      // 2 dx^2 e0^2 a_h^(2s), a_h = a(tau_n - dt/2)  (R4)
+};
+
+// One record per block / final result of the reduction (fixed 8 x 8 bytes).
+struct DiagPartial {
+    unsigned long long n_pierced;
+    unsigned long long sum_abs_w;
+    double num, den, lsum;
+    double gmax;
+    double rhs2;
+    unsigned long long nonfinite;
+};
+
+template <typename T>
+struct FieldPtrs {
+    const T* phi_re; const T* phi_im; const T* th[3];   // level n (read only)
+    T* phi_re_out; T* phi_im_out; T* th_out[3];         // level n+1 (other buffer)
+    T* pi_re; T* pi_im; T* eps[3];                      // in place
+};
+
+template <typename T>
+struct DiagPtrs {
+    const T* phi_re; const T* phi_im; const T* th[3];
+    const T* pi_re; const T* pi_im; const T* eps[3];
+};
+
+// ---- kernel launchers (each returns the number of kernels it launched, or a negative ahs error) -------------
+template <typename T> int launch_ic(T* phi_re, T* phi_im, int N, double sigma, uint64_t seed, int kind, cudaStream_t st);
+template <typename T> int launch_step_generic(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st);
+template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st);
+template <typename T> bool march_supported(int N);
+template <typename T> int launch_diag_generic(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
+                                              int max_partials, DiagPartial* result, cudaStream_t st);
+template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
+                                            int max_partials, DiagPartial* result, cudaStream_t st);
+int launch_diag_finish(const DiagPartial* partials, int n, DiagPartial* result, cudaStream_t st);
+template <typename T> int launch_convert_from_double(const double* src, T* dst, int64_t n, cudaStream_t st);
+template <typename T> int launch_convert_to_double(const T* src, double* dst, int64_t n, cudaStream_t st);
+
+static const int kMaxDiagPartials = 1 << 16;
+
+}  // namespace ahs

@@ -1,0 +1,311 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 CPU oracle, element by element on the same
+seeded inputs.  Needs a B200: run with -m gpu.
+
+Tolerances (BASELINE.json north_star; definitions DESIGN.md "Tolerances"):
+  fp64 fields after 20 steps : max_x |gpu - oracle| / max(1, max_x |oracle|) <= 1e-12 per field array
+  fp32 fields after 20 steps : max_x |gpu - oracle| / max(1, max_x |oracle|) <= 2e-4 per field array
+  winding                    : bit-exact on identical snapshots (produced by the oracle, uploaded with ahs_set_fields)
+  <v^2> sums                 : fp64 1e-10 relative, fp32 2e-5 relative to sum |K Lag|, sum |G Lag|
+  Gauss residual             : at roundoff of the storage type on both paths
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-4}
+
+
+@pytest.fixture(scope="module")
+def ahs():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1809_00995_b200 import binding
+    binding.load()
+    return binding
+
+
+def field_errors(got, ref):
+    return [np.abs(got[k] - ref[k]).max() / max(1.0, np.abs(ref[k]).max()) for k in range(10)]
+
+
+def oracle_params(O, sim):
+    q = dict(sim.params)
+    q.pop("seed")
+    return O.Params(**q)
+
+
+def check_diag(O, p, sim, prec, snap, n):
+    """Diagnostics on an identical snapshot.  `snap` comes from the ORACLE side (never from the CUDA path); it is
+    uploaded with ahs_set_fields (fp32 storage: the test rounds it to fp32 first so both sides see the same values)."""
+    if prec == "f32":
+        snap = snap.astype(np.float32).astype(np.float64)
+    sim.set_fields(snap, n)
+    d = sim.diagnostics()
+    r = O.diagnostics(p, snap, n)
+    assert d["step"] == n and d["tau"] == pytest.approx(p.tau0 + n * p.dt, rel=1e-15)
+    assert d["n_pierced"] == r["n_pierced"] and d["sum_abs_w"] == r["sum_abs_w"]          # bit-exact
+    assert d["L"] == pytest.approx(r["L"], rel=1e-14)
+    assert (math.isinf(d["xi"]) and math.isinf(r["xi"])) or d["xi"] == pytest.approx(r["xi"], rel=1e-14)
+    K, G, Lg = O.site_fields(p, snap, n)
+    rel = 1e-10 if prec == "f64" else 2e-5
+    assert abs(d["v2_num"] - r["v2_num"]) <= rel * np.abs(K * Lg).sum() + 1e-300
+    assert abs(d["v2_den"] - r["v2_den"]) <= rel * np.abs(G * Lg).sum() + 1e-300
+    assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= rel * np.abs(Lg).mean() + 1e-300
+    eps_m = 2.3e-16 if prec == "f64" else 6e-8
+    gscale = max(1.0, r["gauss_rhs_rms"], np.abs(snap[7:10]).max())
+    assert abs(d["gauss_max"] - r["gauss_max"]) <= 64 * eps_m * gscale
+    assert d["gauss_rhs_rms"] == pytest.approx(r["gauss_rhs_rms"], rel=1e-5, abs=1e-30)
+    assert d["nonfinite"] == r["nonfinite"] == 0
+    return d, r
+
+
+def rounded(f, prec):
+    return f.astype(np.float32).astype(np.float64) if prec == "f32" else f
+
+
+# ---------------------------------------------------------------------------------------------------------
+# initial condition
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,N", [("f64", 32), ("f32", 32), ("f32", 128), ("f64", 64)])
+@pytest.mark.parametrize("ic", ["random_phase", "gaussian"])
+def test_initial_condition_matches_oracle(ahs, oracle, prec, N, ic):
+    seed = 180900995
+    with ahs.Simulation(N=N, precision=prec, seed=seed, ic=ic, sigma=1.1) as sim:
+        got = sim.get_fields()
+    p = oracle.Params(N=N, sigma=1.1)
+    ref = oracle.initial_condition(p, seed, oracle.IC_GAUSSIAN if ic == "gaussian" else oracle.IC_RANDOM_PHASE)
+    assert not got[2:].any()
+    if prec == "f32":
+        ref32 = ref.astype(np.float32).astype(np.float64)
+        # fp64 sincos on the device may differ from glibc by an ulp of fp64 -> at most 1 ulp of fp32 after rounding
+        assert np.abs(got[:2] - ref32[:2]).max() <= 2.0 ** -23 * max(1.0, np.abs(ref[:2]).max())
+        assert np.mean(got[:2] == ref32[:2]) > 0.999
+    else:
+        assert np.abs(got[:2] - ref[:2]).max() <= 4e-16 * max(1.0, np.abs(ref[:2]).max())
+
+
+# ---------------------------------------------------------------------------------------------------------
+# fields after 20 steps from an identical uploaded snapshot (north_star)
+# ---------------------------------------------------------------------------------------------------------
+CASES = [
+    # N, precision, m, s, kernel
+    (32, "f64", 1.0, 1.0, "generic"),     # config 1
+    (32, "f32", 1.0, 0.0, "generic"),
+    (20, "f64", 2.0, 0.5, "generic"),     # ragged: N not a multiple of the block size, several blocks
+    (36, "f32", 2.0, 0.0, "generic"),
+    (64, "f64", 1.0, 1.0, "auto"),
+    (128, "f32", 1.0, 0.0, "auto"),       # config 2 / 4 physics at an oracle-sized lattice
+    (128, "f32", 2.0, 1.0, "auto"),       # config 3 physics (matter, s=1), 20 steps are inside the stable window
+]
+
+
+@pytest.mark.parametrize("N,prec,m,s,kernel", CASES)
+def test_fields_after_20_steps(ahs, oracle, N, prec, m, s, kernel):
+    from paper_1809_00995_b200 import synthetic
+    nsteps = 20 if N <= 64 else 6        # the oracle needs ~1 us per site-update
+    with ahs.Simulation(N=N, precision=prec, m=m, s=s, ic="none", kernel=kernel) as sim:
+        p = oracle_params(oracle, sim)
+        ref = rounded(oracle.initial_condition(p, synthetic.SEED_PRIMARY), prec)   # the oracle's IC, uploaded
+        sim.set_fields(ref, 0)
+        sim.step(nsteps)
+        got = sim.get_fields()
+        assert sim.step_count == nsteps
+        oracle.step(p, ref, 0, nsteps)
+        errs = field_errors(got, ref)
+        for k, e in enumerate(errs):
+            assert e <= TOL[prec], (oracle.FIELD_NAMES[k], e)
+        # Gauss's law on the device trajectory itself
+        d = sim.diagnostics()
+        assert d["gauss_max"] <= (1e-12 if prec == "f64" else 2e-5) * max(1.0, d["gauss_rhs_rms"])
+        check_diag(oracle, p, sim, prec, ref, nsteps)
+
+
+@pytest.mark.parametrize("N,prec,kernel", [(24, "f64", "generic"), (24, "f32", "generic"), (64, "f64", "auto"), (128, "f32", "auto")])
+def test_step_from_generic_snapshot(ahs, oracle, N, prec, kernel):
+    """All ten fields non-zero (theta, eps, Pi of order 0.3): exercises every term of Eqs. 4-5 from step one."""
+    from paper_1809_00995_b200 import synthetic
+    f0 = synthetic.random_snapshot(N, seed=77)
+    if prec == "f32":
+        f0 = f0.astype(np.float32).astype(np.float64)
+    nsteps = 3
+    with ahs.Simulation(N=N, precision=prec, m=1.0, s=1.0, ic="none", kernel=kernel, tau0=2.0) as sim:
+        p = oracle_params(oracle, sim)
+        sim.set_fields(f0, step=7)
+        assert np.array_equal(sim.get_fields(), f0)                 # round trip is exact
+        np.testing.assert_allclose(sim.coefficients(7), oracle.coeffs(p, 7), rtol=1e-14)
+        sim.step(nsteps)
+        got = sim.get_fields()
+        ref = oracle.step(p, f0.copy(), 7, nsteps)
+        for k, e in enumerate(field_errors(got, ref)):
+            assert e <= (1e-13 if prec == "f64" else 2e-5), (oracle.FIELD_NAMES[k], e)
+        check_diag(oracle, p, sim, prec, ref, 7 + nsteps)
+
+
+def test_march_and_generic_kernels_agree_on_device(ahs):
+    """The two CUDA implementations are independent code: they must agree to rounding at sizes the oracle cannot reach."""
+    for prec, N, tol in (("f32", 256, 2e-5), ("f64", 128, 1e-13)):
+        with ahs.Simulation(N=N, precision=prec, kernel="auto", seed=5) as a, \
+             ahs.Simulation(N=N, precision=prec, kernel="generic", seed=5) as b:
+            if a.kernel_kind != "march":
+                pytest.skip("z-marching kernel not available for this size")
+            a.step(10); b.step(10)
+            fa, fb = a.get_fields_native(), b.get_fields_native()
+            for k in range(10):
+                assert np.abs(fa[k] - fb[k]).max() <= tol * max(1.0, np.abs(fb[k]).max()), k
+            da, db = a.diagnostics(), b.diagnostics()
+            assert da["n_pierced"] > 0
+            if np.array_equal(fa, fb):
+                assert da["n_pierced"] == db["n_pierced"]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# config 1 in full: 100 steps, diagnostics every 10 (literal reading finite to step ~80; also tau_ref = 11)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tau_ref,last", [(0.0, 60), (11.0, 100)])
+def test_config1_series(ahs, oracle, tau_ref, last):
+    """Both paths run config 1 side by side from the oracle's IC; the series of diagnostics must agree."""
+    from paper_1809_00995_b200 import synthetic
+    kw = dict(N=32, precision="f64", m=1.0, s=1.0, tau_ref=tau_ref)
+    with ahs.Simulation(ic="none", **kw) as sim, ahs.Simulation(ic="none", **kw) as probe:
+        p = oracle_params(oracle, sim)
+        ref = oracle.initial_condition(p, synthetic.SEED_PRIMARY)
+        sim.set_fields(ref, 0)
+        for n in range(0, last + 1, 10):
+            if n:
+                sim.step(10)
+                oracle.step(p, ref, n - 10, 10)
+            d = sim.diagnostics()                               # the device's own trajectory
+            ro = oracle.diagnostics(p, ref, n)                  # the oracle's own trajectory
+            assert d["n_pierced"] == ro["n_pierced"]
+            assert d["xi"] == pytest.approx(ro["xi"], rel=1e-12)
+            assert d["gauss_max"] < 1e-12 * max(1.0, d["gauss_rhs_rms"])
+            K, G, Lg = oracle.site_fields(p, ref, n)
+            assert abs(d["v2_num"] - ro["v2_num"]) <= 1e-8 * np.abs(K * Lg).sum() + 1e-300
+            assert abs(d["v2_den"] - ro["v2_den"]) <= 1e-8 * np.abs(G * Lg).sum() + 1e-300
+            check_diag(oracle, p, probe, "f64", ref, n)         # identical snapshot: bit-exact winding
+            if n <= 20:
+                assert max(field_errors(sim.get_fields(), ref)) <= 1e-12
+
+
+def test_config1_literal_reading_goes_nonfinite_and_is_reported(ahs):
+    """DESIGN.md R3: config 1 read literally (a = tau) leaves the leapfrog stability region before step 100."""
+    with ahs.Simulation(N=32, precision="f64", m=1.0, s=1.0, seed=1) as sim:
+        sim.step(60)
+        assert sim.diagnostics()["nonfinite"] == 0
+        sim.step(60)
+        d = sim.diagnostics()
+        f = sim.get_fields()
+        assert d["nonfinite"] == 1 or np.abs(f[0:2]).max() > 1e3
+        if d["nonfinite"]:
+            with pytest.raises(ahs.AhsError) as e:
+                sim.diagnostics(allow_nonfinite=False)
+            assert e.value.code == ahs.AHS_ERR_NONFINITE
+
+
+# ---------------------------------------------------------------------------------------------------------
+# invariants on the device path itself (properties that hold at any size)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,N", [("f64", 32), ("f32", 128)])
+def test_vacuum_and_string_pair(ahs, oracle, prec, N):
+    with ahs.Simulation(N=N, precision=prec, ic="none", m=1.0, s=1.0) as sim:
+        f = np.zeros((10, N, N, N)); f[0] = 1.0
+        sim.set_fields(f, 0)
+        sim.step(5)
+        assert np.array_equal(sim.get_fields(), f)                # the vacuum stays the vacuum, bitwise
+        d = sim.diagnostics()
+        assert d["n_pierced"] == 0 and math.isinf(d["xi"]) and d["gauss_max"] == 0.0
+    M = 16 if N == 32 else N
+    if prec == "f64":
+        M = 16
+    z, y, x = np.meshgrid(np.arange(M), np.arange(M), np.arange(M), indexing="ij")
+    th = np.arctan2(y - (M / 2 - 0.5), x - (M / 4 - 0.5)) - np.arctan2(y - (M / 2 - 0.5), x - (3 * M / 4 - 0.5))
+    f = np.zeros((10, M, M, M)); f[0] = np.cos(th); f[1] = np.sin(th)
+    with ahs.Simulation(N=M, precision=prec, ic="none") as sim:
+        sim.set_fields(f, 0)
+        d = sim.diagnostics()
+        assert d["n_pierced"] == 2 * M and d["sum_abs_w"] == 2 * M       # north_star: exactly 2N pierced plaquettes
+        assert d["L"] == pytest.approx(math.pi / 6 * 0.5 * 2 * M)
+
+
+@pytest.mark.parametrize("prec,N", [("f64", 32), ("f32", 64)])
+def test_gauge_transformation_leaves_diagnostics_unchanged(ahs, oracle, prec, N):
+    from paper_1809_00995_b200 import synthetic
+    with ahs.Simulation(N=N, precision=prec, ic="none", m=1.0, s=0.0) as sim:
+        p = oracle_params(oracle, sim)
+        f = oracle.step(p, oracle.initial_condition(p, 3), 0, 30)
+        sim.set_fields(f, 30)
+        d0 = sim.diagnostics()
+        al = synthetic.gauge_angles(N, seed=9)
+        g = f.copy()
+        c, s_ = np.cos(al), np.sin(al)
+        g[0], g[1] = f[0] * c - f[1] * s_, f[0] * s_ + f[1] * c
+        g[2], g[3] = f[2] * c - f[3] * s_, f[2] * s_ + f[3] * c
+        for i in range(3):
+            g[4 + i] = f[4 + i] + (np.roll(al, -1, axis=2 - i) - al)
+        sim.set_fields(g, 30)
+        d1 = sim.diagnostics()
+        if prec == "f64":
+            assert d1["n_pierced"] == d0["n_pierced"] and d0["n_pierced"] > 0
+            assert d1["v2"] == pytest.approx(d0["v2"], rel=1e-9)
+        else:
+            # fp32 storage rounds the transformed fields: counts may move by a few ties, sums by ~1e-5
+            assert abs(int(d1["n_pierced"]) - int(d0["n_pierced"])) <= 1e-4 * d0["n_pierced"] + 2
+            assert d1["v2"] == pytest.approx(d0["v2"], rel=2e-3)
+
+
+def test_long_run_series_fp32_vs_oracle(ahs, oracle):
+    """north_star: long-run xi(tau) and <v^2> agree within 2 % (fp32 GPU vs fp64 oracle, config-2 physics, 48^3... here
+    at a size the oracle finishes in seconds; the 2 % criterion is applied to <v^2> where |den| is well away from 0)."""
+    N, nsteps, every = 48, 160, 20
+    with ahs.Simulation(N=N, precision="f32", ic="none", m=1.0, s=0.0, kernel="generic") as sim:
+        p = oracle_params(oracle, sim)
+        ref = rounded(oracle.initial_condition(p, 11), "f32")
+        sim.set_fields(ref, 0)
+        for n in range(every, nsteps + 1, every):
+            sim.step(every)
+            oracle.step(p, ref, n - every, every)
+            d = sim.diagnostics()
+            r = oracle.diagnostics(p, ref, n)
+            assert d["xi"] == pytest.approx(r["xi"], rel=0.02)
+            assert abs(int(d["n_pierced"]) - int(r["n_pierced"])) <= 0.02 * r["n_pierced"]
+            K, G, Lg = oracle.site_fields(p, ref, n)
+            if abs(r["v2_den"]) > 0.05 * np.abs(G * Lg).sum():
+                assert d["v2"] == pytest.approx(r["v2"], rel=0.02)
+            assert d["gauss_max"] < 5e-5 * max(1.0, d["gauss_rhs_rms"])
+        assert max(field_errors(sim.get_fields(), ref)) < 5e-3
+
+
+def test_native_transfer_and_device_pointers(ahs):
+    import torch
+    N = 32
+    with ahs.Simulation(N=N, precision="f32", seed=2) as sim:
+        sim.step(3)
+        a = sim.get_fields_native()
+        assert a.dtype == np.float32 and np.array_equal(a.astype(np.float64), sim.get_fields())
+        pinned = torch.empty((10, N, N, N), dtype=torch.float32).pin_memory()
+        sim.get_fields_native(pinned.data_ptr())
+        assert np.array_equal(pinned.numpy(), a)
+        sim.set_fields_native(pinned.data_ptr(), step=3)
+        assert np.array_equal(sim.get_fields_native(), a)
+        ptr = sim.field_device_ptr(0)
+        assert ptr != 0 and ptr % 256 == 0
+        st, tau, nl = sim.state()
+        assert st == 3 and tau == pytest.approx(1.3) and nl >= 4
+    # the plain north_star constructor: library-owned memory, default stream
+    h = ahs.create(32, 0.5, 0.1, 2.0, 1.0, 1.0, 1.0, 0.0, 1.0, 5)
+    lib = ahs.load()
+    import ctypes as C
+    assert lib.ahs_step(C.c_void_p(h), 2) == 0
+    L, v2, g = C.c_double(), C.c_double(), C.c_double()
+    assert lib.ahs_diagnostics(C.c_void_p(h), C.byref(L), C.byref(v2), C.byref(g)) == 0
+    assert L.value > 0 and g.value < 1e-5
+    ahs.destroy_raw(h)
+
+
+def test_create_rejects_bad_arguments(ahs):
+    for kw in (dict(N=2), dict(N=32, dt=0.0), dict(N=32, tau0=0.01, m=1.0), dict(N=32, precision="f32", kernel="march")):
+        with pytest.raises(ahs.AhsError):
+            ahs.Simulation(**kw)
