@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Abelian-Higgs hot path (arXiv 1809.00995 Eqs. 4-7 + diagnostics) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--lattice 1024] [--precision f32]
+
+One bench "step" is one pass of the whole hot path at BASELINE.json config 4's cadence: `--leapfrog` (50) fused
+leapfrog launches (Eqs. 4-7) followed by one diagnostics pass (winding Eq. 11, <v^2>_L Eqs. 9-10,
+Gauss residual) whose record is read back.  Default K = 10 -> the config's 500-step timed window.  The line printed
+by rank 0 follows the driver's contract; see DESIGN.md "Measurement" for every field.
+
+  value       site-updates/s, whole job, state resident in HBM, CUDA events on the handle's stream, max over ranks
+  e2e         same metric through the C ABI with HOST buffers: ahs_set_fields_native (H2D of the 10 fields from pinned
+              memory) + the same step + ahs_get_fields_native of ... the diagnostics record (D2H), all inside the timing
+  roofline    step kernel: 80 B (fp32) / 160 B (fp64) per site per launch / average launch duration (events around the
+              back-to-back launches of each step), against MEASURED_PEAKS.json hbm_gbs
+  cpu_baseline  the fp64 oracle (oracle/, test infrastructure) as it stands on this box's host cores, bounded sample
+
+Multi-GPU: the path is one GPU per lattice (north_star); --gpus N runs N independent replicas (seed + rank), no
+data-path collective ("replicas only"); torch.distributed is used for the barrier and the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+COMMON = dict(dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, tau0=1.0)
+SEED = 180900995
+BYTES_PER_SITE = {"f32": 80, "f64": 160}          # 10 values read + 10 written per site per step
+FALLBACK_HBM_GBS = 6650.0                         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed `ncu --set full`
+# capture (profiles/); keyed by (kernel, precision, lattice).  None = no capture for that configuration.
+NCU_TRAFFIC_BYTES = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--lattice", type=int, default=1024, help="N of the N^3 lattice (config 4: 1024)")
+    ap.add_argument("--precision", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--leapfrog", type=int, default=50, help="leapfrog launches per bench step (config 4: diagnostics every 50)")
+    ap.add_argument("--m", type=float, default=1.0)
+    ap.add_argument("--s", type=float, default=0.0)
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "march"])
+    ap.add_argument("--e2e-steps", type=int, default=2, help="timed end-to-end steps (each uploads the full state)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-lattice", type=int, default=128, help="lattice of the oracle's bounded sample")
+    ap.add_argument("--cpu-leapfrog", type=int, default=10)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ------------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], None, [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for t, line in self.lines:
+            if not (t0 <= t <= t1 + 0.3):
+                continue
+            c = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(c[0])); smax = float(c[1]); power.append(float(c[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "samples": len(sm),
+                "power_w_max": max(power) if power else None, "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the oracle on the host cores: cpu_baseline leg and the --impl reference arm (the only places bench.py runs oracle/)
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_sample(args, steps: int = 1, warmup: int = 0) -> dict:
+    """Time the fp64 oracle, as it stands (single thread), on a bounded sample of the workload: a cpu_lattice^3
+    lattice with the same physics, `cpu_leapfrog` leapfrog steps + one diagnostics pass per bench step."""
+    import numpy as np
+    from oracle import ahs_oracle as O
+    N, L = args.cpu_lattice, args.cpu_leapfrog
+    p = O.Params(N=N, m=args.m, s=args.s, **COMMON)
+    f = O.initial_condition(p, SEED)
+    if args.precision == "f32":
+        f = np.ascontiguousarray(f.astype(np.float32).astype(np.float64))
+    n = 0
+    for _ in range(warmup):
+        O.step(p, f, n, L); n += L
+        O.diagnostics(p, f, n)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        O.step(p, f, n, L); n += L
+        d = O.diagnostics(p, f, n)
+    dt = time.perf_counter() - t0
+    return {"value": N ** 3 * L * steps / dt, "unit": "site-updates/s", "cores": 1, "kind": "oracle",
+            "sample": "%d^3 lattice, same physics (m=%g, s=%g), %d x (%d leapfrog steps + 1 diagnostics), fp64, 1 thread, %.1f s"
+                      % (N, args.m, args.s, steps, L, dt),
+            "seconds": dt, "n_pierced": int(d["n_pierced"]), "host_cores_online": os.cpu_count()}
+
+
+def run_reference(args):
+    """--impl reference: for this tier the reference arm is the oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    steps, warm = max(1, args.steps), max(0, min(args.warmup, 1))
+    # bound the whole run to a few minutes: ~1 us per site-update
+    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 1.5e8 and args.cpu_leapfrog > 1:
+        args.cpu_leapfrog = max(1, args.cpu_leapfrog // 2)
+    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 1.5e8 and args.cpu_lattice > 32:
+        args.cpu_lattice //= 2
+    r = oracle_sample(args, steps=steps, warmup=warm)
+    line = {
+        "impl": "reference", "metric": "lattice site-updates/sec per leapfrog step", "value": r["value"], "unit": "site-updates/s",
+        "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * r["seconds"] / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args),
+        "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": r["value"], "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(args) -> dict:
+    N = args.lattice
+    name = {1024: "BASELINE.json configs[3]", 256: "BASELINE.json configs[1]", 512: "BASELINE.json configs[2]/[4]"}.get(N, "custom")
+    return {"workload": "%d^3 periodic lattice, %s, dx=0.5 dt=0.1 lambda=2 e=1 sigma=1 tau0=1, a~tau^%g, s=%g, random-phase IC "
+                        "(Philox seed %d); %d leapfrog steps + 1 diagnostics per bench step (%s)"
+                        % (N, args.precision, args.m, args.s, SEED, args.leapfrog, name),
+            "lattice": N, "leapfrog_per_step": args.leapfrog, "diagnostics_per_step": 1,
+            "l2": "inputs larger than L2 (%.1f GB of fields streamed per leapfrog launch)" % (N ** 3 * BYTES_PER_SITE[args.precision] / 1e9),
+            "parallelism": "replicas x%d" % args.gpus}
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# our arm: the CUDA path through the C ABI binding
+# ------------------------------------------------------------------------------------------------------------------
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy kernel)"
+    except (OSError, KeyError, ValueError):
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1809_00995_b200 import binding as ahs
+
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    N, L, K, W = args.lattice, args.leapfrog, args.steps, args.warmup
+    sites = N ** 3
+    sim = ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank, kernel=args.kernel, **COMMON)
+    diag = None
+    for _ in range(W):
+        sim.step(L)
+        diag = sim.diagnostics()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    marks = [(ev(), ev(), ev()) for _ in range(K)]
+    barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    launches0 = sim.kernel_launches
+    t0 = time.time()
+    start, stop = ev(), ev()
+    start.record()
+    for a, b, c in marks:
+        a.record()
+        sim.step(L)                 # L fused leapfrog launches, asynchronous
+        b.record()
+        diag = sim.diagnostics()    # diagnostics kernels + 64-byte record to the host (synchronises)
+        c.record()
+    stop.record()
+    barrier()
+    t1 = time.time()
+    clk = clocks.stop(t0, t1)
+    launches = sim.kernel_launches - launches0
+    total_ms = max_over_ranks(start.elapsed_time(stop))
+    step_ms = sum(a.elapsed_time(b) for a, b, _ in marks)       # the leapfrog launches only
+    diag_ms = sum(b.elapsed_time(c) for _, b, c in marks)
+    value = world * sites * L * K / (total_ms * 1e-3)
+
+    launch_s = step_ms * 1e-3 / (K * L)
+    peak, peak_src = measured_peak()
+    achieved = BYTES_PER_SITE[args.precision] * sites / launch_s / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get((sim.kernel_kind, args.precision, N)),
+                "kernel": "fused leapfrog step (%s)" % sim.kernel_kind, "peak_source": peak_src,
+                "bytes_per_launch": BYTES_PER_SITE[args.precision] * sites, "launch_ms": launch_s * 1e3,
+                "frac_of_nominal_8TBps": achieved / 8000.0,
+                "diagnostics_ms_per_call": diag_ms / K, "diagnostics_in_steps": (diag_ms / K) / (launch_s * 1e3),
+                "diagnostics_GBps": (BYTES_PER_SITE[args.precision] // 2) * sites / (diag_ms / K * 1e-3) / 1e9,
+                "diagnostics_overhead_at_this_cadence": diag_ms / step_ms}
+
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(args, sim, torch, max_over_ranks, barrier, world)
+
+    line = {
+        "metric": "lattice site-updates/sec per leapfrog step", "value": value, "unit": "site-updates/s", "n_gpus": world,
+        "steps": K, "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.precision, "data": "synthetic", "config": workload_config(args),
+        "roofline": roofline, "clocks": clk, "gpu_launches": int(launches),
+        "ms_per_leapfrog_step": launch_s * 1e3, "step_only_site_updates_per_s": sites / launch_s,
+        "kernel": sim.kernel_kind,
+        "last_diagnostics": {k: diag[k] for k in ("step", "n_pierced", "xi", "v2", "gauss_max", "gauss_rhs_rms", "nonfinite")} if diag else None,
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    sim.destroy()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = oracle_sample(args)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores_online")}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_e2e(args, sim, torch, max_over_ranks, barrier, world):
+    """The same step through the C ABI with HOST buffers: every timed step uploads the 10 fields from pinned memory
+    (ahs_set_fields_native), runs L leapfrog launches + diagnostics and reads the diagnostics record back."""
+    N, L, E = args.lattice, args.leapfrog, max(1, args.e2e_steps)
+    sites = N ** 3
+    tdtype = torch.float32 if args.precision == "f32" else torch.float64
+    try:
+        host = torch.empty((10, N, N, N), dtype=tdtype, pin_memory=True)
+    except RuntimeError as exc:
+        return {"value": None, "unit": "site-updates/s", "error": "pinned host allocation failed: %s" % str(exc)[:120]}
+    n0 = sim.step_count
+    sim.get_fields_native(host.data_ptr())            # the resident state, downloaded once (untimed)
+    h2d = host.numel() * host.element_size()
+    import ctypes
+    d2h = ctypes.sizeof(__import__("paper_1809_00995_b200.binding", fromlist=["ahs_diag"]).ahs_diag)
+
+    def one():
+        sim.set_fields_native(host.data_ptr(), step=n0)
+        sim.step(L)
+        return sim.diagnostics()
+
+    one()                                             # warm-up
+    barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.perf_counter()
+    a.record()
+    for _ in range(E):
+        one()
+    b.record()
+    barrier()
+    wall = time.perf_counter() - w0
+    ms = max_over_ranks(max(a.elapsed_time(b), 0.0))
+    del host
+    return {"value": world * sites * L * E / (ms * 1e-3), "unit": "site-updates/s", "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "steps": E, "ms_per_step": ms / E, "wall_ms_per_step": 1e3 * wall / E,
+            "what": "ahs_set_fields_native (pinned host -> HBM) + %d x ahs_step + ahs_diagnostics_ex (record -> host) per step" % L}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

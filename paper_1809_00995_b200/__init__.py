@@ -2,5 +2,5 @@
 network leapfrog update and its diagnostics.  The product is the C-ABI library csrc/libahs.so (include/ahs.h);
 `binding` is its thin ctypes mirror.  Nothing in this package imports oracle/ (test infrastructure)."""
 
-__all__ = ["binding", "build", "synthetic", "harness"]
+__all__ = ["binding", "build", "synthetic"]
 __version__ = "0.1"
