@@ -89,7 +89,11 @@ __device__ __forceinline__ void issue_plane(T* stage, uint64_t* bar, const T* co
         const int a = i / G::ROWS, rr = i - a * G::ROWS;
         int y = y0 + rr - 1;
         y = y < 0 ? y + N : (y >= N ? y - N : y);
-        const T* row = src[a] + ((size_t)z * N + y) * N;
+        // (a select chain, not src[a]: a dynamically indexed pointer array would live in local memory)
+        const T* base = src[0];
+#pragma unroll
+        for (int j = 1; j < G::NA; ++j) base = (a == j) ? src[j] : base;
+        const T* row = base + ((size_t)z * N + y) * N;
         T* dst = stage + (a * G::ROWS + rr) * G::PITCH;
         if (interior) {
             bulk_g2s(dst, row + x0 - G::V, G::PITCH * sizeof(T), bar);

@@ -1,26 +1,34 @@
 // ahs_step_march.cu -- the fused leapfrog step (Eqs. 4-7) as a 2.5D z-march for sm_100a.
 //
-// One CTA owns a tile of TX x TY sites in (x, y) (TX = 32 lanes x one 16-byte vector, TY = 8 rows = 8 compute
-// warps) and marches over `zlen` planes.  A ninth warp is the producer: it streams the level-n fields phi, theta
-// (5 arrays) of plane k+2 into a 3-stage ring of halo'd shared-memory tiles with cp.async.bulk (UBLKCP) + mbarrier
-// while planes k, k+1 are in use (ahs_stage.cuh); Pi and eps (no halo) are read with streaming 16-byte loads and
-// all ten outputs leave as 16-byte stores.
+// One CTA owns a tile of TX x TY sites in (x, y) (TX = 32 lanes x one 16-byte vector, TY rows = TY warps) and
+// marches over `zlen` planes.  The level-n fields phi, theta (5 arrays) of plane k+2 are streamed into a 3-stage
+// ring of halo'd shared-memory tiles with cp.async.bulk (UBLKCP) + mbarrier while planes k, k+1 are in use
+// (ahs_stage.cuh; the issuing warp rotates); Pi and eps (no halo) are read with streaming 16-byte loads and all ten
+// outputs leave as 16-byte stores.
 //
 // Compute-once form.  Each site owner computes, from raw phi, theta of the site and of its FORWARD neighbours only,
 //   U_j = exp(-i theta_j)                         3 sincos       (link phases, Eq. 3 / L46-51, q = +1)
 //   f_j = U_j phi^{x+k_j}, b_j = conj(U_j) phi^x, J_j = Im[conj(phi^x) f_j]
 //   S_01, S_02, S_12 = sin Xi_ij^x                3 sin          (plaquettes based at x, Eq. 3)
 // and receives the six products owned by its BACKWARD neighbours:
-//   -x : b_0, S_01, S_02   through a small shared-memory exchange (slot lane-1; slot "-1" = halo column)
+//   -x : b_0, S_01, S_02   from the thread's previous vector element, else from lane-1 by warp shuffle, else
+//                          (lane 0) from the halo column x0-1 through shared memory
 //   -y : b_1, S_01, S_12   through a shared-memory exchange row (row -1 = halo row)
 //   -z : b_2, S_02, S_12   in the thread's own registers from the previous plane of the march.
-// The products of the halo row y0-1 and of the halo column x0-1 are recomputed by the producer warp (same
-// function, same inputs => bit-identical link phases on both sides of a tile edge, which is what keeps the Gauss
-// law at roundoff: it needs the same U in Eq. 4 and Eq. 5).  Then
+// The products of the halo row y0-1 and of the halo column x0-1 are recomputed inside the CTA, one site per lane,
+// by warps that take the job in rotation (same function, same inputs => bit-identical link phases on both sides of a tile edge, which is what keeps the Gauss
+// law at roundoff: it needs the same U in Eq. 4 and Eq. 5, R4).  Then
 //   Lap    = sum_j (f_j + b_j^{x-k_j}) - 6 phi                                              (Eq. 4)
 //   curl_0 = (S01 - S01^{-y}) + (S02 - S02^{-z}),  curl_1 = (S01^{-x} - S01) + (S12 - S12^{-z}),
 //   curl_2 = (S02^{-x} - S02) + (S12^{-y} - S12)                                            (Eq. 5)
 // followed by the kicks and the drift into the other (phi, theta) buffer (Eqs. 6-7).
+//
+// One CTA barrier per plane.  Phase 1 (before the barrier) does all the trigonometry and folds every term that the
+// thread owns -- including the -x terms obtained by shuffle and the -z terms carried in registers -- into partial
+// results (q = Pi' without the -y / halo hops, phi + dt q, eps' and theta + dt eps' without the -y / halo sines).
+// Phase 2 (after the barrier) adds the few terms that crossed a warp boundary and stores.  The exchange rows are
+// double-buffered by plane parity so that the barrier of plane k+1 also orders "everyone has read plane k's
+// exchange" before it is overwritten at plane k+2.
 // The paper's kernels stage raw fields per kernel and recompute every phase (L107-109); this is a different design.
 #include <cstdlib>
 #include <cstring>
@@ -28,6 +36,7 @@
 #include "ahs_internal.cuh"
 #include "ahs_math.cuh"
 #include "ahs_stage.cuh"
+#include "ahs_trig.cuh"
 
 namespace ahs {
 
@@ -39,18 +48,17 @@ template <typename T> struct NativeVec;
 template <> struct NativeVec<float> { using type = float4; };
 template <> struct NativeVec<double> { using type = double2; };
 
-template <typename T>
+template <typename T, int TY_>
 struct MarchCfg {
     static constexpr int V = 16 / sizeof(T);
-    static constexpr int TY = 8;
+    static constexpr int TY = TY_;
     static constexpr int NSTAGE = 3;
     using G = TileGeom<T, V, TY, 5, NSTAGE>;
     static constexpr int TX = G::TX;
-    static constexpr int NTHREADS = (TY + 1) * 32;
-    static constexpr int XP = 33;                         // x-exchange pitch: slot 0 = halo column, slot l+1 = lane l
-    static constexpr int YEX_ELEMS = 4 * (TY + 1) * TX;   // b1.re, b1.im, S01, S12 for rows -1 .. TY-1
-    static constexpr int XEX_ELEMS = 4 * TY * XP;         // b0.re, b0.im, S01, S02
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + YEX_ELEMS + XEX_ELEMS);
+    static constexpr int NTHREADS = TY * 32;
+    static constexpr int YEX_ELEMS = 4 * (TY + 1) * TX;   // b1.re, b1.im, S01, S12 for rows -1 .. TY-1 (one parity)
+    static constexpr int XEX_ELEMS = 4 * TY;              // b0.re, b0.im, S01, S02 of the halo column (one parity)
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
 
 template <typename T, int V>
@@ -77,24 +85,26 @@ __device__ __forceinline__ void stg_vec(T* p, const Vec<T, V>& v)
     *reinterpret_cast<NV*>(p) = n;
 }
 
-// Barrier over the whole CTA, executed from warp-specialised (warp-uniform) branches: a named barrier with an
-// explicit thread count, as the producer warp and the compute warps reach it from different code.
-template <int NT>
-__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); }
+// element v+1 of a vector, or the scalar `edge` (the first element of the next vector) for the last one
+template <typename T, int V>
+__device__ __forceinline__ T next_x(const Vec<T, V>& a, int v, T edge) { return v + 1 < V ? a.v[v + 1 < V ? v + 1 : v] : edge; }
 
-template <typename T, int MINB>
-__global__ void __launch_bounds__(MarchCfg<T>::NTHREADS, MINB) step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k)
+template <typename T, int TY, int MINB>
+__global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k)
 {
-    using C = MarchCfg<T>;
+    using C = MarchCfg<T, TY>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
-    constexpr int V = C::V, TX = C::TX, TY = C::TY, NS = C::NSTAGE, XP = C::XP, SE = G::STAGE_ELEMS;
+    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS;
+    // rotation of the side jobs over the warps at plane `it` (by (w + it) % ...): the halo row takes TX/32 = V warps
+    constexpr int HSTRIDE = TY / V, COLUMN = 1 % TY, ISSUER = 3 % TY;
+    static_assert(TY % V == 0, "the halo row is shared out over V warps");
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
     T* stages = reinterpret_cast<T*>(smem + 128);
     T* yex = stages + NS * SE;
-    T* xex = yex + C::YEX_ELEMS;
+    T* xex = yex + 2 * C::YEX_ELEMS;
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tiles_x = N / TX, tiles_y = N / TY;
@@ -116,7 +126,7 @@ __global__ void __launch_bounds__(MarchCfg<T>::NTHREADS, MINB) step_march_kernel
 
     // plane index i of this CTA's march = lattice plane z0 - 1 + i (periodic)
     auto plane_of = [&](int i) { const int z = z0 - 1 + i; return z < 0 ? z + N : (z >= N ? z - N : z); };
-    if (w == TY) {
+    if (w == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) issue_plane<G>(stages + i * SE, &full[i], src, N, x0, y0, plane_of(i), lane);
     }
@@ -127,7 +137,7 @@ __global__ void __launch_bounds__(MarchCfg<T>::NTHREADS, MINB) step_march_kernel
     // ---- prologue: z-products of plane z0-1 (needs planes z0-1 and z0) ---------------------------------------------
     mbar_wait(&full[0], 0);
     mbar_wait(&full[1], 0);
-    if (w < TY) {
+    {
         const T* sc = stages;
         const T* sn = stages + SE;
         const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
@@ -138,72 +148,31 @@ __global__ void __launch_bounds__(MarchCfg<T>::NTHREADS, MINB) step_march_kernel
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             T s, c;
-            sincos_t(t2.v[v], s, c);
+            sincos_fast(t2.v[v], s, c);
             const Cx<T> b = mulUc<T>(c, s, { pr.v[v], pi.v[v] });
             cb2r[v] = b.re;
             cb2i[v] = b.im;
-            const T t2x = (v < V - 1) ? t2.v[v + 1 < V ? v + 1 : v] : t2x_edge;
-            cS02[v] = sin_t(t0.v[v] + t2x - t0z.v[v] - t2.v[v]);
-            cS12[v] = sin_t(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
+            cS02[v] = sin_fast(t0.v[v] + next_x<T, V>(t2, v, t2x_edge) - t0z.v[v] - t2.v[v]);
+            cS12[v] = sin_fast(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
         }
     }
     __syncthreads();
+
+    const T dtc2 = k.dt * k.c2, dtd3 = k.dt * k.d3;
 
     // ---- the march -----------------------------------------------------------------------------------------------------
     for (int it = 1; it <= zlen; ++it) {
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
+        T* yexp = yex + (it & 1) * C::YEX_ELEMS;
+        T* xexp = xex + (it & 1) * C::XEX_ELEMS;
 
-        if (w == TY) {
-            // ------------------------------- producer + halo warp -------------------------------------------------------
-            if (it + 2 <= zlen + 1) {
-                const int s = (it + 2) % NS;   // held plane it-1: every thread finished it before the last barrier
-                issue_plane<G>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + 2), lane);
-            }
-            mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
-            {   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
-                const VecT pr = lds_vec<T, V>(sc + G::idx(0, -1, xi)), pi = lds_vec<T, V>(sc + G::idx(1, -1, xi));
-                const VecT t0 = lds_vec<T, V>(sc + G::idx(2, -1, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, -1, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, -1, xi));
-                const VecT t0y = lds_vec<T, V>(sc + G::idx(2, 0, xi)), t2y = lds_vec<T, V>(sc + G::idx(4, 0, xi));
-                const VecT t1z = lds_vec<T, V>(sn + G::idx(3, -1, xi));
-                const T t1x_edge = sc[G::idx(3, -1, xi + V)];
-                VecT b1r, b1i, s01, s12;
-#pragma unroll
-                for (int v = 0; v < V; ++v) {
-                    T s, c;
-                    sincos_t(t1.v[v], s, c);
-                    const Cx<T> b = mulUc<T>(c, s, { pr.v[v], pi.v[v] });
-                    b1r.v[v] = b.re;
-                    b1i.v[v] = b.im;
-                    const T t1x = (v < V - 1) ? t1.v[v + 1 < V ? v + 1 : v] : t1x_edge;
-                    s01.v[v] = sin_t(t0.v[v] + t1x - t0y.v[v] - t1.v[v]);
-                    s12.v[v] = sin_t(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
-                }
-                sts_vec<T, V>(yex + (0 * (TY + 1) + 0) * TX + xi, b1r);
-                sts_vec<T, V>(yex + (1 * (TY + 1) + 0) * TX + xi, b1i);
-                sts_vec<T, V>(yex + (2 * (TY + 1) + 0) * TX + xi, s01);
-                sts_vec<T, V>(yex + (3 * (TY + 1) + 0) * TX + xi, s12);
-            }
-            if (lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02 -> exchange slot 0
-                const int r = lane;
-                const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
-                const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = sc[G::idx(4, r, -1)];
-                const T t1x = sc[G::idx(3, r, 0)], t2x = sc[G::idx(4, r, 0)];
-                const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
-                T s, c;
-                sincos_t(t0, s, c);
-                const Cx<T> b = mulUc<T>(c, s, { pr, pi });
-                xex[(0 * TY + r) * XP] = b.re;
-                xex[(1 * TY + r) * XP] = b.im;
-                xex[(2 * TY + r) * XP] = sin_t(t0 + t1x - t0y - t1);
-                xex[(3 * TY + r) * XP] = sin_t(t0 + t2x - t0z - t2);
-            }
-            cta_sync<C::NTHREADS>();   // (A) products visible
-            cta_sync<C::NTHREADS>();   // (B) exchange buffers, and the stage of plane it, are free again
-            continue;
+        // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
+        if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1) {
+            const int s = (it + 2) % NS;
+            issue_plane<G>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + 2), lane);
         }
 
-        // ----------------------------------- compute warps ---------------------------------------------------------------
         const int z = z0 + it - 1;
         const size_t g = ((size_t)z * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
@@ -211,105 +180,168 @@ __global__ void __launch_bounds__(MarchCfg<T>::NTHREADS, MINB) step_march_kernel
 
         mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
 
-        const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
-        const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, w, xi));
-        T lfr[V], lfi[V], ep0[V], ep1[V], ep2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], nb2r[V], nb2i[V];
+        // partial results that cross the barrier (phase 1 -> phase 2)
+        T qr[V], qi[V], fr[V], fi[V], e0[V], e1[V], e2[V], g0[V], g1[V], g2[V];
         {
+            // ---- phase 1: products and everything this thread owns -----------------------------------------------------
+            const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
+            const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, w, xi));
             const VecT pry = lds_vec<T, V>(sc + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(sc + G::idx(1, w + 1, xi));
             const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(sc + G::idx(4, w + 1, xi));
             const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
             const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
             const T prx_e = sc[G::idx(0, w, xi + V)], pix_e = sc[G::idx(1, w, xi + V)];
             const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = sc[G::idx(4, w, xi + V)];
+            T lfr[V], lfi[V], J0[V], J1[V], J2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], b2r[V], b2i[V];
             VecT yb1r, yb1i, yS01, yS12;
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                const int vn = v + 1 < V ? v + 1 : v;
-                const T prx = (v < V - 1) ? pr.v[vn] : prx_e, pix = (v < V - 1) ? pi.v[vn] : pix_e;
-                const T t1x = (v < V - 1) ? t1.v[vn] : t1x_e, t2x = (v < V - 1) ? t2.v[vn] : t2x_e;
                 const Cx<T> ph = { pr.v[v], pi.v[v] };
                 T s, c;
-                sincos_t(t0.v[v], s, c);
-                const Cx<T> f0 = mulU<T>(c, s, { prx, pix });
+                sincos_fast(t0.v[v], s, c);
+                const Cx<T> f0 = mulU<T>(c, s, { next_x<T, V>(pr, v, prx_e), next_x<T, V>(pi, v, pix_e) });
                 const Cx<T> b0 = mulUc<T>(c, s, ph);
-                sincos_t(t1.v[v], s, c);
+                sincos_fast(t1.v[v], s, c);
                 const Cx<T> f1 = mulU<T>(c, s, { pry.v[v], piy.v[v] });
                 const Cx<T> b1 = mulUc<T>(c, s, ph);
-                sincos_t(t2.v[v], s, c);
+                sincos_fast(t2.v[v], s, c);
                 const Cx<T> f2 = mulU<T>(c, s, { prz.v[v], piz.v[v] });
                 const Cx<T> b2 = mulUc<T>(c, s, ph);
                 lfr[v] = (f0.re + f1.re) + f2.re;
                 lfi[v] = (f0.im + f1.im) + f2.im;
                 // J_j = Im[conj(phi^x) U_j phi^{x+k_j}]  (Eq. 5, 2nd term)
-                ep0[v] = k.d1 * E0.v[v] + k.d2 * (ph.re * f0.im - ph.im * f0.re);
-                ep1[v] = k.d1 * E1.v[v] + k.d2 * (ph.re * f1.im - ph.im * f1.re);
-                ep2[v] = k.d1 * E2.v[v] + k.d2 * (ph.re * f2.im - ph.im * f2.re);
+                J0[v] = ph.re * f0.im - ph.im * f0.re;
+                J1[v] = ph.re * f1.im - ph.im * f1.re;
+                J2[v] = ph.re * f2.im - ph.im * f2.re;
                 b0r[v] = b0.re; b0i[v] = b0.im;
                 yb1r.v[v] = b1.re; yb1i.v[v] = b1.im;
-                nb2r[v] = b2.re; nb2i[v] = b2.im;
+                b2r[v] = b2.re; b2i[v] = b2.im;
                 // Xi_ij^x = th_i^x + th_j^{x+k_i} - th_i^{x+k_j} - th_j^x  (Eq. 3)
-                S01[v] = sin_t(t0.v[v] + t1x - t0y.v[v] - t1.v[v]);
-                S02[v] = sin_t(t0.v[v] + t2x - t0z.v[v] - t2.v[v]);
-                S12[v] = sin_t(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
+                S01[v] = sin_fast(t0.v[v] + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - t1.v[v]);
+                S02[v] = sin_fast(t0.v[v] + next_x<T, V>(t2, v, t2x_e) - t0z.v[v] - t2.v[v]);
+                S12[v] = sin_fast(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
                 yS01.v[v] = S01[v];
                 yS12.v[v] = S12[v];
             }
-            sts_vec<T, V>(yex + (0 * (TY + 1) + w + 1) * TX + xi, yb1r);
-            sts_vec<T, V>(yex + (1 * (TY + 1) + w + 1) * TX + xi, yb1i);
-            sts_vec<T, V>(yex + (2 * (TY + 1) + w + 1) * TX + xi, yS01);
-            sts_vec<T, V>(yex + (3 * (TY + 1) + w + 1) * TX + xi, yS12);
-            xex[(0 * TY + w) * XP + lane + 1] = b0r[V - 1];
-            xex[(1 * TY + w) * XP + lane + 1] = b0i[V - 1];
-            xex[(2 * TY + w) * XP + lane + 1] = S01[V - 1];
-            xex[(3 * TY + w) * XP + lane + 1] = S02[V - 1];
-        }
-        cta_sync<C::NTHREADS>();   // (A)
-        {
-            const VecT yb1r = lds_vec<T, V>(yex + (0 * (TY + 1) + w) * TX + xi), yb1i = lds_vec<T, V>(yex + (1 * (TY + 1) + w) * TX + xi);
-            const VecT yS01 = lds_vec<T, V>(yex + (2 * (TY + 1) + w) * TX + xi), yS12 = lds_vec<T, V>(yex + (3 * (TY + 1) + w) * TX + xi);
-            const T xb0r = xex[(0 * TY + w) * XP + lane], xb0i = xex[(1 * TY + w) * XP + lane];
-            const T xS01 = xex[(2 * TY + w) * XP + lane], xS02 = xex[(3 * TY + w) * XP + lane];
-            VecT oPr, oPi, oE0, oE1, oE2, oFr, oFi, oT0, oT1, oT2;
+            sts_vec<T, V>(yexp + (0 * (TY + 1) + w + 1) * TX + xi, yb1r);
+            sts_vec<T, V>(yexp + (1 * (TY + 1) + w + 1) * TX + xi, yb1i);
+            sts_vec<T, V>(yexp + (2 * (TY + 1) + w + 1) * TX + xi, yS01);
+            sts_vec<T, V>(yexp + (3 * (TY + 1) + w + 1) * TX + xi, yS12);
+            // -x products of the lane to the left (lane 0 gets its halo-column values in phase 2)
+            T lb0r = __shfl_up_sync(0xffffffffu, b0r[V - 1], 1), lb0i = __shfl_up_sync(0xffffffffu, b0i[V - 1], 1);
+            T lS01 = __shfl_up_sync(0xffffffffu, S01[V - 1], 1), lS02 = __shfl_up_sync(0xffffffffu, S02[V - 1], 1);
+            if (lane == 0) { lb0r = T(0); lb0i = T(0); lS01 = T(0); lS02 = T(0); }
 #pragma unroll
             for (int v = 0; v < V; ++v) {
                 const int vp = v > 0 ? v - 1 : 0;
-                const T mb0r = v > 0 ? b0r[vp] : xb0r, mb0i = v > 0 ? b0i[vp] : xb0i;
-                const T mS01 = v > 0 ? S01[vp] : xS01, mS02 = v > 0 ? S02[vp] : xS02;
-                const T lap_re = (lfr[v] - T(6) * pr.v[v]) + ((mb0r + yb1r.v[v]) + cb2r[v]);
-                const T lap_im = (lfi[v] - T(6) * pi.v[v]) + ((mb0i + yb1i.v[v]) + cb2i[v]);
+                const T mb0r = v > 0 ? b0r[vp] : lb0r, mb0i = v > 0 ? b0i[vp] : lb0i;
+                const T mS01 = v > 0 ? S01[vp] : lS01, mS02 = v > 0 ? S02[vp] : lS02;
+                const T lap_re = (lfr[v] - T(6) * pr.v[v]) + (mb0r + cb2r[v]);   // without b_1^{-y} (and the halo b_0)
+                const T lap_im = (lfi[v] - T(6) * pi.v[v]) + (mb0i + cb2i[v]);
                 const T higgs = k.c3 * (pr.v[v] * pr.v[v] + pi.v[v] * pi.v[v] - k.sigma2);
-                const T npr = k.c1 * Pr.v[v] - higgs * pr.v[v] + k.c2 * lap_re;     // Eq. 4
-                const T npi = k.c1 * Pi.v[v] - higgs * pi.v[v] + k.c2 * lap_im;
-                const T curl0 = (S01[v] - yS01.v[v]) + (S02[v] - cS02[v]);
-                const T curl1 = (mS01 - S01[v]) + (S12[v] - cS12[v]);
-                const T curl2 = (mS02 - S02[v]) + (yS12.v[v] - S12[v]);
-                const T ne0 = ep0[v] - k.d3 * curl0, ne1 = ep1[v] - k.d3 * curl1, ne2 = ep2[v] - k.d3 * curl2;   // Eq. 5
-                oPr.v[v] = npr; oPi.v[v] = npi; oE0.v[v] = ne0; oE1.v[v] = ne1; oE2.v[v] = ne2;
-                oFr.v[v] = pr.v[v] + k.dt * npr;                                      // Eq. 6
-                oFi.v[v] = pi.v[v] + k.dt * npi;
-                oT0.v[v] = t0.v[v] + k.dt * ne0;                                      // Eq. 7
-                oT1.v[v] = t1.v[v] + k.dt * ne1;
-                oT2.v[v] = t2.v[v] + k.dt * ne2;
-                cb2r[v] = nb2r[v]; cb2i[v] = nb2i[v]; cS02[v] = S02[v]; cS12[v] = S12[v];
+                qr[v] = k.c1 * Pr.v[v] - higgs * pr.v[v] + k.c2 * lap_re;       // Eq. 4, owned part
+                qi[v] = k.c1 * Pi.v[v] - higgs * pi.v[v] + k.c2 * lap_im;
+                fr[v] = pr.v[v] + k.dt * qr[v];                                  // Eq. 6, owned part
+                fi[v] = pi.v[v] + k.dt * qi[v];
+                // Eq. 5, owned part of the curl: everything except S01^{-y}, S12^{-y} (and the halo S01^{-x}, S02^{-x})
+                e0[v] = k.d1 * E0.v[v] + k.d2 * J0[v] - k.d3 * ((S01[v] + S02[v]) - cS02[v]);
+                e1[v] = k.d1 * E1.v[v] + k.d2 * J1[v] - k.d3 * ((S12[v] - S01[v]) + (mS01 - cS12[v]));
+                e2[v] = k.d1 * E2.v[v] + k.d2 * J2[v] - k.d3 * (mS02 - (S02[v] + S12[v]));
+                g0[v] = t0.v[v] + k.dt * e0[v];                                  // Eq. 7, owned part
+                g1[v] = t1.v[v] + k.dt * e1[v];
+                g2[v] = t2.v[v] + k.dt * e2[v];
+                cb2r[v] = b2r[v]; cb2i[v] = b2i[v]; cS02[v] = S02[v]; cS12[v] = S12[v];
+            }
+        }
+        // ---- halo products, shared out over the warps (no dedicated producer warp: 8 warps x 2 CTAs fill the register
+        //      file evenly).  Row y0-1: one site per lane, HSTRIDE-th warps in rotation; column x0-1: one warp per plane.
+        if (((w + it) % HSTRIDE) == 0) {
+            const int x = 32 * (w / HSTRIDE) + lane;   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
+            const T pr = sc[G::idx(0, -1, x)], pi = sc[G::idx(1, -1, x)];
+            const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = sc[G::idx(4, -1, x)];
+            const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = sc[G::idx(4, 0, x)], t1z = sn[G::idx(3, -1, x)];
+            T s, c;
+            sincos_fast(t1, s, c);
+            const Cx<T> b = mulUc<T>(c, s, { pr, pi });
+            yexp[(0 * (TY + 1) + 0) * TX + x] = b.re;
+            yexp[(1 * (TY + 1) + 0) * TX + x] = b.im;
+            yexp[(2 * (TY + 1) + 0) * TX + x] = sin_fast(t0 + t1x - t0y - t1);
+            yexp[(3 * (TY + 1) + 0) * TX + x] = sin_fast(t1 + t2y - t1z - t2);
+        }
+        if (((w + it) % TY) == COLUMN && lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02
+            const int r = lane;
+            const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
+            const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = sc[G::idx(4, r, -1)];
+            const T t1x = sc[G::idx(3, r, 0)], t2x = sc[G::idx(4, r, 0)];
+            const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
+            T s, c;
+            sincos_fast(t0, s, c);
+            const Cx<T> b = mulUc<T>(c, s, { pr, pi });
+            xexp[0 * TY + r] = b.re;
+            xexp[1 * TY + r] = b.im;
+            xexp[2 * TY + r] = sin_fast(t0 + t1x - t0y - t1);
+            xexp[3 * TY + r] = sin_fast(t0 + t2x - t0z - t2);
+        }
+        __syncthreads();
+        {
+            // ---- phase 2: the terms that crossed a warp or tile boundary, then the stores ----------------------------
+            const VecT yb1r = lds_vec<T, V>(yexp + (0 * (TY + 1) + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * (TY + 1) + w) * TX + xi);
+            const VecT yS01 = lds_vec<T, V>(yexp + (2 * (TY + 1) + w) * TX + xi), yS12 = lds_vec<T, V>(yexp + (3 * (TY + 1) + w) * TX + xi);
+            T hb0r = xexp[0 * TY + w], hb0i = xexp[1 * TY + w], hS01 = xexp[2 * TY + w], hS02 = xexp[3 * TY + w];
+            if (lane != 0) { hb0r = T(0); hb0i = T(0); hS01 = T(0); hS02 = T(0); }
+            VecT oPr, oPi, oE0, oE1, oE2, oFr, oFi, oT0, oT1, oT2;
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const T nr = v == 0 ? yb1r.v[v] + hb0r : yb1r.v[v];
+                const T ni = v == 0 ? yb1i.v[v] + hb0i : yb1i.v[v];
+                const T c1x = v == 0 ? hS01 : T(0);                 // S01^{-x} of the halo column
+                const T c2x = v == 0 ? yS12.v[v] + hS02 : yS12.v[v];   // S12^{-y} + S02^{-x}(halo)
+                oPr.v[v] = qr[v] + k.c2 * nr;
+                oPi.v[v] = qi[v] + k.c2 * ni;
+                oFr.v[v] = fr[v] + dtc2 * nr;
+                oFi.v[v] = fi[v] + dtc2 * ni;
+                oE0.v[v] = e0[v] + k.d3 * yS01.v[v];
+                oT0.v[v] = g0[v] + dtd3 * yS01.v[v];
+                oE1.v[v] = v == 0 ? e1[v] - k.d3 * c1x : e1[v];
+                oT1.v[v] = v == 0 ? g1[v] - dtd3 * c1x : g1[v];
+                oE2.v[v] = e2[v] - k.d3 * c2x;
+                oT2.v[v] = g2[v] - dtd3 * c2x;
             }
             stg_vec<T, V>(f.pi_re + g, oPr); stg_vec<T, V>(f.pi_im + g, oPi);
             stg_vec<T, V>(f.eps[0] + g, oE0); stg_vec<T, V>(f.eps[1] + g, oE1); stg_vec<T, V>(f.eps[2] + g, oE2);
             stg_vec<T, V>(f.phi_re_out + g, oFr); stg_vec<T, V>(f.phi_im_out + g, oFi);
             stg_vec<T, V>(f.th_out[0] + g, oT0); stg_vec<T, V>(f.th_out[1] + g, oT1); stg_vec<T, V>(f.th_out[2] + g, oT2);
         }
-        cta_sync<C::NTHREADS>();   // (B)
     }
 }
 
-template <typename T>
-int pick_zlen(int N)
+template <typename T, int TY>
+int pick_zlen(int N, int ctas_per_sm)
 {
-    using C = MarchCfg<T>;
-    const long tiles = (long)(N / C::TX) * (N / C::TY);
+    using C = MarchCfg<T, TY>;
+    const long tiles = (long)(N / C::TX) * (N / TY);
     const int cands[4] = { 64, 32, 16, 8 };
     for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) >= 8 * 148) return c;   // enough CTAs for >= 4 waves at 2 CTAs per SM
+        if (N % c == 0 && tiles * (N / c) >= 4L * ctas_per_sm * 148) return c;   // >= 4 waves of resident CTAs
     return 8;
+}
+
+template <typename T, int TY, int MINB>
+int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st)
+{
+    using C = MarchCfg<T, TY>;
+    auto kern = step_march_kernel<T, TY, MINB>;
+    static bool configured = false;
+    if (!configured) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return AHS_ERR_CUDA;
+        configured = true;
+    }
+    static const int zlen_env = [] { const char* e = getenv("AHS_MARCH_ZLEN"); return e ? atoi(e) : 0; }();
+    const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB);
+    const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
+    StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k);
+    return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
 
 }  // namespace
@@ -317,28 +349,19 @@ int pick_zlen(int N)
 template <typename T>
 bool march_supported(int N)
 {
-    using C = MarchCfg<T>;
-    return N >= C::TX && N % C::TX == 0 && N % C::TY == 0;
+    using C = MarchCfg<T, 8>;
+    return N >= C::TX && N % C::TX == 0 && N % 8 == 0;
 }
 
 template <typename T>
 int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st)
 {
-    using C = MarchCfg<T>;
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
-    // tuning knob (experiments only): AHS_MARCH_MINB=1 compiles for one resident CTA per SM (more registers)
-    static const int minb = [] { const char* e = getenv("AHS_MARCH_MINB"); return (e && e[0] == '1') ? 1 : 2; }();
-    auto kern = minb == 1 ? step_march_kernel<T, 1> : step_march_kernel<T, 2>;
-    static bool configured = false;
-    if (!configured) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return AHS_ERR_CUDA;
-        configured = true;
-    }
-    const int zlen = pick_zlen<T>(N);
-    const long blocks = (long)(N / C::TX) * (N / C::TY) * (N / zlen);
-    StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k);
-    return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
+    // 4-row tiles, four CTAs (barrier domains) per SM, measured fastest (profiles/); AHS_MARCH_TY=8 (experiments
+    // only) selects 8-row tiles, two CTAs per SM
+    static const int ty = [] { const char* e = getenv("AHS_MARCH_TY"); return e ? atoi(e) : 4; }();
+    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, st);
+    return launch_cfg<T, 4, 4>(f, N, c, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu

@@ -1,0 +1,120 @@
+// ahs_trig.cuh -- branch-free sine / cosine for the marching kernels (fp32 and fp64), accurate to ~1-2 ulp.
+//
+// Why not libdevice sincosf/sinf: the step is issue-bound as much as HBM-bound, six
+// transcendental evaluations per site are half of its instructions, and every libdevice call carries a
+// Payne-Hanek slow path whose branch (BSSY/BSYNC) stalls instruction fetch and bloats the loop past the
+// instruction cache (profiles/r1_step512_march_v1.md).  Why not the __sinf/__cosf intrinsics: their absolute
+// error (2^-21) is what PAPER.md L142 reports as degrading the diagnostics.  So: Cody-Waite reduction with a
+// three-term split of pi/2 (or pi) carried by FMAs, then minimax-style polynomials on the reduced interval.
+//
+//   sincos_fast(x): k = rint(x * 2/pi), r = x - k*pi/2 in [-pi/4, pi/4]; sin and cos polynomials; quadrant fix-up.
+//   sin_fast(x)   : fp32: k = rint(x / pi), r in [-pi/2, pi/2], odd polynomial, sign (-1)^k;
+//                   fp64: the quadrant form with the coefficient set chosen by the parity of k.
+// Measured against fp64 / long double references (csrc/fit_trig.py): fp32 sincos <= 0.9 ulp, fp32 sin <= 1.9 ulp
+// (abs 1.2e-7), fp64 <= 1.3 ulp.  Domain: |x| < 2^22 * pi/2 (fp32: 6.5e6; fp64: |x| < 2^30); beyond it the result
+// is finite garbage or NaN (a link angle that large has no phase information left in fp32 anyway); NaN and Inf
+// inputs give NaN, so blown-up lattices still reach the diagnostics' non-finite flag.
+// The polynomial coefficients were fitted by csrc/fit_trig.py (least squares on Chebyshev nodes, relative
+// weighting), not copied from a library.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace ahs {
+
+// ---- fp32 ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sincos_fast(float x, float& s, float& c)
+{
+    const float t = fmaf(x, 0.6366197466850281f, 12582912.0f);   // 1.5 * 2^23: the low mantissa bits hold rint(x * 2/pi)
+    const int q = __float_as_int(t);
+    const float k = t - 12582912.0f;
+    float r = fmaf(k, -1.5707963705062866f, x);
+    r = fmaf(k, 4.371138828673793e-08f, r);
+    r = fmaf(k, 1.7151245100058819e-15f, r);
+    const float z = r * r;
+    float ps = fmaf(z, -0.00019513866573106498f, 0.00833214819431305f);
+    ps = fmaf(z, ps, -0.16666653752326965f);
+    const float sr = fmaf(r * z, ps, r);
+    float pc = fmaf(z, 2.438912088109646e-05f, -0.0013886747183278203f);
+    pc = fmaf(z, pc, 0.04166662320494652f);
+    pc = fmaf(z, pc, -0.5f);
+    const float cr = fmaf(z, pc, 1.0f);
+    const bool odd = q & 1;
+    const float so = odd ? cr : sr, co = odd ? sr : cr;
+    s = __int_as_float(__float_as_int(so) ^ ((q << 30) & 0x80000000));
+    c = __int_as_float(__float_as_int(co) ^ (((q + 1) << 30) & 0x80000000));
+}
+
+__device__ __forceinline__ float sin_fast(float x)
+{
+    const float t = fmaf(x, 0.31830987334251404f, 12582912.0f);
+    const int q = __float_as_int(t);
+    const float k = t - 12582912.0f;
+    float r = fmaf(k, -3.1415927410125732f, x);
+    r = fmaf(k, 8.742277657347586e-08f, r);
+    r = fmaf(k, 3.4302490200117637e-15f, r);
+    const float z = r * r;
+    float p = fmaf(z, -2.388586395341008e-08f, 2.752518867055187e-06f);
+    p = fmaf(z, p, -0.00019840864115394652f);
+    p = fmaf(z, p, 0.008333330973982811f);
+    p = fmaf(z, p, -0.1666666716337204f);
+    const float sr = fmaf(r * z, p, r);
+    return __int_as_float(__float_as_int(sr) ^ (q << 31));
+}
+
+// ---- fp64 ---------------------------------------------------------------------------------------------------------------
+namespace trig64 {
+__device__ __forceinline__ double reduce(double x, int& q)
+{
+    const double t = fma(x, 0.6366197723675814, 6755399441055744.0);   // 1.5 * 2^52
+    q = __double2loint(t);
+    const double k = t - 6755399441055744.0;
+    double r = fma(k, -1.5707963267948966, x);
+    r = fma(k, -6.123233995736766e-17, r);
+    r = fma(k, 1.4973849048591698e-33, r);
+    return r;
+}
+__device__ __forceinline__ double flip(double v, int bit)   // negate v if bit 1 of `bit` is set
+{
+    return __hiloint2double(__double2hiint(v) ^ ((bit << 30) & 0x80000000), __double2loint(v));
+}
+}  // namespace trig64
+
+__device__ __forceinline__ void sincos_fast(double x, double& s, double& c)
+{
+    int q;
+    const double r = trig64::reduce(x, q);
+    const double z = r * r;
+    double ps = fma(z, 1.5895906110388965e-10, -2.505074159906586e-08);
+    ps = fma(z, ps, 2.7557313577062805e-06);
+    ps = fma(z, ps, -0.00019841269829441296);
+    ps = fma(z, ps, 0.008333333333321893);
+    ps = fma(z, ps, -0.1666666666666663);
+    const double sr = fma(r * z, ps, r);
+    double pc = fma(z, -1.1359191040163257e-11, 2.087571361252908e-09);
+    pc = fma(z, pc, -2.755731427353126e-07);
+    pc = fma(z, pc, 2.480158728917463e-05);
+    pc = fma(z, pc, -0.0013888888888873554);
+    pc = fma(z, pc, 0.041666666666666595);
+    const double cr = fma(z * z, pc, fma(z, -0.5, 1.0));
+    const bool odd = q & 1;
+    s = trig64::flip(odd ? cr : sr, q);
+    c = trig64::flip(odd ? sr : cr, q + 1);
+}
+
+__device__ __forceinline__ double sin_fast(double x)
+{
+    int q;
+    const double r = trig64::reduce(x, q);
+    const double z = r * r;
+    const bool odd = q & 1;
+    double p = fma(z, odd ? -1.1359191040163257e-11 : 1.5895906110388965e-10, odd ? 2.087571361252908e-09 : -2.505074159906586e-08);
+    p = fma(z, p, odd ? -2.755731427353126e-07 : 2.7557313577062805e-06);
+    p = fma(z, p, odd ? 2.480158728917463e-05 : -0.00019841269829441296);
+    p = fma(z, p, odd ? -0.0013888888888873554 : 0.008333333333321893);
+    p = fma(z, p, odd ? 0.041666666666666595 : -0.1666666666666663);
+    const double base = odd ? fma(z, -0.5, 1.0) : r;
+    const double mult = (odd ? z : r) * z;
+    return trig64::flip(fma(mult, p, base), q);
+}
+
+}  // namespace ahs
