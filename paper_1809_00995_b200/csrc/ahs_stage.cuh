@@ -6,7 +6,7 @@
 // elements, so that every row segment is a 16-byte aligned contiguous run in global memory; periodic wrap
 // is resolved per row segment by the issuing lane).  No tensor map is needed: a row segment of an x-fastest
 // SoA array IS contiguous.  The paper stages tiles with per-thread loads and explicit halo threads
-// (Fig. 1); here one warp issues ~50 row copies per plane and nobody touches the data until
+// (Fig. 1); here one thread issues the row copies of a plane and nobody touches the data until
 // the mbarrier flips.
 #pragma once
 #include <cuda_runtime.h>
@@ -43,6 +43,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
             : "memory");
     } while (!done);
 }
+// one lane of the (converged) warp: elect.sync tells the compiler that exactly one thread runs the guarded code, so
+// the uniform-register operands of cp.async.bulk need no per-lane serialisation loop
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
 // global -> shared bulk copy of `bytes` (multiple of 16; both addresses 16-byte aligned), completion on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
 {
@@ -70,39 +82,53 @@ struct TileGeom {
     static constexpr int ARR_ELEMS = ROWS * PITCH;
     static constexpr int STAGE_ELEMS = NA * ARR_ELEMS;
     static constexpr uint32_t STAGE_BYTES = STAGE_ELEMS * sizeof(T);
+    static constexpr uint32_t ARR_BYTES = ARR_ELEMS * sizeof(T);
     static_assert(sizeof(T) * V == 16, "a vector is 16 bytes");
 
     // element (array a, row r in [-1, TY], column xi in [-V, TX+V)) of a stage
     __device__ __forceinline__ static int idx(int a, int r, int xi) { return (a * ROWS + (r + 1)) * PITCH + (xi + V); }
 };
 
-// Issue the copies of one z-plane into one stage.  Called by all 32 lanes of the producer warp.
-//   src[a]  : global base pointers of the NA staged arrays
+// Issue the copies of one z-plane of NA arrays into NA consecutive array slots at `dst`.  Called by ONE thread, after
+// it has posted the expected byte count on `bar` (mbar_arrive_expect_tx).  cp.async.bulk takes its operands from
+// uniform registers, so copies issued by several lanes of a warp are serialised by a per-lane loop of ~15
+// instructions each (profiles/r3: 15 % of all instructions executed); a single thread walking the rows with
+// running pointers costs a third of that.
+//   src[a]  : global base pointers of the arrays
 //   z       : plane (already wrapped into [0, N))
-template <typename G, typename T>
-__device__ __forceinline__ void issue_plane(T* stage, uint64_t* bar, const T* const (&src)[G::NA], int N, int x0, int y0, int z, int lane)
+template <typename G, int NA, typename T>
+__device__ __forceinline__ void issue_rows(T* dst_base, uint64_t* bar, const T* const (&src)[NA], int N, int x0, int y0, int z)
 {
-    if (lane == 0) mbar_arrive_expect_tx(bar, G::STAGE_BYTES);
-    __syncwarp();
-    const bool interior = (x0 > 0) && (x0 + G::TX < N);   // warp-uniform
-    for (int i = lane; i < G::NA * G::ROWS; i += 32) {
-        const int a = i / G::ROWS, rr = i - a * G::ROWS;
-        int y = y0 + rr - 1;
-        y = y < 0 ? y + N : (y >= N ? y - N : y);
-        // (a select chain, not src[a]: a dynamically indexed pointer array would live in local memory)
-        const T* base = src[0];
+    const bool x_interior = (x0 > 0) && (x0 + G::TX < N);
+    const bool y_interior = (y0 > 0) && (y0 + G::TY < N);
+    const size_t plane = (size_t)z * N * N;
+    if (x_interior && y_interior) {
 #pragma unroll
-        for (int j = 1; j < G::NA; ++j) base = (a == j) ? src[j] : base;
-        const T* row = base + ((size_t)z * N + y) * N;
-        T* dst = stage + (a * G::ROWS + rr) * G::PITCH;
-        if (interior) {
-            bulk_g2s(dst, row + x0 - G::V, G::PITCH * sizeof(T), bar);
-        } else {
-            const int xl = x0 == 0 ? N - G::V : x0 - G::V;
-            const int xr = x0 + G::TX == N ? 0 : x0 + G::TX;
-            bulk_g2s(dst, row + xl, 16, bar);
-            bulk_g2s(dst + G::V, row + x0, G::TX * sizeof(T), bar);
-            bulk_g2s(dst + G::V + G::TX, row + xr, 16, bar);
+        for (int a = 0; a < NA; ++a) {
+            const T* row = src[a] + plane + (size_t)(y0 - 1) * N + (x0 - G::V);
+            T* dst = dst_base + a * G::ARR_ELEMS;
+#pragma unroll
+            for (int rr = 0; rr < G::ROWS; ++rr) bulk_g2s(dst + rr * G::PITCH, row + (size_t)rr * N, G::PITCH * sizeof(T), bar);
+        }
+        return;
+    }
+    const int xl = x0 == 0 ? N - G::V : x0 - G::V;
+    const int xr = x0 + G::TX == N ? 0 : x0 + G::TX;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        T* dst = dst_base + a * G::ARR_ELEMS;
+#pragma unroll 1
+        for (int rr = 0; rr < G::ROWS; ++rr) {
+            int y = y0 + rr - 1;
+            y = y < 0 ? y + N : (y >= N ? y - N : y);
+            const T* row = src[a] + plane + (size_t)y * N;
+            if (x_interior) {
+                bulk_g2s(dst + rr * G::PITCH, row + x0 - G::V, G::PITCH * sizeof(T), bar);
+            } else {
+                bulk_g2s(dst + rr * G::PITCH, row + xl, 16, bar);
+                bulk_g2s(dst + rr * G::PITCH + G::V, row + x0, G::TX * sizeof(T), bar);
+                bulk_g2s(dst + rr * G::PITCH + G::V + G::TX, row + xr, 16, bar);
+            }
         }
     }
 }

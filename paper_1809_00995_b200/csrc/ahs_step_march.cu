@@ -53,12 +53,13 @@ struct MarchCfg {
     static constexpr int V = 16 / sizeof(T);
     static constexpr int TY = TY_;
     static constexpr int NSTAGE = 3;
-    using G = TileGeom<T, V, TY, 5, NSTAGE>;
+    using G = TileGeom<T, V, TY, 4, NSTAGE>;                // a stage: phi_re, phi_im, theta_0, theta_1 of one plane
+    static constexpr int T2_SLOTS = 2;                       // theta_2 is never read one plane ahead: a ring of two
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
-    static constexpr int YEX_ELEMS = 4 * (TY + 1) * TX;   // b1.re, b1.im, S01, S12 for rows -1 .. TY-1 (one parity)
+    static constexpr int YEX_ELEMS = 4 * TY * TX;         // b1.re, b1.im, S01, S12 of rows -1 .. TY-2 (one parity)
     static constexpr int XEX_ELEMS = 4 * TY;              // b0.re, b0.im, S01, S02 of the halo column (one parity)
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * G::ARR_ELEMS + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
 
 template <typename T, int V>
@@ -103,7 +104,8 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
     T* stages = reinterpret_cast<T*>(smem + 128);
-    T* yex = stages + NS * SE;
+    T* th2ring = stages + NS * SE;
+    T* yex = th2ring + C::T2_SLOTS * G::ARR_ELEMS;
     T* xex = yex + 2 * C::YEX_ELEMS;
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -115,7 +117,8 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     const int x0 = tx * TX, y0 = ty * TY, z0 = zc * zlen;
     const int xi = V * lane;
 
-    const T* const src[5] = { f.phi_re, f.phi_im, f.th[0], f.th[1], f.th[2] };
+    const T* const src[4] = { f.phi_re, f.phi_im, f.th[0], f.th[1] };
+    const T* const src2[1] = { f.th[2] };
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -128,7 +131,14 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     auto plane_of = [&](int i) { const int z = z0 - 1 + i; return z < 0 ? z + N : (z >= N ? z - N : z); };
     if (w == 0) {
 #pragma unroll
-        for (int i = 0; i < NS; ++i) issue_plane<G>(stages + i * SE, &full[i], src, N, x0, y0, plane_of(i), lane);
+        for (int i = 0; i < NS; ++i) {
+            const bool t2 = i < C::T2_SLOTS;   // theta_2 of planes 0, 1 ride on the barriers of planes 0, 1
+            if (elect_one()) {
+                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + (t2 ? G::ARR_BYTES : 0u));
+                issue_rows<G, 4>(stages + i * SE, &full[i], src, N, x0, y0, plane_of(i));
+                if (t2) issue_rows<G, 1>(th2ring + i * G::ARR_ELEMS, &full[i], src2, N, x0, y0, plane_of(i));
+            }
+        }
     }
 
     // products of the previous plane, carried in registers: b_2 = conj(U_2) phi, S_02, S_12
@@ -140,11 +150,12 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     {
         const T* sc = stages;
         const T* sn = stages + SE;
+        const T* t2c = th2ring;
         const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
-        const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, w, xi));
-        const VecT t2y = lds_vec<T, V>(sc + G::idx(4, w + 1, xi));
+        const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(t2c + G::idx(0, w, xi));
+        const VecT t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
-        const T t2x_edge = sc[G::idx(4, w, xi + V)];
+        const T t2x_edge = t2c[G::idx(0, w, xi + V)];
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             T s, c;
@@ -164,13 +175,16 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     for (int it = 1; it <= zlen; ++it) {
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
+        const T* t2c = th2ring + (it & 1) * G::ARR_ELEMS;
         T* yexp = yex + (it & 1) * C::YEX_ELEMS;
         T* xexp = xex + (it & 1) * C::XEX_ELEMS;
 
         // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
-        if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1) {
-            const int s = (it + 2) % NS;
-            issue_plane<G>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + 2), lane);
+        if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
+            const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
+            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES);
+            issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + 2));
+            issue_rows<G, 1>(th2ring + ((it + 1) & 1) * G::ARR_ELEMS, &full[s], src2, N, x0, y0, plane_of(it + 1));
         }
 
         const int z = z0 + it - 1;
@@ -185,13 +199,13 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
         {
             // ---- phase 1: products and everything this thread owns -----------------------------------------------------
             const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
-            const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, w, xi));
+            const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(t2c + G::idx(0, w, xi));
             const VecT pry = lds_vec<T, V>(sc + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(sc + G::idx(1, w + 1, xi));
-            const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(sc + G::idx(4, w + 1, xi));
+            const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
             const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
             const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
             const T prx_e = sc[G::idx(0, w, xi + V)], pix_e = sc[G::idx(1, w, xi + V)];
-            const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = sc[G::idx(4, w, xi + V)];
+            const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = t2c[G::idx(0, w, xi + V)];
             T lfr[V], lfi[V], J0[V], J1[V], J2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], b2r[V], b2i[V];
             VecT yb1r, yb1i, yS01, yS12;
 #pragma unroll
@@ -223,10 +237,12 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
                 yS01.v[v] = S01[v];
                 yS12.v[v] = S12[v];
             }
-            sts_vec<T, V>(yexp + (0 * (TY + 1) + w + 1) * TX + xi, yb1r);
-            sts_vec<T, V>(yexp + (1 * (TY + 1) + w + 1) * TX + xi, yb1i);
-            sts_vec<T, V>(yexp + (2 * (TY + 1) + w + 1) * TX + xi, yS01);
-            sts_vec<T, V>(yexp + (3 * (TY + 1) + w + 1) * TX + xi, yS12);
+            if (w + 1 < TY) {   // (the last row's -y products belong to the tile above, which recomputes them)
+            sts_vec<T, V>(yexp + (0 * TY + w + 1) * TX + xi, yb1r);
+            sts_vec<T, V>(yexp + (1 * TY + w + 1) * TX + xi, yb1i);
+            sts_vec<T, V>(yexp + (2 * TY + w + 1) * TX + xi, yS01);
+            sts_vec<T, V>(yexp + (3 * TY + w + 1) * TX + xi, yS12);
+            }
             // -x products of the lane to the left (lane 0 gets its halo-column values in phase 2)
             T lb0r = __shfl_up_sync(0xffffffffu, b0r[V - 1], 1), lb0i = __shfl_up_sync(0xffffffffu, b0i[V - 1], 1);
             T lS01 = __shfl_up_sync(0xffffffffu, S01[V - 1], 1), lS02 = __shfl_up_sync(0xffffffffu, S02[V - 1], 1);
@@ -258,21 +274,21 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
         if (((w + it) % HSTRIDE) == 0) {
             const int x = 32 * (w / HSTRIDE) + lane;   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
             const T pr = sc[G::idx(0, -1, x)], pi = sc[G::idx(1, -1, x)];
-            const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = sc[G::idx(4, -1, x)];
-            const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = sc[G::idx(4, 0, x)], t1z = sn[G::idx(3, -1, x)];
+            const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = t2c[G::idx(0, -1, x)];
+            const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = t2c[G::idx(0, 0, x)], t1z = sn[G::idx(3, -1, x)];
             T s, c;
             sincos_fast(t1, s, c);
             const Cx<T> b = mulUc<T>(c, s, { pr, pi });
-            yexp[(0 * (TY + 1) + 0) * TX + x] = b.re;
-            yexp[(1 * (TY + 1) + 0) * TX + x] = b.im;
-            yexp[(2 * (TY + 1) + 0) * TX + x] = sin_fast(t0 + t1x - t0y - t1);
-            yexp[(3 * (TY + 1) + 0) * TX + x] = sin_fast(t1 + t2y - t1z - t2);
+            yexp[(0 * TY + 0) * TX + x] = b.re;
+            yexp[(1 * TY + 0) * TX + x] = b.im;
+            yexp[(2 * TY + 0) * TX + x] = sin_fast(t0 + t1x - t0y - t1);
+            yexp[(3 * TY + 0) * TX + x] = sin_fast(t1 + t2y - t1z - t2);
         }
         if (((w + it) % TY) == COLUMN && lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02
             const int r = lane;
             const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
-            const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = sc[G::idx(4, r, -1)];
-            const T t1x = sc[G::idx(3, r, 0)], t2x = sc[G::idx(4, r, 0)];
+            const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = t2c[G::idx(0, r, -1)];
+            const T t1x = sc[G::idx(3, r, 0)], t2x = t2c[G::idx(0, r, 0)];
             const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
             T s, c;
             sincos_fast(t0, s, c);
@@ -285,8 +301,8 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
         __syncthreads();
         {
             // ---- phase 2: the terms that crossed a warp or tile boundary, then the stores ----------------------------
-            const VecT yb1r = lds_vec<T, V>(yexp + (0 * (TY + 1) + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * (TY + 1) + w) * TX + xi);
-            const VecT yS01 = lds_vec<T, V>(yexp + (2 * (TY + 1) + w) * TX + xi), yS12 = lds_vec<T, V>(yexp + (3 * (TY + 1) + w) * TX + xi);
+            const VecT yb1r = lds_vec<T, V>(yexp + (0 * TY + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * TY + w) * TX + xi);
+            const VecT yS01 = lds_vec<T, V>(yexp + (2 * TY + w) * TX + xi), yS12 = lds_vec<T, V>(yexp + (3 * TY + w) * TX + xi);
             T hb0r = xexp[0 * TY + w], hb0i = xexp[1 * TY + w], hS01 = xexp[2 * TY + w], hS02 = xexp[3 * TY + w];
             if (lane != 0) { hb0r = T(0); hb0i = T(0); hS01 = T(0); hS02 = T(0); }
             VecT oPr, oPi, oE0, oE1, oE2, oFr, oFi, oT0, oT1, oT2;
@@ -361,7 +377,8 @@ int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStrea
     // only) selects 8-row tiles, two CTAs per SM
     static const int ty = [] { const char* e = getenv("AHS_MARCH_TY"); return e ? atoi(e) : 4; }();
     if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, st);
-    return launch_cfg<T, 4, 4>(f, N, c, st);
+    if (ty == 16 && N % 16 == 0) return launch_cfg<T, 16, 1>(f, N, c, st);
+    return launch_cfg<T, 4, 3>(f, N, c, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu
