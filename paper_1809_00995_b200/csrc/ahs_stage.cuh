@@ -11,6 +11,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 namespace ahs {
 
@@ -68,6 +69,40 @@ template <typename T, int V>
 struct alignas(sizeof(T) * V) Vec {
     T v[V];
 };
+
+// ---- vector access helpers shared by the marching kernels -------------------------------------------------------
+template <typename T> struct NativeVec;
+template <> struct NativeVec<float> { using type = float4; };
+template <> struct NativeVec<double> { using type = double2; };
+
+template <typename T, int V>
+__device__ __forceinline__ Vec<T, V> lds_vec(const T* p) { return *reinterpret_cast<const Vec<T, V>*>(p); }
+template <typename T, int V>
+__device__ __forceinline__ void sts_vec(T* p, const Vec<T, V>& v) { *reinterpret_cast<Vec<T, V>*>(p) = v; }
+
+// streaming 16-byte global load / store (each momentum value is read once and written once per step)
+template <typename T, int V>
+__device__ __forceinline__ Vec<T, V> ldg_vec(const T* p)
+{
+    using NV = typename NativeVec<T>::type;
+    const NV n = __ldcs(reinterpret_cast<const NV*>(p));
+    Vec<T, V> r;
+    memcpy(&r, &n, sizeof(r));
+    return r;
+}
+template <typename T, int V>
+__device__ __forceinline__ void stg_vec(T* p, const Vec<T, V>& v)
+{
+    using NV = typename NativeVec<T>::type;
+    NV n;
+    memcpy(&n, &v, sizeof(n));
+    *reinterpret_cast<NV*>(p) = n;
+}
+
+// element v+1 of a vector, or the scalar `edge` (the first element of the next vector) for the last one
+template <typename T, int V>
+__device__ __forceinline__ T next_x(const Vec<T, V>& a, int v, T edge) { return v + 1 < V ? a.v[v + 1 < V ? v + 1 : v] : edge; }
+
 
 // Geometry of a staged tile.  NA = number of staged arrays.
 template <typename T, int V_, int TY_, int NA_, int NSTAGE_>

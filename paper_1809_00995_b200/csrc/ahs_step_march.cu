@@ -44,10 +44,6 @@ namespace {
 
 template <typename T> struct StepCoefT { T c1, c2, c3, d1, d2, d3, dt, sigma2; };
 
-template <typename T> struct NativeVec;
-template <> struct NativeVec<float> { using type = float4; };
-template <> struct NativeVec<double> { using type = double2; };
-
 template <typename T, int TY_>
 struct MarchCfg {
     static constexpr int V = 16 / sizeof(T);
@@ -61,34 +57,6 @@ struct MarchCfg {
     static constexpr int XEX_ELEMS = 4 * TY;              // b0.re, b0.im, S01, S02 of the halo column (one parity)
     static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * G::ARR_ELEMS + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
-
-template <typename T, int V>
-__device__ __forceinline__ Vec<T, V> lds_vec(const T* p) { return *reinterpret_cast<const Vec<T, V>*>(p); }
-template <typename T, int V>
-__device__ __forceinline__ void sts_vec(T* p, const Vec<T, V>& v) { *reinterpret_cast<Vec<T, V>*>(p) = v; }
-
-// streaming 16-byte global load / store (each momentum value is read once and written once per step)
-template <typename T, int V>
-__device__ __forceinline__ Vec<T, V> ldg_vec(const T* p)
-{
-    using NV = typename NativeVec<T>::type;
-    const NV n = __ldcs(reinterpret_cast<const NV*>(p));
-    Vec<T, V> r;
-    memcpy(&r, &n, sizeof(r));
-    return r;
-}
-template <typename T, int V>
-__device__ __forceinline__ void stg_vec(T* p, const Vec<T, V>& v)
-{
-    using NV = typename NativeVec<T>::type;
-    NV n;
-    memcpy(&n, &v, sizeof(n));
-    *reinterpret_cast<NV*>(p) = n;
-}
-
-// element v+1 of a vector, or the scalar `edge` (the first element of the next vector) for the last one
-template <typename T, int V>
-__device__ __forceinline__ T next_x(const Vec<T, V>& a, int v, T edge) { return v + 1 < V ? a.v[v + 1 < V ? v + 1 : v] : edge; }
 
 template <typename T, int TY, int MINB>
 __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k)

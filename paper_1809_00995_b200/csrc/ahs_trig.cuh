@@ -10,7 +10,7 @@
 //   sincos_fast(x): k = rint(x * 2/pi), r = x - k*pi/2 in [-pi/4, pi/4]; sin and cos polynomials; quadrant fix-up.
 //   sin_fast(x)   : fp32: k = rint(x / pi), r in [-pi/2, pi/2], odd polynomial, sign (-1)^k;
 //                   fp64: the quadrant form with the coefficient set chosen by the parity of k.
-// Measured against fp64 / long double references (csrc/fit_trig.py): fp32 sincos <= 0.9 ulp, fp32 sin <= 1.9 ulp
+// Measured against fp64 references (csrc/fit_trig.py): fp32 sincos <= 0.9 ulp, fp32 sin <= 1.9 ulp
 // (abs 1.2e-7), fp64 <= 1.3 ulp.  Domain: |x| < 2^22 * pi/2 (fp32: 6.5e6; fp64: |x| < 2^30); beyond it the result
 // is finite garbage or NaN (a link angle that large has no phase information left in fp32 anyway); NaN and Inf
 // inputs give NaN, so blown-up lattices still reach the diagnostics' non-finite flag.
@@ -59,6 +59,27 @@ __device__ __forceinline__ float sin_fast(float x)
     p = fmaf(z, p, -0.1666666716337204f);
     const float sr = fmaf(r * z, p, r);
     return __int_as_float(__float_as_int(sr) ^ (q << 31));
+}
+
+// atan2 for the winding fast path (ahs_diag_march.cu): branch-free, absolute error <= 2.5e-7 rad in the fp32 emulation of
+// fit_trig.py (the fast path's error budget assumes <= 4.8e-7).  q = min/max in [0, 1], odd polynomial of degree 15, then
+// the octant fix-ups.  atan2_fast(0, 0) and non-finite inputs give NaN, which sends the link to the fp64 evaluation.
+__device__ __forceinline__ float atan2_fast(float y, float x)
+{
+    const float ax = fabsf(x), ay = fabsf(y);
+    const float q = __fdividef(fminf(ax, ay), fmaxf(ax, ay));
+    const float z = q * q;
+    float p = fmaf(z, -0.004054565913975239f, 0.021862955763936043f);
+    p = fmaf(z, p, -0.055912330746650696f);
+    p = fmaf(z, p, 0.096421979367733f);
+    p = fmaf(z, p, -0.1390863060951233f);
+    p = fmaf(z, p, 0.19946566224098206f);
+    p = fmaf(z, p, -0.33329859375953674f);
+    p = fmaf(z, p, 0.9999993443489075f);
+    float r = q * p;
+    r = ay > ax ? 1.5707963705062866f - r : r;
+    r = x < 0 ? 3.1415927410125732f - r : r;
+    return copysignf(r, y);
 }
 
 // ---- fp64 ---------------------------------------------------------------------------------------------------------------

@@ -309,3 +309,34 @@ def test_create_rejects_bad_arguments(ahs):
     for kw in (dict(N=2), dict(N=32, dt=0.0), dict(N=32, tau0=0.01, m=1.0), dict(N=32, precision="f32", kernel="march")):
         with pytest.raises(ahs.AhsError):
             ahs.Simulation(**kw)
+
+
+@pytest.mark.parametrize("prec,N", [("f64", 64), ("f32", 128)])
+def test_winding_bit_exact_when_links_sit_next_to_ties(ahs, oracle, prec, N):
+    """The marching diagnostics kernel decides rint() from fp32 phases and falls back to fp64 when a link is within
+    4e-6 (1 + |t|) turns of a half-integer.  Here a third of the links are PUT next to a tie, at
+    distances from 1e-12 to 1e-4 turns on either side, so fast path, fallback and the boundary between them are all
+    hit; the count must still equal the oracle's fp64 decision, integer for integer."""
+    rng = np.random.default_rng(20260101 + N)
+    f = np.zeros((10, N, N, N))
+    ph = rng.uniform(-np.pi, np.pi, (N, N, N))
+    mod = 1.0 + 0.3 * rng.standard_normal((N, N, N))
+    f[0], f[1] = mod * np.cos(ph), mod * np.sin(ph)
+    f = rounded(f, prec)
+    arg = np.arctan2(f[1], f[0])
+    for i, ax in enumerate((2, 1, 0)):                      # direction i = x, y, z <-> numpy axis 2, 1, 0
+        d = np.roll(arg, -1, axis=ax) - arg
+        turns = rng.integers(-2, 3, (N, N, N)) + 0.5
+        off = rng.choice([-1.0, 1.0], (N, N, N)) * 10.0 ** rng.uniform(-12, -4, (N, N, N))
+        near = d - 2 * np.pi * (turns + off)                # (d - theta) / 2 pi = turns + off
+        plain = 0.3 * rng.standard_normal((N, N, N))
+        f[4 + i] = np.where(rng.random((N, N, N)) < 1 / 3, near, plain)
+    f = rounded(f, prec)
+    p = oracle.Params(N=N, m=1.0, s=0.0)
+    for kernel in ("auto", "generic"):
+        with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.0, ic="none", kernel=kernel) as sim:
+            sim.set_fields(f, 0)
+            d = sim.diagnostics()
+        r = oracle.diagnostics(p, f, 0)
+        assert r["n_pierced"] > N ** 3 // 10
+        assert (d["n_pierced"], d["sum_abs_w"]) == (r["n_pierced"], r["sum_abs_w"]), kernel
