@@ -143,7 +143,8 @@ int do_diag(ahs_sim* s)
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
     const DiagCoef c = diag_coefficients(s->p, s->step);
     return s->kernel == AHS_KERNEL_MARCH
-               ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream)
+               ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result,
+                                      slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1), 5 * s->array_bytes, s->stream)   // shadow buffer: dead between steps
                : launch_diag_generic<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream);
 }
 

@@ -3,18 +3,20 @@
 //
 // Same tile and staging as the step kernel (ahs_step_march.cu): a CTA owns TX x TY sites in (x, y) and marches over
 // `zlen` planes; phi_re, phi_im, theta_0..2 of plane k+3 are streamed by cp.async.bulk into a 4-stage ring of halo'd
-// shared-memory tiles while planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
+// shared-memory tiles (full / empty mbarrier pairs) while planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
 // All the estimators need only FORWARD neighbours (x+k_i, x+k_i+k_j) of phi, theta -- except the divergence of eps,
 // whose -x / -y / -z terms come by shuffle, one extra row load and a carried register.
 //
-// Winding, compute-once form.  arg phi is evaluated ONCE per site (phase A: plane k+1 -> a shared "arg tile", plus the
-// forward halo row/column shared out over the threads), one CTA barrier, then (phase B) every link number
-//     n_i^x = rint((arg^{x+k_i} - arg^x - theta_i^x) / 2 pi)
-// a plaquette needs is formed from the arg tiles of planes k and k+1 and W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x)
-// is summed exactly.  The decision is the fp64 one: the arg tile holds atan2f values (error
-// <= 2 ulp(pi) = 5e-7 rad), the quotient is formed in fp32 from them, and any link whose quotient lies within
-// 1e-5 (1 + |t|) of a half-integer -- thirty times the worst-case error -- is redone with fp64 atan2 of both ends, so every
-// rint is the one an all-fp64 evaluation takes (probability of the slow path: 4e-5 per link at |theta| <~ 1).
+// Winding.  Every thread evaluates arg phi (branch-free atan2_fast) at the ten points of plane k+1 its V sites need and
+// carries them to the next plane in registers; there is NO exchange between warps and therefore no CTA barrier in the
+// march: the warps of a CTA drift freely and meet only at the stage ring's full / empty mbarriers (an earlier version
+// computed each phase once into a shared arg tile and lost 31 % of its issue slots at the per-plane barrier, profiles/r2).
+// The link numbers n_i^x = rint((arg^{x+k_i} - arg^x - theta_i^x) / 2 pi) are formed in fp32 and
+// W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x) is summed exactly.  The decision is the fp64 one:
+// a phase is off by <= 6e-7 rad, a quotient by <= 3.5e-7 + 2.5e-7 |t| turns, and whenever a link of a thread-plane lies
+// within 4e-6 (1 + |t|) turns of a half-integer -- ten times that bound -- the thread redoes the plane's plaquettes with
+// fp64 atan2 in a second pass over a device-side doubt list (diag_resolve_kernel; ~4e-4 of the thread-planes), so every
+// rint is the one an all-fp64 evaluation takes and the march itself never diverges.
 // <v^2>_L sums: products and the sum over the 16-byte vector of a thread in the storage type, then fp64 accumulation.
 // The paper runs Winding and VelRWLag as two kernels over raw fields with a CUB block sum and a host-side final sum
 // (L140); this is a different design.
@@ -41,22 +43,14 @@ struct DiagCfg {
     using G = TileGeom<T, V, TY, 5, NSTAGE>;                 // a stage: phi_re, phi_im, theta_0, theta_1, theta_2 of one plane
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
-    static constexpr int APITCH = TX + 4;                    // arg tile: rows 0 .. TY, columns 0 .. TX (floats)
-    static constexpr int ATILE = (TY + 1) * APITCH;
-    static constexpr int NARG = 3;                           // planes k, k+1 in use while k+2's slot may still be read
-    static constexpr int NJOBS = TX + 1 + TY;                // forward halo: row TY (TX+1 sites) and column TX (TY sites)
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS) + sizeof(float) * (size_t)(NARG * ATILE);
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS);
 };
-
-template <int V> struct FVec;
-template <> struct FVec<4> { using type = float4; };
-template <> struct FVec<2> { using type = float2; };
 
 // Link number of the link s -> t with angle th, fast path, all in fp32: t = (arg_t - arg_s - th) / 2 pi from the
 // atan2_fast phases of the arg tile, n = rint(t) (ties to even) as a float.  |t - t_exact| <= 3.5e-7 + 2.5e-7 |t| turns
 // (6e-7 rad per phase, three roundings, the fp32 constant), so whenever |t - n| < 1/2 - kTieMargin (1 + |t|), n IS the
-// fp64 decision.  `slack` keeps the smallest margin seen; the caller redoes the whole thread-plane in fp64
-// (winding_fp64, out of line) when it is not positive.  Everything here is branch-free.
+// fp64 decision.  `slack` keeps the smallest margin seen; when it is not positive the caller drops the thread-plane's
+// fast count and appends the thread-plane to the doubt list (diag_resolve_kernel).  Everything here is branch-free.
 __device__ __forceinline__ float link_number(float as, float at, float th, float& slack)
 {
     const float t = ((at - as) - th) * 0.15915494309189535f;
@@ -65,54 +59,60 @@ __device__ __forceinline__ float link_number(float as, float at, float th, float
     return n;
 }
 
-// The winding of the V sites of one thread in one plane, every phase and every quotient in fp64, straight from the
-// staged raw fields (same arithmetic as diag_generic_kernel).  Returns n_pierced | sum|W| << 16.  Out of line on purpose:
-// it runs for ~4e-4 of the thread-planes, and thirty inlined copies of the fp64 atan2 made the loop overflow the
-// instruction cache (profiles/r2).
-template <typename T, typename G>
-__device__ __noinline__ unsigned winding_fp64(const T* sc, const T* sn, int w, int xi)
+// Second pass over the doubt list: the winding of the V sites of each listed (x/V, y, z), every phase and every quotient
+// in fp64 straight from global memory (same arithmetic as diag_generic_kernel), added to one extra partial record.
+// Integer sums: the order of the atomics does not matter.  ~4e-4 of the thread-planes end up here on smooth or random
+// fields; resolving them in-line (an out-of-line call inside the march) made every warp of the CTA wait for the one
+// that took the slow path (profiles/r2: 30 % of the issue slots), a separate pass costs ~0.1 ms at 1024^3.
+template <typename T>
+__global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N, const unsigned* __restrict__ list,
+                                                           const unsigned long long* __restrict__ count, DiagPartial* __restrict__ extra)
 {
-    constexpr int V = G::V;
-    double a[2][2][V + 1];
-    for (int pl = 0; pl < 2; ++pl)
-        for (int r = 0; r < 2; ++r)
-            for (int c = 0; c <= V; ++c) {
-                const T* st = pl ? sn : sc;
-                a[pl][r][c] = atan2((double)st[G::idx(1, w + r, xi + c)], (double)st[G::idx(0, w + r, xi + c)]);
-            }
-    auto ln = [](double as, double at, T th) { return (int)rint((at - as - (double)th) * kInv2Pi); };
+    constexpr int V = 16 / sizeof(T);
+    const unsigned long long n = *count;
     unsigned pierced = 0u, absw = 0u;
-    for (int v = 0; v < V; ++v) {
-        const int n0 = ln(a[0][0][v], a[0][0][v + 1], sc[G::idx(2, w, xi + v)]);
-        const int n1 = ln(a[0][0][v], a[0][1][v], sc[G::idx(3, w, xi + v)]);
-        const int n2 = ln(a[0][0][v], a[1][0][v], sc[G::idx(4, w, xi + v)]);
-        const int n1x = ln(a[0][0][v + 1], a[0][1][v + 1], sc[G::idx(3, w, xi + v + 1)]);
-        const int n2x = ln(a[0][0][v + 1], a[1][0][v + 1], sc[G::idx(4, w, xi + v + 1)]);
-        const int n0y = ln(a[0][1][v], a[0][1][v + 1], sc[G::idx(2, w + 1, xi + v)]);
-        const int n2y = ln(a[0][1][v], a[1][1][v], sc[G::idx(4, w + 1, xi + v)]);
-        const int n0z = ln(a[1][0][v], a[1][0][v + 1], sn[G::idx(2, w, xi + v)]);
-        const int n1z = ln(a[1][0][v], a[1][1][v], sn[G::idx(3, w, xi + v)]);
-        const int W01 = -(n0 + n1x - n0y - n1), W02 = -(n0 + n2x - n0z - n2), W12 = -(n1 + n2y - n1z - n2);
-        pierced += (W01 != 0) + (W02 != 0) + (W12 != 0);
-        absw += (unsigned)(abs(W01) + abs(W02) + abs(W12));
+    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned u = list[e];
+        const int xv = (int)(u & 1023u), y = (int)((u >> 10) & 2047u), z = (int)(u >> 21);
+        const int yp = y + 1 == N ? 0 : y + 1, zp = z + 1 == N ? 0 : z + 1;
+        auto at = [&](int x, int yy, int zz) { return ((size_t)zz * N + (size_t)yy) * N + (size_t)x; };
+        auto arg = [&](size_t i) { return atan2((double)f.phi_im[i], (double)f.phi_re[i]); };
+        auto ln = [](double as, double a_t, T th) { return (int)rint((a_t - as - (double)th) * kInv2Pi); };
+        for (int v = 0; v < V; ++v) {
+            const int x = xv * V + v, xp = x + 1 == N ? 0 : x + 1;
+            const size_t s0 = at(x, y, z), sx = at(xp, y, z), sy = at(x, yp, z), sz = at(x, y, zp);
+            const double a0 = arg(s0), ax = arg(sx), ay = arg(sy), az = arg(sz);
+            const double axy = arg(at(xp, yp, z)), axz = arg(at(xp, y, zp)), ayz = arg(at(x, yp, zp));
+            const int n0 = ln(a0, ax, f.th[0][s0]), n1 = ln(a0, ay, f.th[1][s0]), n2 = ln(a0, az, f.th[2][s0]);
+            const int n1x = ln(ax, axy, f.th[1][sx]), n2x = ln(ax, axz, f.th[2][sx]);
+            const int n0y = ln(ay, axy, f.th[0][sy]), n2y = ln(ay, ayz, f.th[2][sy]);
+            const int n0z = ln(az, axz, f.th[0][sz]), n1z = ln(az, ayz, f.th[1][sz]);
+            const int W01 = -(n0 + n1x - n0y - n1), W02 = -(n0 + n2x - n0z - n2), W12 = -(n1 + n2y - n1z - n2);
+            pierced += (W01 != 0) + (W02 != 0) + (W12 != 0);
+            absw += (unsigned)(abs(W01) + abs(W02) + abs(W12));
+        }
     }
-    return pierced | (absw << 16);
+    unsigned long long p64 = warp_sum((unsigned long long)pierced), w64 = warp_sum((unsigned long long)absw);
+    if ((threadIdx.x & 31) == 0 && (p64 | w64)) {
+        atomicAdd(&extra->n_pierced, p64);
+        atomicAdd(&extra->sum_abs_w, w64);
+    }
 }
 
 template <typename T, int TY, int MINB>
 __global__ void __launch_bounds__(DiagCfg<T, TY>::NTHREADS, MINB)
-diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials)
+diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
+                  unsigned long long* __restrict__ doubt_count)
 {
     using C = DiagCfg<T, TY>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
-    using FV = typename FVec<C::V>::type;
-    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS, ARR = G::ARR_ELEMS, AP = C::APITCH;
+    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS;
 
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
+    uint64_t* empty = full + NS;                           // empty[s]: all TY warps have finished reading stage s
     T* stages = reinterpret_cast<T*>(smem + 128);
-    float* argt = reinterpret_cast<float*>(stages + NS * SE);
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tiles_x = N / TX, tiles_y = N / TY;
@@ -129,7 +129,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
 
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], TY); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -146,35 +146,33 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         }
     }
 
-    // phase A of a plane: arg phi of the tile (own sites, then the forward halo row and column) -> arg tile `dst`
-    auto fill_args = [&](const T* st, float* dst, int rot) {
+    // arg phi at the V sites of this thread and at the site right of them, rows w and w+1 of a staged plane.  Every
+    // thread evaluates the ten phases it needs itself (2.5 per site instead of 1): no exchange, hence no CTA barrier
+    // anywhere in the march -- the warps of a CTA drift freely and only meet at the stage ring's mbarriers.
+    auto args_of = [&](const T* st, float (&a0)[V + 1], float (&a1)[V + 1]) {
         const VecT pr = lds_vec<T, V>(st + G::idx(0, w, xi)), pi = lds_vec<T, V>(st + G::idx(1, w, xi));
-        float a[V];
+        const VecT pry = lds_vec<T, V>(st + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(st + G::idx(1, w + 1, xi));
 #pragma unroll
-        for (int v = 0; v < V; ++v) a[v] = atan2_fast((float)pi.v[v], (float)pr.v[v]);
-        FV av;
-        memcpy(&av, a, sizeof(av));
-        *reinterpret_cast<FV*>(dst + w * AP + xi) = av;
-        const int t = (threadIdx.x + 32 * rot) % C::NTHREADS;   // the halo jobs rotate over the warps
-        for (int j = t; j < C::NJOBS; j += C::NTHREADS) {
-            const int r = j <= TX ? TY : j - (TX + 1), c = j <= TX ? j : TX;
-            dst[r * AP + c] = atan2_fast((float)st[G::idx(1, r, c)], (float)st[G::idx(0, r, c)]);
+        for (int v = 0; v < V; ++v) {
+            a0[v] = atan2_fast((float)pi.v[v], (float)pr.v[v]);
+            a1[v] = atan2_fast((float)piy.v[v], (float)pry.v[v]);
         }
+        a0[V] = atan2_fast((float)st[G::idx(1, w, xi + V)], (float)st[G::idx(0, w, xi + V)]);
+        a1[V] = atan2_fast((float)st[G::idx(1, w + 1, xi + V)], (float)st[G::idx(0, w + 1, xi + V)]);
     };
 
     mbar_wait(&full[0], 0);
-    fill_args(stages, argt, 0);
-    __syncthreads();
-    // n_0, n_1 of the current plane (own sites; n_1 also right of the vector), carried along the march, with their margin
-    float n0c[V], n1c[V + 1], slack_c = 1.0f;
+    // phases of the current plane and n_0, n_1 of its links (own sites; n_1 also right of the vector), carried along
+    // the march together with the smallest margin of those link numbers
+    float a[V + 1], ay[V + 1], n0c[V], n1c[V + 1], slack_c = 1.0f;
+    args_of(stages, a, ay);
     {
         const VecT t0 = lds_vec<T, V>(stages + G::idx(2, w, xi)), t1 = lds_vec<T, V>(stages + G::idx(3, w, xi));
         const T t1x_e = stages[G::idx(3, w, xi + V)];
 #pragma unroll
         for (int v = 0; v <= V; ++v) {
-            const float as = argt[w * AP + xi + v], ay = argt[(w + 1) * AP + xi + v];
-            n1c[v] = link_number(as, ay, (float)(v < V ? t1.v[v < V ? v : 0] : t1x_e), slack_c);
-            if (v < V) n0c[v < V ? v : 0] = link_number(as, argt[w * AP + xi + v + 1], (float)t0.v[v < V ? v : 0], slack_c);
+            n1c[v] = link_number(a[v], ay[v], (float)(v < V ? t1.v[v < V ? v : 0] : t1x_e), slack_c);
+            if (v < V) n0c[v < V ? v : 0] = link_number(a[v], a[v < V ? v + 1 : v], (float)t0.v[v < V ? v : 0], slack_c);
         }
     }
 
@@ -193,8 +191,14 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     for (int it = 0; it < zlen; ++it) {
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
-        const float* ac = argt + (it % C::NARG) * C::ATILE;
-        float* an = argt + ((it + 1) % C::NARG) * C::ATILE;
+
+        // plane it+3 -> the stage that held plane it-1, once all TY warps have released it
+        if (w == 0 && it + NS - 1 <= zlen && elect_one()) {
+            const int s = (it + NS - 1) % NS;
+            if (it > 0) mbar_wait(&empty[s], ((it - 1) / NS) & 1);
+            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES);
+            issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + NS - 1));
+        }
 
         const int z = z0 + it, y = y0 + w;
         const size_t grow = ((size_t)z * N + (size_t)y) * N;
@@ -207,15 +211,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         if (lane == 0) e0_halo = f.eps[0][grow + (size_t)(x0 == 0 ? N - 1 : x0 - 1)];
 
         mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
-        fill_args(sn, an, it + 1);
-        __syncthreads();
-
-        // plane it+3 -> the stage that held plane it-1 (its last readers, phase B of iteration it-1, passed the barrier above)
-        if (((w + it) % TY) == 0 && it + NS - 1 <= zlen && elect_one()) {
-            const int s = (it + NS - 1) % NS;
-            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES);
-            issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + NS - 1));
-        }
+        float az[V + 1], azy[V + 1];
+        args_of(sn, az, azy);
 
         // ---- phase B: everything of plane `it` ---------------------------------------------------------------------------
         const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
@@ -226,15 +223,6 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
         const T prx_e = sc[G::idx(0, w, xi + V)], pix_e = sc[G::idx(1, w, xi + V)];
         const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = sc[G::idx(4, w, xi + V)];
-        // arg tiles: this plane (rows w, w+1) and the next (rows w, w+1), each with the element right of the vector
-        float a[V + 1], ay[V + 1], az[V + 1], azy[V + 1];
-        {
-            const FV va = *reinterpret_cast<const FV*>(ac + w * AP + xi), vy = *reinterpret_cast<const FV*>(ac + (w + 1) * AP + xi);
-            const FV vz = *reinterpret_cast<const FV*>(an + w * AP + xi), vzy = *reinterpret_cast<const FV*>(an + (w + 1) * AP + xi);
-            memcpy(a, &va, sizeof(va)); memcpy(ay, &vy, sizeof(vy)); memcpy(az, &vz, sizeof(vz)); memcpy(azy, &vzy, sizeof(vzy));
-            a[V] = ac[w * AP + xi + V]; ay[V] = ac[(w + 1) * AP + xi + V];
-            az[V] = an[w * AP + xi + V]; azy[V] = an[(w + 1) * AP + xi + V];
-        }
         // E0 of the site to the left: previous element, else lane-1's last element, else (lane 0) the halo value
         T e0_left = __shfl_up_sync(0xffffffffu, E0.v[V - 1], 1);
         if (lane == 0) e0_left = e0_halo;
@@ -270,16 +258,17 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         }
         unsigned absw_u = (unsigned)abs_w;
         if (!(fminf(slack, slack_c) > 0.0f) || !(abs_w < 1.0e6f)) {   // a link too close to a tie (or NaN / huge): fp64 decides
-            const unsigned r = winding_fp64<T, G>(sc, sn, w, xi);
-            pierced = r & 0xffffu;
-            absw_u = r >> 16;
+            const unsigned long long e = atomicAdd(doubt_count, 1ull);
+            doubt_list[e] = (unsigned)((x0 + xi) / V) | ((unsigned)(y0 + w) << 10) | ((unsigned)(z0 + it) << 21);
+            pierced = 0u;
+            absw_u = 0u;
         }
         n_pierced += pierced;
         sum_abs_w += absw_u;
 #pragma unroll
         for (int v = 0; v < V; ++v) n0c[v] = n0z[v];
 #pragma unroll
-        for (int v = 0; v <= V; ++v) n1c[v] = n1z[v];
+        for (int v = 0; v <= V; ++v) { n1c[v] = n1z[v]; a[v] = az[v]; ay[v] = azy[v]; }
 
         T p_num = T(0), p_den = T(0), p_l = T(0), p_r2 = T(0);   // per thread and plane (V sites), then into the fp64 sums
 #pragma unroll
@@ -325,6 +314,9 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         }
         num += (double)p_num; den += (double)p_den; lsum += (double)p_l; rhs2 += (double)p_r2;
         E2m = E2;
+        // this warp is done with stage `sc` (plane it): release it to the copy-issuing thread
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[it % NS]);
     }
 
     gmax = (double)gmax_t;
@@ -339,14 +331,15 @@ int pick_zlen(int N, int ctas_per_sm, int max_partials)
     const long tiles = (long)(N / C::TX) * (N / TY);
     const int cands[5] = { 128, 64, 32, 16, 8 };
     for (int c : cands)   // the longest march that still gives >= 4 waves of resident CTAs (the prologue costs one plane)
-        if (N % c == 0 && tiles * (N / c) <= max_partials && tiles * (N / c) >= 4L * ctas_per_sm * 148) return c;
+        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials && tiles * (N / c) >= 4L * ctas_per_sm * 148) return c;
     for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) <= max_partials) return c;
+        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials) return c;
     return N;
 }
 
 template <typename T, int TY, int MINB>
-int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result, cudaStream_t st)
+int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
+               void* list, size_t list_bytes, cudaStream_t st)
 {
     using C = DiagCfg<T, TY>;
     auto kern = diag_march_kernel<T, TY, MINB>;
@@ -358,26 +351,33 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
     static const int zlen_env = [] { const char* e = getenv("AHS_DIAG_ZLEN"); return e ? atoi(e) : 0; }();
     const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB, max_partials);
     const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
-    if (blocks > max_partials) return AHS_ERR_INVALID_ARG;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials);
+    // partials[blocks] collects the second pass, partials[blocks + 1].n_pierced is the length of the doubt list
+    if (blocks + 2 > max_partials || list_bytes < sizeof(unsigned) * ((size_t)N * N * N / C::V)) return AHS_ERR_INVALID_ARG;
+    DiagPartial* extra = partials + blocks;
+    unsigned long long* count = &partials[blocks + 1].n_pierced;
+    if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
-    const int r = launch_diag_finish(partials, (int)blocks, result, st);
-    return r < 0 ? r : 2;
+    diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
+    if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
+    const int r = launch_diag_finish(partials, (int)blocks + 1, result, st);
+    return r < 0 ? r : 3;
 }
 
 }  // namespace
 
 template <typename T>
-int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result, cudaStream_t st)
+int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
+                      void* list, size_t list_bytes, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
     // 4-row tiles (3 CTAs/SM) by default; AHS_DIAG_TY=8 selects 8-row tiles, two CTAs per SM (experiments)
     static const int ty = [] { const char* e = getenv("AHS_DIAG_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, st);
-    return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, st);
+    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, list, list_bytes, st);
+    return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, list, list_bytes, st);
 }
 
-template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, cudaStream_t);
-template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, cudaStream_t);
+template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, cudaStream_t);
+template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, cudaStream_t);
 
 }  // namespace ahs

@@ -66,8 +66,9 @@ template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const 
 template <typename T> bool march_supported(int N);
 template <typename T> int launch_diag_generic(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
                                               int max_partials, DiagPartial* result, cudaStream_t st);
+// `list`: DEVICE scratch of >= 4 N^3 / (16 / sizeof(T)) bytes for the winding doubt list (the dead phi', theta' shadow buffer)
 template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
-                                            int max_partials, DiagPartial* result, cudaStream_t st);
+                                            int max_partials, DiagPartial* result, void* list, size_t list_bytes, cudaStream_t st);
 int launch_diag_finish(const DiagPartial* partials, int n, DiagPartial* result, cudaStream_t st);
 template <typename T> int launch_convert_from_double(const double* src, T* dst, int64_t n, cudaStream_t st);
 template <typename T> int launch_convert_to_double(const T* src, double* dst, int64_t n, cudaStream_t st);
