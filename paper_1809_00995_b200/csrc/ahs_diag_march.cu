@@ -40,7 +40,7 @@ struct DiagCfg {
     static constexpr int V = 16 / sizeof(T);
     static constexpr int TY = TY_;
     static constexpr int NSTAGE = 4;
-    using G = TileGeom<T, V, TY, 5, NSTAGE>;                 // a stage: phi_re, phi_im, theta_0, theta_1, theta_2 of one plane
+    using G = TileGeom<T, V, TY, 5, NSTAGE, 0, 0>;           // a stage: phi_re, phi_im, theta_0..2 of one plane, forward halo only
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
     static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS);

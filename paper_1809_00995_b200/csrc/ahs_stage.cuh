@@ -108,24 +108,28 @@ template <typename T, int V>
 __device__ __forceinline__ T next_x(const Vec<T, V>& a, int v, T edge) { return v + 1 < V ? a.v[v + 1 < V ? v + 1 : v] : edge; }
 
 
-// Geometry of a staged tile.  NA = number of staged arrays.
-template <typename T, int V_, int TY_, int NA_, int NSTAGE_>
+// Geometry of a staged tile.  NA = number of staged arrays; LH = halo columns left of the tile (V or 0), BH = halo rows
+// below it (1 or 0).  The forward halo (V columns right, one row above) is always there.
+template <typename T, int V_, int TY_, int NA_, int NSTAGE_, int LH_ = V_, int BH_ = 1>
 struct TileGeom {
     static constexpr int V = V_;
     static constexpr int TY = TY_;
     static constexpr int NA = NA_;
     static constexpr int NSTAGE = NSTAGE_;
+    static constexpr int LH = LH_;
+    static constexpr int BH = BH_;
     static constexpr int TX = 32 * V;              // one warp spans the tile in x
-    static constexpr int PITCH = TX + 2 * V;       // x0-V .. x0+TX+V-1
-    static constexpr int ROWS = TY + 2;            // y0-1 .. y0+TY
+    static constexpr int PITCH = TX + LH + V;      // x0-LH .. x0+TX+V-1
+    static constexpr int ROWS = TY + BH + 1;       // y0-BH .. y0+TY
     static constexpr int ARR_ELEMS = ROWS * PITCH;
     static constexpr int STAGE_ELEMS = NA * ARR_ELEMS;
     static constexpr uint32_t STAGE_BYTES = STAGE_ELEMS * sizeof(T);
     static constexpr uint32_t ARR_BYTES = ARR_ELEMS * sizeof(T);
     static_assert(sizeof(T) * V == 16, "a vector is 16 bytes");
+    static_assert(LH == 0 || LH == V, "the left halo is one vector or nothing");
 
-    // element (array a, row r in [-1, TY], column xi in [-V, TX+V)) of a stage
-    __device__ __forceinline__ static int idx(int a, int r, int xi) { return (a * ROWS + (r + 1)) * PITCH + (xi + V); }
+    // element (array a, row r in [-BH, TY], column xi in [-LH, TX+V)) of a stage
+    __device__ __forceinline__ static int idx(int a, int r, int xi) { return (a * ROWS + (r + BH)) * PITCH + (xi + LH); }
 };
 
 // Issue the copies of one z-plane of NA arrays into NA consecutive array slots at `dst`.  Called by ONE thread, after
@@ -138,13 +142,13 @@ struct TileGeom {
 template <typename G, int NA, typename T>
 __device__ __forceinline__ void issue_rows(T* dst_base, uint64_t* bar, const T* const (&src)[NA], int N, int x0, int y0, int z)
 {
-    const bool x_interior = (x0 > 0) && (x0 + G::TX < N);
-    const bool y_interior = (y0 > 0) && (y0 + G::TY < N);
+    const bool x_interior = (G::LH == 0 || x0 > 0) && (x0 + G::TX < N);
+    const bool y_interior = (G::BH == 0 || y0 > 0) && (y0 + G::TY < N);
     const size_t plane = (size_t)z * N * N;
     if (x_interior && y_interior) {
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            const T* row = src[a] + plane + (size_t)(y0 - 1) * N + (x0 - G::V);
+            const T* row = src[a] + plane + (size_t)(y0 - G::BH) * N + (x0 - G::LH);
             T* dst = dst_base + a * G::ARR_ELEMS;
 #pragma unroll
             for (int rr = 0; rr < G::ROWS; ++rr) bulk_g2s(dst + rr * G::PITCH, row + (size_t)rr * N, G::PITCH * sizeof(T), bar);
@@ -158,15 +162,15 @@ __device__ __forceinline__ void issue_rows(T* dst_base, uint64_t* bar, const T* 
         T* dst = dst_base + a * G::ARR_ELEMS;
 #pragma unroll 1
         for (int rr = 0; rr < G::ROWS; ++rr) {
-            int y = y0 + rr - 1;
+            int y = y0 + rr - G::BH;
             y = y < 0 ? y + N : (y >= N ? y - N : y);
             const T* row = src[a] + plane + (size_t)y * N;
             if (x_interior) {
-                bulk_g2s(dst + rr * G::PITCH, row + x0 - G::V, G::PITCH * sizeof(T), bar);
+                bulk_g2s(dst + rr * G::PITCH, row + x0 - G::LH, G::PITCH * sizeof(T), bar);
             } else {
-                bulk_g2s(dst + rr * G::PITCH, row + xl, 16, bar);
-                bulk_g2s(dst + rr * G::PITCH + G::V, row + x0, G::TX * sizeof(T), bar);
-                bulk_g2s(dst + rr * G::PITCH + G::V + G::TX, row + xr, 16, bar);
+                if (G::LH > 0) bulk_g2s(dst + rr * G::PITCH, row + xl, 16, bar);
+                bulk_g2s(dst + rr * G::PITCH + G::LH, row + x0, G::TX * sizeof(T), bar);
+                bulk_g2s(dst + rr * G::PITCH + G::LH + G::TX, row + xr, 16, bar);
             }
         }
     }
