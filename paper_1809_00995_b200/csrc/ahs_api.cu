@@ -28,6 +28,8 @@ struct ahs_sim {
     DiagPartial* result_host;  // pinned host, 1 record
     int64_t diag_step;       // step the pending diagnostics launch refers to (-1: none)
     int device;
+    CUtensorMap diag_map[2];   // TMA descriptors of (phi, theta) buffer 0 / 1 for the diagnostics march
+    bool diag_map_ok;
 };
 
 namespace {
@@ -144,7 +146,8 @@ int do_diag(ahs_sim* s)
     const DiagCoef c = diag_coefficients(s->p, s->step);
     return s->kernel == AHS_KERNEL_MARCH
                ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result,
-                                      slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1), 5 * s->array_bytes, s->stream)   // shadow buffer: dead between steps
+                                      slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1), 5 * s->array_bytes,
+                                      s->diag_map_ok ? &s->diag_map[s->cur] : nullptr, s->stream)   // shadow buffer: dead between steps
                : launch_diag_generic<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream);
 }
 
@@ -227,6 +230,15 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     s->result = s->partials + kMaxDiagPartials;
     ce = cudaMallocHost((void**)&s->result_host, sizeof(DiagPartial));
     if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMallocHost: %s", cudaGetErrorString(ce)); ahs_destroy(s); return nullptr; }
+
+    s->diag_map_ok = false;
+    if (s->kernel == AHS_KERNEL_MARCH) {
+        s->diag_map_ok = p.precision == AHS_F32
+            ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
+              make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)
+            : make_diag_march_map<double>(&s->diag_map[0], slot<double>(s, PHI_RE0), p.N, s->array_bytes) &&
+              make_diag_march_map<double>(&s->diag_map[1], slot<double>(s, PHI_RE1), p.N, s->array_bytes);
+    }
 
     // initial condition (L72): everything zero, then phi from Philox
     ce = cudaMemsetAsync(s->base, 0, (size_t)NUM_SLOTS * s->array_bytes, s->stream);

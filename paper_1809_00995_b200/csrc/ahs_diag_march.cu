@@ -21,11 +21,13 @@
 // The paper runs Winding and VelRWLag as two kernels over raw fields with a CUB block sum and a host-side final sum
 // (L140); this is a different design.
 #include <cstdlib>
+#include <cstring>
 
 #include "ahs_internal.cuh"
 #include "ahs_math.cuh"
 #include "ahs_reduce.cuh"
 #include "ahs_stage.cuh"
+#include "ahs_tma.cuh"
 #include "ahs_trig.cuh"
 
 namespace ahs {
@@ -43,7 +45,8 @@ struct DiagCfg {
     using G = TileGeom<T, V, TY, 5, NSTAGE, 0, 0>;           // a stage: phi_re, phi_im, theta_0..2 of one plane, forward halo only
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS);
+    static constexpr int STAGE_STRIDE = (int)(((G::STAGE_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * STAGE_STRIDE);
 };
 
 // Link number of the link s -> t with angle th, fast path, all in fp32: t = (arg_t - arg_s - th) / 2 pi from the
@@ -102,12 +105,12 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
 template <typename T, int TY, int MINB>
 __global__ void __launch_bounds__(DiagCfg<T, TY>::NTHREADS, MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
-                  unsigned long long* __restrict__ doubt_count)
+                  unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap, int use_tma)
 {
     using C = DiagCfg<T, TY>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
-    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS;
+    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = C::STAGE_STRIDE;
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
@@ -136,14 +139,17 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
 
     // plane index p of this CTA's march = lattice plane z0 + p (periodic); planes 0 .. zlen are needed
     auto plane_of = [&](int p) { const int z = z0 + p; return z >= N ? z - N : z; };
+    // one tensor copy per plane for tiles that do not touch the periodic boundary, row copies for the others
+    const bool tma_tile = use_tma && (x0 + TX < N) && (y0 + TY < N);
+    auto issue_plane = [&](int s, int p) {
+        mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES);
+        if (tma_tile) tma_load_4d(stages + s * SE, &tmap, x0, y0, plane_of(p), 0, &full[s]);
+        else issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+    };
     if (w == 0 && elect_one()) {
 #pragma unroll
-        for (int p = 0; p < NS - 1; ++p) {
-            if (p <= zlen) {
-                mbar_arrive_expect_tx(&full[p], G::STAGE_BYTES);
-                issue_rows<G, 5>(stages + p * SE, &full[p], src, N, x0, y0, plane_of(p));
-            }
-        }
+        for (int p = 0; p < NS - 1; ++p)
+            if (p <= zlen) issue_plane(p, p);
     }
 
     // arg phi at the V sites of this thread and at the site right of them, rows w and w+1 of a staged plane.  Every
@@ -196,8 +202,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         if (w == 0 && it + NS - 1 <= zlen && elect_one()) {
             const int s = (it + NS - 1) % NS;
             if (it > 0) mbar_wait(&empty[s], ((it - 1) / NS) & 1);
-            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES);
-            issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + NS - 1));
+            issue_plane(s, it + NS - 1);
         }
 
         const int z = z0 + it, y = y0 + w;
@@ -339,7 +344,7 @@ int pick_zlen(int N, int ctas_per_sm, int max_partials)
 
 template <typename T, int TY, int MINB>
 int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-               void* list, size_t list_bytes, cudaStream_t st)
+               void* list, size_t list_bytes, const CUtensorMap* tmap, cudaStream_t st)
 {
     using C = DiagCfg<T, TY>;
     auto kern = diag_march_kernel<T, TY, MINB>;
@@ -356,7 +361,11 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
     DiagPartial* extra = partials + blocks;
     unsigned long long* count = &partials[blocks + 1].n_pierced;
     if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count);
+    static const bool tma_off = getenv("AHS_NO_TMA") != nullptr;
+    CUtensorMap none;
+    memset(&none, 0, sizeof(none));
+    const bool use_tma = tmap && !tma_off;
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, use_tma ? *tmap : none, use_tma ? 1 : 0);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
@@ -368,16 +377,27 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
 
 template <typename T>
 int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-                      void* list, size_t list_bytes, cudaStream_t st)
+                      void* list, size_t list_bytes, const CUtensorMap* tmap, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
     // 4-row tiles (3 CTAs/SM) by default; AHS_DIAG_TY=8 selects 8-row tiles, two CTAs per SM (experiments)
     static const int ty = [] { const char* e = getenv("AHS_DIAG_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, list, list_bytes, st);
-    return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, list, list_bytes, st);
+    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, list, list_bytes, nullptr, st);
+    return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
 }
 
-template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, cudaStream_t);
-template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, cudaStream_t);
+// the tensor map of one (phi, theta) buffer for the default tile shape (4 rows): box (TX + V, TY + 1, 1, 5)
+template <typename T>
+bool make_diag_march_map(CUtensorMap* out, const void* phi_re_base, int N, size_t array_bytes)
+{
+    using G = typename DiagCfg<T, 4>::G;
+    if (!march_supported<T>(N)) return false;
+    return make_tile_map<T>(out, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 5);
+}
+template bool make_diag_march_map<float>(CUtensorMap*, const void*, int, size_t);
+template bool make_diag_march_map<double>(CUtensorMap*, const void*, int, size_t);
+
+template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const CUtensorMap*, cudaStream_t);
+template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const CUtensorMap*, cudaStream_t);
 
 }  // namespace ahs
