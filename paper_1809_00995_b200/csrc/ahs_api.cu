@@ -30,6 +30,8 @@ struct ahs_sim {
     int device;
     CUtensorMap diag_map[2];   // TMA descriptors of (phi, theta) buffer 0 / 1 for the diagnostics march
     bool diag_map_ok;
+    StepMaps step_maps[2];     // the same for the step march (buffer 0 / 1 as the level-n input)
+    bool step_maps_ok;
 };
 
 namespace {
@@ -131,7 +133,7 @@ int do_step(ahs_sim* s)
     }
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
     const StepCoef c = step_coefficients(s->p, s->step);
-    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->stream)
+    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->step_maps_ok ? &s->step_maps[s->cur] : nullptr, s->stream)
                                          : launch_step_generic<T>(f, s->p.N, c, s->stream);
 }
 
@@ -232,7 +234,13 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMallocHost: %s", cudaGetErrorString(ce)); ahs_destroy(s); return nullptr; }
 
     s->diag_map_ok = false;
+    s->step_maps_ok = false;
     if (s->kernel == AHS_KERNEL_MARCH) {
+        s->step_maps_ok = p.precision == AHS_F32
+            ? make_step_march_maps<float>(&s->step_maps[0], slot<float>(s, PHI_RE0), slot<float>(s, PI_RE), p.N, s->array_bytes) &&
+              make_step_march_maps<float>(&s->step_maps[1], slot<float>(s, PHI_RE1), slot<float>(s, PI_RE), p.N, s->array_bytes)
+            : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), slot<double>(s, PI_RE), p.N, s->array_bytes) &&
+              make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), slot<double>(s, PI_RE), p.N, s->array_bytes);
         s->diag_map_ok = p.precision == AHS_F32
             ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
               make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)

@@ -37,11 +37,11 @@ namespace {
 constexpr double kInv2Pi = 0.15915494309189535;
 constexpr float kTieMargin = 4e-6f;   // in units of a full turn, relative to 1 + |t|: ten times the error bound
 
-template <typename T, int TY_>
+template <typename T, int TY_, int NS_ = 4>
 struct DiagCfg {
     static constexpr int V = 16 / sizeof(T);
     static constexpr int TY = TY_;
-    static constexpr int NSTAGE = 4;
+    static constexpr int NSTAGE = NS_;
     using G = TileGeom<T, V, TY, 5, NSTAGE, 0, 0>;           // a stage: phi_re, phi_im, theta_0..2 of one plane, forward halo only
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
@@ -102,12 +102,12 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
     }
 }
 
-template <typename T, int TY, int MINB>
-__global__ void __launch_bounds__(DiagCfg<T, TY>::NTHREADS, MINB)
+template <typename T, int TY, int MINB, int NSTAGES>
+__global__ void __launch_bounds__(DiagCfg<T, TY, NSTAGES>::NTHREADS, MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
-                  unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap, int use_tma)
+                  unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap, int use_tma, int rotate)
 {
-    using C = DiagCfg<T, TY>;
+    using C = DiagCfg<T, TY, NSTAGES>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
     constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = C::STAGE_STRIDE;
@@ -199,7 +199,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         const T* sn = stages + ((it + 1) % NS) * SE;
 
         // plane it+3 -> the stage that held plane it-1, once all TY warps have released it
-        if (w == 0 && it + NS - 1 <= zlen && elect_one()) {
+        if (w == (rotate ? it % TY : 0) && it + NS - 1 <= zlen && elect_one()) {
             const int s = (it + NS - 1) % NS;
             if (it > 0) mbar_wait(&empty[s], ((it - 1) / NS) & 1);
             issue_plane(s, it + NS - 1);
@@ -342,12 +342,12 @@ int pick_zlen(int N, int ctas_per_sm, int max_partials)
     return N;
 }
 
-template <typename T, int TY, int MINB>
+template <typename T, int TY, int MINB, int NSTAGES = 4>
 int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
                void* list, size_t list_bytes, const CUtensorMap* tmap, cudaStream_t st)
 {
-    using C = DiagCfg<T, TY>;
-    auto kern = diag_march_kernel<T, TY, MINB>;
+    using C = DiagCfg<T, TY, NSTAGES>;
+    auto kern = diag_march_kernel<T, TY, MINB, NSTAGES>;
     static bool configured = false;
     if (!configured) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return AHS_ERR_CUDA;
@@ -362,10 +362,11 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
     unsigned long long* count = &partials[blocks + 1].n_pierced;
     if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
     static const bool tma_off = getenv("AHS_NO_TMA") != nullptr;
+    static const int rot = [] { const char* e = getenv("AHS_DIAG_ROT"); return e ? atoi(e) : 1; }();
     CUtensorMap none;
     memset(&none, 0, sizeof(none));
     const bool use_tma = tmap && !tma_off;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, use_tma ? *tmap : none, use_tma ? 1 : 0);
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, use_tma ? *tmap : none, use_tma ? 1 : 0, rot);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
@@ -383,6 +384,9 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartia
     // 4-row tiles (3 CTAs/SM) by default; AHS_DIAG_TY=8 selects 8-row tiles, two CTAs per SM (experiments)
     static const int ty = [] { const char* e = getenv("AHS_DIAG_TY"); return e ? atoi(e) : 4; }();
     if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, list, list_bytes, nullptr, st);
+    static const int ns = [] { const char* e = getenv("AHS_DIAG_NS"); return e ? atoi(e) : 4; }();
+    if (ns == 5) return launch_cfg<T, 4, 3, 5>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
+    if (ns == 3) return launch_cfg<T, 4, 3, 3>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
     return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
 }
 

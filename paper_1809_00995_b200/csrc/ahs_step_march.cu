@@ -36,6 +36,7 @@
 #include "ahs_internal.cuh"
 #include "ahs_math.cuh"
 #include "ahs_stage.cuh"
+#include "ahs_tma.cuh"
 #include "ahs_trig.cuh"
 
 namespace ahs {
@@ -55,11 +56,15 @@ struct MarchCfg {
     static constexpr int NTHREADS = TY * 32;
     static constexpr int YEX_ELEMS = 4 * TY * TX;         // b1.re, b1.im, S01, S12 of rows -1 .. TY-2 (one parity)
     static constexpr int XEX_ELEMS = 4 * TY;              // b0.re, b0.im, S01, S02 of the halo column (one parity)
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * G::ARR_ELEMS + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
+    static constexpr int T2_STRIDE = (int)(((G::ARR_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
+    static_assert(G::STAGE_BYTES % 128 == 0, "stages stay 128-byte aligned");
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * T2_STRIDE + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
 
 template <typename T, int TY, int MINB>
-__global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k)
+__global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB)
+step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
+                  const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_mom, int use_tma)
 {
     using C = MarchCfg<T, TY>;
     using G = typename C::G;
@@ -73,7 +78,7 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
     T* stages = reinterpret_cast<T*>(smem + 128);
     T* th2ring = stages + NS * SE;
-    T* yex = th2ring + C::T2_SLOTS * G::ARR_ELEMS;
+    T* yex = th2ring + C::T2_SLOTS * C::T2_STRIDE;
     T* xex = yex + 2 * C::YEX_ELEMS;
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -97,14 +102,33 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
 
     // plane index i of this CTA's march = lattice plane z0 - 1 + i (periodic)
     auto plane_of = [&](int i) { const int z = z0 - 1 + i; return z < 0 ? z + N : (z >= N ? z - N : z); };
+    // Tiles that do not touch the periodic boundary fetch a plane with two tensor copies (UTMALDG: the four-array stage
+    // and theta_2) instead of 30 row copies; the others keep the row copies (TMA zero-fills out of bounds, it does not wrap).
+    const bool tma_tile = (use_tma & 1) && x0 > 0 && x0 + TX < N && y0 > 0 && y0 + TY < N;
+    auto issue_stage = [&](int s, int p) {   // phi_re, phi_im, theta_0, theta_1 of march plane p -> stage s
+        if (tma_tile) tma_load_4d(stages + s * SE, &map_stage, x0 - V, y0 - 1, plane_of(p), 0, &full[s]);
+        else issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+    };
+    auto issue_th2 = [&](int slot, int bar, int p) {   // theta_2 of march plane p -> ring slot, completion on full[bar]
+        if (tma_tile) tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &full[bar]);
+        else issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &full[bar], src2, N, x0, y0, plane_of(p));
+    };
+    // the momenta of plane z (no halo) are asked into L2 one plane ahead of the streaming loads that consume them
+    auto prefetch_momenta = [&](int z) {
+        if (use_tma & 2)
+            asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_mom)),
+                         "r"(x0), "r"(y0), "r"(z), "r"(0)
+                         : "memory");
+    };
     if (w == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
             const bool t2 = i < C::T2_SLOTS;   // theta_2 of planes 0, 1 ride on the barriers of planes 0, 1
             if (elect_one()) {
                 mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + (t2 ? G::ARR_BYTES : 0u));
-                issue_rows<G, 4>(stages + i * SE, &full[i], src, N, x0, y0, plane_of(i));
-                if (t2) issue_rows<G, 1>(th2ring + i * G::ARR_ELEMS, &full[i], src2, N, x0, y0, plane_of(i));
+                issue_stage(i, i);
+                if (t2) issue_th2(i, i, i);
+                if (i == 0) prefetch_momenta(z0);
             }
         }
     }
@@ -143,7 +167,7 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
     for (int it = 1; it <= zlen; ++it) {
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
-        const T* t2c = th2ring + (it & 1) * G::ARR_ELEMS;
+        const T* t2c = th2ring + (it & 1) * C::T2_STRIDE;
         T* yexp = yex + (it & 1) * C::YEX_ELEMS;
         T* xexp = xex + (it & 1) * C::XEX_ELEMS;
 
@@ -151,9 +175,10 @@ __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB) step_march_ke
         if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
             const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES);
-            issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(it + 2));
-            issue_rows<G, 1>(th2ring + ((it + 1) & 1) * G::ARR_ELEMS, &full[s], src2, N, x0, y0, plane_of(it + 1));
+            issue_stage(s, it + 2);
+            issue_th2((it + 1) & 1, s, it + 1);
         }
+        if (((w + it) % TY) == ISSUER && it < zlen && elect_one()) prefetch_momenta(z0 + it);   // plane of iteration it+1
 
         const int z = z0 + it - 1;
         const size_t g = ((size_t)z * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
@@ -311,7 +336,7 @@ int pick_zlen(int N, int ctas_per_sm)
 }
 
 template <typename T, int TY, int MINB>
-int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st)
+int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, cudaStream_t st)
 {
     using C = MarchCfg<T, TY>;
     auto kern = step_march_kernel<T, TY, MINB>;
@@ -324,7 +349,15 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st)
     const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB);
     const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k);
+    // AHS_STEP_TMA (experiments): bit 0 = tensor copies for the stages, bit 1 = L2 prefetch of the momenta
+    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 3 : 3); }();
+    if (maps && tma_mode) {
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, tma_mode);
+    } else {
+        StepMaps none;
+        memset(&none, 0, sizeof(none));
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, none.stage, none.th2, none.mom, 0);
+    }
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
 
@@ -338,21 +371,35 @@ bool march_supported(int N)
 }
 
 template <typename T>
-int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st)
+int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
     // 4-row tiles, four CTAs (barrier domains) per SM, measured fastest (profiles/); AHS_MARCH_TY=8 (experiments
     // only) selects 8-row tiles, two CTAs per SM
     static const int ty = [] { const char* e = getenv("AHS_MARCH_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, st);
-    if (ty == 16 && N % 16 == 0) return launch_cfg<T, 16, 1>(f, N, c, st);
-    return launch_cfg<T, 4, 3>(f, N, c, st);
+    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, nullptr, st);
+    if (ty == 16 && N % 16 == 0) return launch_cfg<T, 16, 1>(f, N, c, nullptr, st);
+    return launch_cfg<T, 4, 3>(f, N, c, maps, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu
 template bool march_supported<float>(int);
 template bool march_supported<double>(int);
-template int launch_step_march<float>(const FieldPtrs<float>&, int, const StepCoef&, cudaStream_t);
-template int launch_step_march<double>(const FieldPtrs<double>&, int, const StepCoef&, cudaStream_t);
+template int launch_step_march<float>(const FieldPtrs<float>&, int, const StepCoef&, const StepMaps*, cudaStream_t);
+template int launch_step_march<double>(const FieldPtrs<double>&, int, const StepCoef&, const StepMaps*, cudaStream_t);
+
+// tensor maps of one (phi, theta) buffer and of the momenta for the default tile shape (4 rows)
+template <typename T>
+bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi_re_base, int N, size_t array_bytes)
+{
+    using C = MarchCfg<T, 4>;
+    using G = typename C::G;
+    if (!march_supported<T>(N)) return false;
+    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
+           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
+           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, C::TY, 5);
+}
+template bool make_step_march_maps<float>(StepMaps*, const void*, const void*, int, size_t);
+template bool make_step_march_maps<double>(StepMaps*, const void*, const void*, int, size_t);
 
 }  // namespace ahs
