@@ -107,6 +107,26 @@ static double aho_u53(uint32_t hi, uint32_t lo)
  * pinned by: Philox KAT; |phi| = sigma exactly-to-rounding; pierced fraction 1/3 (four i.i.d.
  * uniform corner phases); Gauss residual identically 0 at n = 0; sample moments of kind 1.
  * -------------------------------------------------------------------------------------------- */
+static void aho_ic_site(const aho_params* p, const uint32_t key[2], int64_t site, int32_t kind, double* re, double* im)
+{
+    uint32_t ctr[4] = { (uint32_t)((uint64_t)site & 0xffffffffu), (uint32_t)((uint64_t)site >> 32), 0u, 0u };
+    uint32_t r[4];
+    aho_philox4x32_10(ctr, key, r);
+    if (kind == 0) {
+        double th = AHO_TWO_PI * aho_u53(r[0], r[1]);
+        *re = p->sigma * cos(th);
+        *im = p->sigma * sin(th);
+    } else {
+        double u1 = aho_u53(r[0], r[1]) + 1.0 / 18014398509481984.0; /* + 2^-54 */
+        double u2 = aho_u53(r[2], r[3]);
+        double rho = sqrt(-2.0 * log(u1));
+        double amp = (p->sigma / sqrt(2.0)) * rho;
+        double th = AHO_TWO_PI * u2;
+        *re = amp * cos(th);
+        *im = amp * sin(th);
+    }
+}
+
 void aho_ic(const aho_params* p, uint64_t seed, int32_t kind, double* f10)
 {
     const int64_t N = p->N, V = N * N * N;
@@ -114,24 +134,26 @@ void aho_ic(const aho_params* p, uint64_t seed, int32_t kind, double* f10)
     double* phi_re = f10;
     double* phi_im = f10 + V;
     uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
-    for (int64_t site = 0; site < V; ++site) {
-        uint32_t ctr[4] = { (uint32_t)((uint64_t)site & 0xffffffffu), (uint32_t)((uint64_t)site >> 32), 0u, 0u };
-        uint32_t r[4];
-        aho_philox4x32_10(ctr, key, r);
-        if (kind == 0) {
-            double th = AHO_TWO_PI * aho_u53(r[0], r[1]);
-            phi_re[site] = p->sigma * cos(th);
-            phi_im[site] = p->sigma * sin(th);
-        } else {
-            double u1 = aho_u53(r[0], r[1]) + 1.0 / 18014398509481984.0; /* + 2^-54 */
-            double u2 = aho_u53(r[2], r[3]);
-            double rho = sqrt(-2.0 * log(u1));
-            double amp = (p->sigma / sqrt(2.0)) * rho;
-            double th = AHO_TWO_PI * u2;
-            phi_re[site] = amp * cos(th);
-            phi_im[site] = amp * sin(th);
-        }
-    }
+    for (int64_t site = 0; site < V; ++site) aho_ic_site(p, key, site, kind, &phi_re[site], &phi_im[site]);
+}
+
+/* The same initial condition on a WINDOW of a larger lattice: f10 is a B^3 container (B = p->N) that receives the values of
+ * the sites ((x0+i) mod Nfull, (y0+j) mod Nfull, (z0+k) mod Nfull) of the Nfull^3 lattice (site index of the FULL lattice
+ * keys Philox).  Used by the full-size sampled parity test: the window is then stepped as a small periodic lattice and only
+ * its interior, which the wrong wrap cannot have reached after n steps (one site per step), is compared.
+ * pinned by: equality with the corresponding sub-box of aho_ic on a lattice small enough to generate in full. */
+void aho_ic_window(const aho_params* p, uint64_t seed, int32_t kind, int64_t Nfull, int64_t x0, int64_t y0, int64_t z0, double* f10)
+{
+    const int64_t B = p->N, V = B * B * B;
+    memset(f10, 0, (size_t)(10 * V) * sizeof(double));
+    uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+    for (int64_t k = 0; k < B; ++k)
+        for (int64_t j = 0; j < B; ++j)
+            for (int64_t i = 0; i < B; ++i) {
+                const int64_t x = ((x0 + i) % Nfull + Nfull) % Nfull, y = ((y0 + j) % Nfull + Nfull) % Nfull, z = ((z0 + k) % Nfull + Nfull) % Nfull;
+                const int64_t site = x + Nfull * (y + Nfull * z), w = i + B * (j + B * k);
+                aho_ic_site(p, key, site, kind, &f10[w], &f10[V + w]);
+            }
 }
 
 /* ----------------------------------------------------------------------------------------------

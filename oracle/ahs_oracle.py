@@ -81,13 +81,14 @@ def lib():
         dp = C.POINTER(C.c_double)
         _lib.aho_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         _lib.aho_ic.argtypes = [C.POINTER(_Params), C.c_uint64, C.c_int32, dp]
+        _lib.aho_ic_window.argtypes = [C.POINTER(_Params), C.c_uint64, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int64, dp]
         _lib.aho_coeffs.argtypes = [C.POINTER(_Params), C.c_int64, dp]
         _lib.aho_step.argtypes = [C.POINTER(_Params), dp, C.c_int64, C.c_int32]
         _lib.aho_winding.argtypes = [C.POINTER(_Params), dp, C.POINTER(C.c_int32),
                                      C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         _lib.aho_diag_compute.argtypes = [C.POINTER(_Params), dp, C.c_int64, C.POINTER(_Diag)]
         _lib.aho_site_fields.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp]
-        for f in ("aho_philox4x32_10", "aho_ic", "aho_coeffs", "aho_step", "aho_winding",
+        for f in ("aho_philox4x32_10", "aho_ic", "aho_ic_window", "aho_coeffs", "aho_step", "aho_winding",
                   "aho_diag_compute", "aho_site_fields"):
             getattr(_lib, f).restype = None
         assert _lib.aho_sizeof_params() == C.sizeof(_Params)
@@ -115,6 +116,14 @@ def philox4x32_10(ctr, key):
 def initial_condition(p: Params, seed: int, kind: int = IC_RANDOM_PHASE) -> np.ndarray:
     f10 = np.empty((10, p.N, p.N, p.N), dtype=np.float64)
     lib().aho_ic(C.byref(p._c()), C.c_uint64(seed), kind, _dptr(f10))
+    return f10
+
+
+def initial_condition_window(p: Params, seed: int, n_full: int, origin, kind: int = IC_RANDOM_PHASE) -> np.ndarray:
+    """IC of the p.N^3 window at `origin` = (x0, y0, z0) (periodic) of an n_full^3 lattice, as a p.N^3 container."""
+    f10 = np.empty((10, p.N, p.N, p.N), dtype=np.float64)
+    x0, y0, z0 = (int(v) for v in origin)
+    lib().aho_ic_window(C.byref(p._c()), C.c_uint64(seed), kind, n_full, x0, y0, z0, _dptr(f10))
     return f10
 
 

@@ -26,6 +26,24 @@ __device__ __forceinline__ void mbar_fence_init()
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
+// Order this thread's earlier generic-proxy accesses to shared memory (and those it has synchronised with) before its
+// later async-proxy operations: to be executed by the copy-issuing thread before it re-fills a stage that was read
+// with ordinary loads.
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// A shared-memory load the warp really waits for.  BAR.SYNC on sm_100 is DEFER_BLOCKING: the warp runs on until its next
+// instruction that touches barrier-protected state, and a bulk / tensor copy (uniform datapath, async proxy) is not
+// such an instruction -- issued right after __syncthreads() it overwrote a stage other warps were still reading
+// (seen as one corrupted site per ~500 launches at a z-chunk start, profiles/r2_race.md).  Call this between the
+// barrier and the copy.
+__device__ __forceinline__ void wait_barrier_resolved(const uint64_t* any_smem_word)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(any_smem_word)) : "memory");
+    asm volatile("" ::"r"(v) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");

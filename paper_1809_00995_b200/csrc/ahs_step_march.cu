@@ -160,8 +160,17 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         }
     }
     __syncthreads();
+    wait_barrier_resolved(full);   // the first in-loop copy re-fills the stage the prologue has just read
 
     const T dtc2 = k.dt * k.c2, dtd3 = k.dt * k.d3;
+
+    // The momenta (no halo) are streamed with 16-byte loads, software-pipelined by one plane: those of plane it+1 are
+    // requested right after the barrier of plane it, where register pressure is lowest, and consumed at the end of phase 1
+    // of plane it+1 (profiles/r1: requested at the top of their own plane they cost 15 % of the issue slots in stalls).
+    const size_t plane_stride = (size_t)N * N;
+    size_t gnext = ((size_t)z0 * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+    VecT nPr = ldg_vec<T, V>(f.pi_re + gnext), nPi = ldg_vec<T, V>(f.pi_im + gnext);
+    VecT nE0 = ldg_vec<T, V>(f.eps[0] + gnext), nE1 = ldg_vec<T, V>(f.eps[1] + gnext), nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
 
     // ---- the march -----------------------------------------------------------------------------------------------------
     for (int it = 1; it <= zlen; ++it) {
@@ -174,16 +183,21 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
         if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
             const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
+            wait_barrier_resolved(full);
+            fence_proxy_async();
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES);
             issue_stage(s, it + 2);
             issue_th2((it + 1) & 1, s, it + 1);
         }
         if (((w + it) % TY) == ISSUER && it < zlen && elect_one()) prefetch_momenta(z0 + it);   // plane of iteration it+1
 
-        const int z = z0 + it - 1;
-        const size_t g = ((size_t)z * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+        const size_t g = gnext;                                         // plane z0 + it - 1
+#ifdef AHS_NO_PIPELINE
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
         const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
+#else
+        const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested right after the previous plane's barrier
+#endif
 
         mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
 
@@ -292,6 +306,16 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             xexp[3 * TY + r] = sin_fast(t0 + t2x - t0z - t2);
         }
         __syncthreads();
+        gnext = g + plane_stride;
+#ifndef AHS_NO_PIPELINE
+        if (it < zlen)
+#else
+        if (false)
+#endif
+        {
+            nPr = ldg_vec<T, V>(f.pi_re + gnext); nPi = ldg_vec<T, V>(f.pi_im + gnext);
+            nE0 = ldg_vec<T, V>(f.eps[0] + gnext); nE1 = ldg_vec<T, V>(f.eps[1] + gnext); nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
+        }
         {
             // ---- phase 2: the terms that crossed a warp or tile boundary, then the stores ----------------------------
             const VecT yb1r = lds_vec<T, V>(yexp + (0 * TY + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * TY + w) * TX + xi);

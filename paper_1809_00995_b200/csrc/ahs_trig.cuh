@@ -5,7 +5,7 @@
 // Payne-Hanek slow path whose branch (BSSY/BSYNC) stalls instruction fetch and bloats the loop past the
 // instruction cache (profiles/r1_step512_march_v1.md).  Why not the __sinf/__cosf intrinsics: their absolute
 // error (2^-21) is what PAPER.md L142 reports as degrading the diagnostics.  So: Cody-Waite reduction with a
-// three-term split of pi/2 (or pi) carried by FMAs, then minimax-style polynomials on the reduced interval.
+// two-term (fp32) / three-term (fp64) split of pi/2 (or pi) carried by FMAs, then minimax-style polynomials on the reduced interval.
 //
 //   sincos_fast(x): k = rint(x * 2/pi), r = x - k*pi/2 in [-pi/4, pi/4]; sin and cos polynomials; quadrant fix-up.
 //   sin_fast(x)   : fp32: k = rint(x / pi), r in [-pi/2, pi/2], odd polynomial, sign (-1)^k;
@@ -28,8 +28,7 @@ __device__ __forceinline__ void sincos_fast(float x, float& s, float& c)
     const int q = __float_as_int(t);
     const float k = t - 12582912.0f;
     float r = fmaf(k, -1.5707963705062866f, x);
-    r = fmaf(k, 4.371138828673793e-08f, r);
-    r = fmaf(k, 1.7151245100058819e-15f, r);
+    r = fmaf(k, 4.371138828673793e-08f, r);   // (a third term, 1.7e-15 k, is below fp32 resolution over the whole domain)
     const float z = r * r;
     float ps = fmaf(z, -0.00019513866573106498f, 0.00833214819431305f);
     ps = fmaf(z, ps, -0.16666653752326965f);
@@ -51,7 +50,6 @@ __device__ __forceinline__ float sin_fast(float x)
     const float k = t - 12582912.0f;
     float r = fmaf(k, -3.1415927410125732f, x);
     r = fmaf(k, 8.742277657347586e-08f, r);
-    r = fmaf(k, 3.4302490200117637e-15f, r);
     const float z = r * r;
     float p = fmaf(z, -2.388586395341008e-08f, 2.752518867055187e-06f);
     p = fmaf(z, p, -0.00019840864115394652f);

@@ -54,14 +54,13 @@ def header_constants(name: str):
 
 # ---- emulations of the device routines (same operation order as ahs_trig.cuh) -------------------------------------------
 def emu_sincos(x, k):
-    two_over_pi, magic, c1, c2, c3, s3, s2, s1, q3, q2, q1, q0 = k[0], k[1], k[3], k[4], k[5], k[6], k[7], k[8], k[9], k[10], k[11], k[12]
+    two_over_pi, magic, c1, c2, s3, s2, s1, q3, q2, q1, q0 = k[0], k[1], k[3], k[4], k[5], k[6], k[7], k[8], k[9], k[10], k[11]
     x = x.astype(f32)
     t = fma(x, f32(two_over_pi), f32(magic))
     q = t.view(np.int32)
     kk = (t - f32(magic)).astype(f32)
     r = fma(kk, f32(c1), x)
     r = fma(kk, f32(c2), r)
-    r = fma(kk, f32(c3), r)
     z = (r * r).astype(f32)
     ps = fma(z, f32(s3), f32(s2))
     ps = fma(z, ps, f32(s1))

@@ -340,3 +340,81 @@ def test_winding_bit_exact_when_links_sit_next_to_ties(ahs, oracle, prec, N):
         r = oracle.diagnostics(p, f, 0)
         assert r["n_pierced"] > N ** 3 // 10
         assert (d["n_pierced"], d["sum_abs_w"]) == (r["n_pierced"], r["sum_abs_w"]), kernel
+
+
+# ---------------------------------------------------------------------------------------------------------
+# full size (BASELINE.json configs[3]: 1024^3 fp32, the launch configuration bench.py times), sampled outputs
+# ---------------------------------------------------------------------------------------------------------
+class _DeviceArray:
+    """Zero-copy view of a live field (ahs_field_device_ptr) for torch.as_tensor."""
+
+    def __init__(self, ptr, N, typestr):
+        self.__cuda_array_interface__ = {"shape": (N, N, N), "typestr": typestr, "data": (ptr, False), "version": 2}
+
+
+def _gather_window(sim, origin, B):
+    import torch
+    N = sim.N
+    typestr = "<f4" if sim.dtype == np.float32 else "<f8"
+    ix = [torch.as_tensor((np.arange(o, o + B) % N), device="cuda") for o in origin]
+    out = np.empty((10, B, B, B))
+    for k in range(10):
+        t = torch.as_tensor(_DeviceArray(sim.field_device_ptr(k), N, typestr), device="cuda")
+        out[k] = t[ix[2][:, None, None], ix[1][None, :, None], ix[0][None, None, :]].double().cpu().numpy()
+    return out
+
+
+def test_full_size_1024_sampled_windows_and_closed_forms(ahs, oracle):
+    """configs[3] at full size.  (1) Sampled outputs: the oracle generates the initial condition of small windows of the
+    1024^3 lattice from the Philox specification (aho_ic_window), steps each window as a periodic 22^3 lattice and is
+    compared on the 16^3 interior the wrong wrap cannot have reached after 3 steps -- windows sit on tile corners, on
+    z-chunk boundaries of the march and on the periodic corner of the lattice.  (2) Properties that hold at any size:
+    closed forms of the diagnostics on the random-phase initial condition, Gauss's law at fp32 roundoff after stepping."""
+    import torch
+    N, nsteps, halo, inner = 1024, 3, 3, 16
+    free, _ = torch.cuda.mem_get_info()
+    if free < ahs.required_bytes(N, "f32") + (2 << 30):
+        pytest.skip("needs %.0f GB of free device memory" % (ahs.required_bytes(N, "f32") / 1e9))
+    seed, B = 180900995, inner + 2 * halo
+    with ahs.Simulation(N=N, precision="f32", m=1.0, s=0.0, seed=seed) as sim:
+        assert sim.kernel_kind == "march"
+        d0 = sim.diagnostics()
+        sites = float(N) ** 3
+        # i.i.d. uniform phases: a plaquette is pierced with probability 1/3; with theta = Pi = eps = 0 and |phi| = sigma,
+        # Lag = -G, G = (1/dx^2) sum_i 2 (1 - cos D_i) with D_i i.i.d. uniform: E G = 24, E G^2 = 672 at dx = 0.5
+        assert abs(d0["n_pierced"] / (3 * sites) - 1 / 3) < 1e-4
+        assert d0["v2_num"] == 0.0 and d0["gauss_max"] == 0.0 and d0["nonfinite"] == 0
+        assert d0["mean_lagrangian"] == pytest.approx(-24.0, rel=1e-3)
+        assert d0["v2_den"] / sites == pytest.approx(-672.0, rel=2e-3)
+        sim.step(nsteps)
+        rng = np.random.default_rng(5)
+        origins = [(-11, -11, -11), (128 - 11, 4 - 11, 64 - 11), (512 - 5, 700 - 2, 128 - 9), (1024 - 128 - 8, 1024 - 4 - 9, 960 - 3)]
+        origins += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(4)]
+        pw = oracle.Params(N=B, m=1.0, s=0.0)
+        sl = slice(halo, halo + inner)
+        for origin in origins:
+            ref = rounded(oracle.initial_condition_window(pw, seed, N, origin), "f32")
+            oracle.step(pw, ref, 0, nsteps)
+            got = _gather_window(sim, origin, B)
+            for k in range(10):
+                err = np.abs(got[k][sl, sl, sl] - ref[k][sl, sl, sl]).max() / max(1.0, np.abs(ref[k][sl, sl, sl]).max())
+                assert err <= TOL["f32"], (origin, oracle.FIELD_NAMES[k], err)
+        d = sim.diagnostics()
+        assert d["nonfinite"] == 0 and d["step"] == nsteps
+        assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"])
+
+
+def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
+    """Regression for a shared-memory race of the marching step kernel (profiles/r2_race.md): a tensor / bulk copy
+    issued right after __syncthreads() could overwrite a stage other warps were still reading -- about one corrupted
+    site per 500 launches at 512^3, visible as a Gauss-law violation of 1e-2 and as run-to-run differences.  Two runs of
+    60 back-to-back launches must agree bit for bit and keep Gauss's law at fp32 roundoff."""
+    import hashlib
+    out = []
+    for _ in range(2):
+        with ahs.Simulation(N=512, precision="f32", m=1.0, s=0.0, seed=180900995) as sim:
+            sim.step(60)
+            d = sim.diagnostics()
+            out.append((hashlib.md5(sim.get_fields_native().tobytes()).hexdigest(), d["n_pierced"], d["v2_num"], d["gauss_max"]))
+            assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"]), d
+    assert out[0] == out[1]

@@ -725,3 +725,16 @@ def test_config1_literal_reading_leaves_stability_region(oracle):
     f = oracle.initial_condition(p0, seed=1)
     oracle.step(p0, f, 0, 200)
     assert np.isfinite(f).all() and np.abs(f[0:2]).max() < 3
+
+
+def test_ic_window_is_the_sub_box_of_the_full_lattice(oracle):
+    """aho_ic_window (used by the full-size sampled GPU parity test) against aho_ic on a lattice small enough to
+    generate in full, for windows that cross the periodic boundary in every direction and for both IC kinds."""
+    N, B = 24, 10
+    for kind in (oracle.IC_RANDOM_PHASE, oracle.IC_GAUSSIAN):
+        full = oracle.initial_condition(oracle.Params(N=N, sigma=1.3), 42, kind)
+        for origin in ((0, 0, 0), (20, 3, 17), (-4, 22, -1)):
+            win = oracle.initial_condition_window(oracle.Params(N=B, sigma=1.3), 42, N, origin, kind)
+            idx = [np.arange(o, o + B) % N for o in origin]
+            ref = full[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]]
+            assert np.array_equal(win, ref)
