@@ -186,6 +186,26 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+# ------------------------------------------------------------------------------------------------------------------
+# multi-rank host logic ("replicas only"): no data-path collective; torch.distributed carries the barrier
+# and the max over ranks of the device-timed window.  Backend-agnostic so that tests/test_bench_host.py can run it with
+# gloo, world_size 2, on CPU.
+# ------------------------------------------------------------------------------------------------------------------
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, sites: int, leapfrog: int, steps: int, total_ms: float) -> float:
+    """site-updates/s of the whole job: every rank advanced its own replica by leapfrog*steps steps in total_ms (max over ranks)."""
+    return world * sites * leapfrog * steps / (total_ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -203,12 +223,8 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    def max_ranks(x: float) -> float:
+        return max_over_ranks(x, world, "cuda")
 
     N, L, K, W = args.lattice, args.leapfrog, args.steps, args.warmup
     sites = N ** 3
@@ -238,10 +254,10 @@ def run_ours(args):
     t1 = time.time()
     clk = clocks.stop(t0, t1)
     launches = sim.kernel_launches - launches0
-    total_ms = max_over_ranks(start.elapsed_time(stop))
+    total_ms = max_ranks(start.elapsed_time(stop))
     step_ms = sum(a.elapsed_time(b) for a, b, _ in marks)       # the leapfrog launches only
     diag_ms = sum(b.elapsed_time(c) for _, b, c in marks)
-    value = world * sites * L * K / (total_ms * 1e-3)
+    value = whole_job_value(world, sites, L, K, total_ms)
 
     launch_s = step_ms * 1e-3 / (K * L)
     peak, peak_src = measured_peak()
@@ -257,7 +273,7 @@ def run_ours(args):
 
     e2e = None
     if not args.no_e2e:
-        e2e = run_e2e(args, sim, torch, max_over_ranks, barrier, world)
+        e2e = run_e2e(args, sim, torch, max_ranks, barrier, world)
 
     line = {
         "metric": "lattice site-updates/sec per leapfrog step", "value": value, "unit": "site-updates/s", "n_gpus": world,

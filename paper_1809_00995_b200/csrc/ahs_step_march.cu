@@ -76,6 +76,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
+    uint64_t* xch = full + NS;   // exchange barrier: one phase per plane, every thread arrives
     T* stages = reinterpret_cast<T*>(smem + 128);
     T* th2ring = stages + NS * SE;
     T* yex = th2ring + C::T2_SLOTS * C::T2_STRIDE;
@@ -96,6 +97,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        mbar_init(xch, C::NTHREADS);
         mbar_fence_init();
     }
     __syncthreads();
@@ -183,8 +185,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
         if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
             const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
-            wait_barrier_resolved(full);
-            fence_proxy_async();
+            fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1: all reads of that stage are done)
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES);
             issue_stage(s, it + 2);
             issue_th2((it + 1) & 1, s, it + 1);
@@ -200,6 +201,38 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
 #endif
 
         mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
+
+        // ---- halo products, shared out over the warps (no dedicated producer warp).  Row y0-1: one site per lane, every
+        //      HSTRIDE-th warp in rotation; column x0-1: one warp per plane.  Called before the exchange barrier is signalled.
+        auto halo_jobs = [&]() {
+            if (((w + it) % HSTRIDE) == 0) {
+                const int x = 32 * (w / HSTRIDE) + lane;   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
+                const T pr = sc[G::idx(0, -1, x)], pi = sc[G::idx(1, -1, x)];
+                const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = t2c[G::idx(0, -1, x)];
+                const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = t2c[G::idx(0, 0, x)], t1z = sn[G::idx(3, -1, x)];
+                T s, c;
+                sincos_fast(t1, s, c);
+                const Cx<T> b = mulUc<T>(c, s, { pr, pi });
+                yexp[(0 * TY + 0) * TX + x] = b.re;
+                yexp[(1 * TY + 0) * TX + x] = b.im;
+                yexp[(2 * TY + 0) * TX + x] = sin_fast(t0 + t1x - t0y - t1);
+                yexp[(3 * TY + 0) * TX + x] = sin_fast(t1 + t2y - t1z - t2);
+            }
+            if (((w + it) % TY) == COLUMN && lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02
+                const int r = lane;
+                const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
+                const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = t2c[G::idx(0, r, -1)];
+                const T t1x = sc[G::idx(3, r, 0)], t2x = t2c[G::idx(0, r, 0)];
+                const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
+                T s, c;
+                sincos_fast(t0, s, c);
+                const Cx<T> b = mulUc<T>(c, s, { pr, pi });
+                xexp[0 * TY + r] = b.re;
+                xexp[1 * TY + r] = b.im;
+                xexp[2 * TY + r] = sin_fast(t0 + t1x - t0y - t1);
+                xexp[3 * TY + r] = sin_fast(t0 + t2x - t0z - t2);
+            }
+        };
 
         // partial results that cross the barrier (phase 1 -> phase 2)
         T qr[V], qi[V], fr[V], fi[V], e0[V], e1[V], e2[V], g0[V], g1[V], g2[V];
@@ -250,6 +283,11 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             sts_vec<T, V>(yexp + (2 * TY + w + 1) * TX + xi, yS01);
             sts_vec<T, V>(yexp + (3 * TY + w + 1) * TX + xi, yS12);
             }
+            halo_jobs();
+            // Everything other warps need from this one is in shared memory and this warp has finished reading the staged
+            // planes: signal the exchange barrier now and fold the owned terms (no shared memory involved) while the other
+            // warps catch up; the wait comes just before phase 2.
+            mbar_arrive(xch);
             // -x products of the lane to the left (lane 0 gets its halo-column values in phase 2)
             T lb0r = __shfl_up_sync(0xffffffffu, b0r[V - 1], 1), lb0i = __shfl_up_sync(0xffffffffu, b0i[V - 1], 1);
             T lS01 = __shfl_up_sync(0xffffffffu, S01[V - 1], 1), lS02 = __shfl_up_sync(0xffffffffu, S02[V - 1], 1);
@@ -276,36 +314,6 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
                 cb2r[v] = b2r[v]; cb2i[v] = b2i[v]; cS02[v] = S02[v]; cS12[v] = S12[v];
             }
         }
-        // ---- halo products, shared out over the warps (no dedicated producer warp: 8 warps x 2 CTAs fill the register
-        //      file evenly).  Row y0-1: one site per lane, HSTRIDE-th warps in rotation; column x0-1: one warp per plane.
-        if (((w + it) % HSTRIDE) == 0) {
-            const int x = 32 * (w / HSTRIDE) + lane;   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
-            const T pr = sc[G::idx(0, -1, x)], pi = sc[G::idx(1, -1, x)];
-            const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = t2c[G::idx(0, -1, x)];
-            const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = t2c[G::idx(0, 0, x)], t1z = sn[G::idx(3, -1, x)];
-            T s, c;
-            sincos_fast(t1, s, c);
-            const Cx<T> b = mulUc<T>(c, s, { pr, pi });
-            yexp[(0 * TY + 0) * TX + x] = b.re;
-            yexp[(1 * TY + 0) * TX + x] = b.im;
-            yexp[(2 * TY + 0) * TX + x] = sin_fast(t0 + t1x - t0y - t1);
-            yexp[(3 * TY + 0) * TX + x] = sin_fast(t1 + t2y - t1z - t2);
-        }
-        if (((w + it) % TY) == COLUMN && lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02
-            const int r = lane;
-            const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
-            const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = t2c[G::idx(0, r, -1)];
-            const T t1x = sc[G::idx(3, r, 0)], t2x = t2c[G::idx(0, r, 0)];
-            const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
-            T s, c;
-            sincos_fast(t0, s, c);
-            const Cx<T> b = mulUc<T>(c, s, { pr, pi });
-            xexp[0 * TY + r] = b.re;
-            xexp[1 * TY + r] = b.im;
-            xexp[2 * TY + r] = sin_fast(t0 + t1x - t0y - t1);
-            xexp[3 * TY + r] = sin_fast(t0 + t2x - t0z - t2);
-        }
-        __syncthreads();
         gnext = g + plane_stride;
 #ifndef AHS_NO_PIPELINE
         if (it < zlen)
@@ -316,6 +324,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             nPr = ldg_vec<T, V>(f.pi_re + gnext); nPi = ldg_vec<T, V>(f.pi_im + gnext);
             nE0 = ldg_vec<T, V>(f.eps[0] + gnext); nE1 = ldg_vec<T, V>(f.eps[1] + gnext); nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
         }
+        mbar_wait(xch, (it - 1) & 1);   // all 128 threads have signalled plane `it`: exchange rows complete, stages no longer read
         {
             // ---- phase 2: the terms that crossed a warp or tile boundary, then the stores ----------------------------
             const VecT yb1r = lds_vec<T, V>(yexp + (0 * TY + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * TY + w) * TX + xi);
