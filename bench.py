@@ -39,7 +39,11 @@ FALLBACK_HBM_GBS = 6650.0                         # B200_PROFILING.md fallback i
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed `ncu --set full`
 # capture (profiles/); keyed by (kernel, precision, lattice).  None = no capture for that configuration.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r2_step1024_f32_full.md: 49.53 GB read + 42.90 GB written (capture taken with the momenta L2 prefetch still on;
+    # without it the r1 capture of the same stages read 47.08 GB)
+    ("march", "f32", 1024): 92.44e9,
+}
 
 
 def parse_args():
@@ -53,6 +57,8 @@ def parse_args():
     ap.add_argument("--leapfrog", type=int, default=50, help="leapfrog launches per bench step (config 4: diagnostics every 50)")
     ap.add_argument("--m", type=float, default=1.0)
     ap.add_argument("--s", type=float, default=0.0)
+    ap.add_argument("--tau-ref", type=float, default=0.0, help="a = (tau/tau_ref)^m; 0 = tau0 (DESIGN.md R3: s != 0 runs leave the "
+                    "stability region after ~80 steps at m=1 unless tau_ref is the end time)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "march"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="timed end-to-end steps (each uploads the full state)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -122,7 +128,7 @@ def oracle_sample(args, steps: int = 1, warmup: int = 0) -> dict:
     import numpy as np
     from oracle import ahs_oracle as O
     N, L = args.cpu_lattice, args.cpu_leapfrog
-    p = O.Params(N=N, m=args.m, s=args.s, **COMMON)
+    p = O.Params(N=N, m=args.m, s=args.s, tau_ref=args.tau_ref, **COMMON)
     f = O.initial_condition(p, SEED)
     if args.precision == "f32":
         f = np.ascontiguousarray(f.astype(np.float32).astype(np.float64))
@@ -168,8 +174,8 @@ def workload_config(args) -> dict:
     N = args.lattice
     name = {1024: "BASELINE.json configs[3]", 256: "BASELINE.json configs[1]", 512: "BASELINE.json configs[2]/[4]"}.get(N, "custom")
     return {"workload": "%d^3 periodic lattice, %s, dx=0.5 dt=0.1 lambda=2 e=1 sigma=1 tau0=1, a~tau^%g, s=%g, random-phase IC "
-                        "(Philox seed %d); %d leapfrog steps + 1 diagnostics per bench step (%s)"
-                        % (N, args.precision, args.m, args.s, SEED, args.leapfrog, name),
+                        "(Philox seed %d); %d leapfrog steps + 1 diagnostics per bench step (%s)%s"
+                        % (N, args.precision, args.m, args.s, SEED, args.leapfrog, name, ", tau_ref=%g" % args.tau_ref if args.tau_ref else ""),
             "lattice": N, "leapfrog_per_step": args.leapfrog, "diagnostics_per_step": 1,
             "l2": "inputs larger than L2 (%.1f GB of fields streamed per leapfrog launch)" % (N ** 3 * BYTES_PER_SITE[args.precision] / 1e9),
             "parallelism": "replicas x%d" % args.gpus}
@@ -228,7 +234,7 @@ def run_ours(args):
 
     N, L, K, W = args.lattice, args.leapfrog, args.steps, args.warmup
     sites = N ** 3
-    sim = ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank, kernel=args.kernel, **COMMON)
+    sim = ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank, kernel=args.kernel, tau_ref=args.tau_ref, **COMMON)
     diag = None
     for _ in range(W):
         sim.step(L)

@@ -382,8 +382,9 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* 
     const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB);
     const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
-    // AHS_STEP_TMA (experiments): bit 0 = tensor copies for the stages, bit 1 = L2 prefetch of the momenta
-    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 3 : 3); }();
+    // AHS_STEP_TMA (experiments): bit 0 = tensor copies for the stages (default), bit 1 = L2 prefetch of the momenta one
+    // plane ahead (off: with the software-pipelined loads it only adds 5 % of DRAM reads, profiles/r2_step1024_f32_full.md)
+    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 3 : 1); }();
     if (maps && tma_mode) {
         kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, tma_mode);
     } else {
