@@ -59,6 +59,10 @@ typedef struct {
     double gauss_rhs_rms;     /* rms_x of 2 q dx^2 e0^2 a_h^(2s) Im[conj(phi) Pi]               */
     int32_t nonfinite;        /* 1 if any of the 10 N^3 field values is not finite              */
     int32_t pad_;
+    double v2v_num;           /* sum_x |Pi|^2 * Vp    (Eq. 10 with the potential weight, L86)   */
+    double v2v_den;           /* sum_x |D phi|^2 * Vp                                           */
+    double v2_V;              /* 2R/(1+R), R = v2v_num / v2v_den (Eq. 9)                        */
+    double xi_L;              /* sqrt(-mu / mean Lag), mu = 2 pi sigma^2 (Eq. 9; R20); NaN if mean Lag >= 0 */
 } aho_diag;
 
 static const double AHO_TWO_PI  = 6.283185307179586476925286766559;
@@ -364,10 +368,11 @@ void aho_winding(const aho_params* p, const double* f10, int32_t* W3, uint64_t* 
  *   K^x   = |Pi^x|^2
  *   Vp^x  = (a^2 lambda(a)/4) (|phi^x|^2 - sigma^2)^2
  *   Lag^x = [ sum_i eps_i^2 - (c_B/dx^2) sum_i sum_{j!=i} (1 - cos Xi_ij^x) ] / (2 e(a)^2 a^2 dx^2) + K - G - Vp
- * out3 = {K, G, Lag}.  Optional per-site output arrays for the tests.
+ * out4 = {K, G, Lag, Vp}.  Vp is also the weight of the potential-weighted estimator <v^2>_V (L86);
+ * a constant factor on a weight drops out of R, so its a^2 lambda(a)/4 prefactor is immaterial there.
  * -------------------------------------------------------------------------------------------- */
 static void aho_site_lagrangian(const aho_params* p, const double* f10, double a,
-                                int64_t x, int64_t y, int64_t z, double out3[3])
+                                int64_t x, int64_t y, int64_t z, double out4[4])
 {
     const int64_t N = p->N, V = N * N * N;
     const double q = (double)p->q;
@@ -400,13 +405,16 @@ static void aho_site_lagrangian(const aho_params* p, const double* f10, double a
         }
     }
     const double gauge = (e2 - p->c_B * idx2 * mag) / (2.0 * ea * ea * a * a * p->dx * p->dx);
-    out3[0] = K; out3[1] = G; out3[2] = gauge + K - G - Vp;
+    out4[0] = K; out4[1] = G; out4[2] = gauge + K - G - Vp; out4[3] = Vp;
 }
 
 /* ----------------------------------------------------------------------------------------------
  * Diagnostics on the snapshot after n steps.
  *   winding                       : aho_winding above; L = (pi/6) dx n_pierced, xi = sqrt((N dx)^3/L) (L88-93)
  *   <v^2>_L = 2R/(1+R), R = sum K*Lag / sum G*Lag                                  (Eqs. 9-10)
+ *   <v^2>_V : the same with the potential Vp as the weight (L86: "two different weight functions")
+ *   xi_L = sqrt(-mu / mean Lag) (Eq. 9); the paper does not give mu: mu = 2 pi sigma^2, the Bogomolnyi
+ *          string tension at lambda = 2 e^2 (the paper's couplings, L72) -- a labelled assumption (R20)
  *   Gauss residual (L72, L181; derived from Eqs. 4-7, R4), a_h = a(tau_n - dt/2):
  *     g^x = sum_i (eps_i^x - eps_i^{x-k_i}) - 2 q dx^2 e0^2 a_h^(2s) Im[conj(phi^x) Pi^x]
  * Sums are accumulated in fp64 in plain x-fastest order.
@@ -437,16 +445,18 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
     const double a = aho_a(p, tau);
     const double ah = aho_a(p, tau - 0.5 * p->dt);
     const double grhs = 2.0 * q * p->dx * p->dx * p->e0 * p->e0 * pow(ah, 2.0 * p->s);
-    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0;
+    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
         const int64_t s0 = x + N * (y + N * z);
-        double kgl[3];
+        double kgl[4];
         aho_site_lagrangian(p, f10, a, x, y, z, kgl);
         num  += kgl[0] * kgl[2];
         den  += kgl[1] * kgl[2];
         lsum += kgl[2];
+        vnum += kgl[0] * kgl[3];
+        vden += kgl[1] * kgl[3];
         double div = 0.0;
         for (int i = 0; i < 3; ++i) div += eps[i][s0] - eps[i][aho_nb(N, x, y, z, i, -1)];
         const double rhs = grhs * (phr[s0] * pii[s0] - phi_[s0] * pir[s0]);
@@ -461,23 +471,35 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
         out->v2 = 2.0 * R / (1.0 + R);
     }
     out->mean_lagrangian = lsum / (double)V;
+    out->v2v_num = vnum;
+    out->v2v_den = vden;
+    {
+        const double R = vnum / vden;
+        out->v2_V = 2.0 * R / (1.0 + R);
+    }
+    out->xi_L = sqrt(-(AHO_TWO_PI * p->sigma * p->sigma) / out->mean_lagrangian);
     out->gauss_max = gmax;
     out->gauss_rhs_rms = sqrt(rhs2 / (double)V);
 }
 
-/* per-site arrays K, G, Lag (each N^3) for tests that re-evaluate Eq. 2 independently */
-void aho_site_fields(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag)
+/* per-site arrays K, G, Lag and (if not NULL) Vp (each N^3) for tests that re-evaluate Eq. 2 independently */
+void aho_site_fields4(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag, double* Vp)
 {
     const int64_t N = p->N;
     const double a = aho_a(p, aho_tau(p, n));
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
-        double kgl[3];
+        double kgl[4];
         aho_site_lagrangian(p, f10, a, x, y, z, kgl);
         const int64_t s0 = x + N * (y + N * z);
         K[s0] = kgl[0]; G[s0] = kgl[1]; Lag[s0] = kgl[2];
+        if (Vp) Vp[s0] = kgl[3];
     }
+}
+void aho_site_fields(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag)
+{
+    aho_site_fields4(p, f10, n, K, G, Lag, NULL);
 }
 
 /* struct sizes, so the ctypes mirror in ahs_oracle.py can assert it matches */

@@ -46,7 +46,8 @@ class _Diag(C.Structure):
     _fields_ = [("n_pierced", C.c_uint64), ("sum_abs_w", C.c_uint64), ("L", C.c_double), ("xi", C.c_double),
                 ("v2_num", C.c_double), ("v2_den", C.c_double), ("v2", C.c_double),
                 ("mean_lagrangian", C.c_double), ("gauss_max", C.c_double), ("gauss_rhs_rms", C.c_double),
-                ("nonfinite", C.c_int32), ("pad_", C.c_int32)]
+                ("nonfinite", C.c_int32), ("pad_", C.c_int32),
+                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double)]
 
 
 @dataclass
@@ -88,8 +89,9 @@ def lib():
                                      C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         _lib.aho_diag_compute.argtypes = [C.POINTER(_Params), dp, C.c_int64, C.POINTER(_Diag)]
         _lib.aho_site_fields.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp]
+        _lib.aho_site_fields4.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp, dp]
         for f in ("aho_philox4x32_10", "aho_ic", "aho_ic_window", "aho_coeffs", "aho_step", "aho_winding",
-                  "aho_diag_compute", "aho_site_fields"):
+                  "aho_diag_compute", "aho_site_fields", "aho_site_fields4"):
             getattr(_lib, f).restype = None
         assert _lib.aho_sizeof_params() == C.sizeof(_Params)
         assert _lib.aho_sizeof_diag() == C.sizeof(_Diag)
@@ -164,6 +166,14 @@ def site_fields(p: Params, f10: np.ndarray, n: int):
     K = np.empty((p.N,) * 3); G = np.empty((p.N,) * 3); L = np.empty((p.N,) * 3)
     lib().aho_site_fields(C.byref(p._c()), _dptr(f10), n, _dptr(K), _dptr(G), _dptr(L))
     return K, G, L
+
+
+def site_fields4(p: Params, f10: np.ndarray, n: int):
+    """Per-site K, G, Lag and the potential term Vp = (a^2 lambda(a)/4)(|phi|^2 - sigma^2)^2, each of shape (N, N, N)."""
+    _check_f10(p, f10)
+    K = np.empty((p.N,) * 3); G = np.empty((p.N,) * 3); L = np.empty((p.N,) * 3); Vp = np.empty((p.N,) * 3)
+    lib().aho_site_fields4(C.byref(p._c()), _dptr(f10), n, _dptr(K), _dptr(G), _dptr(L), _dptr(Vp))
+    return K, G, L, Vp
 
 
 def params_dict(p: Params) -> dict:

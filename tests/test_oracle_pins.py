@@ -738,3 +738,61 @@ def test_ic_window_is_the_sub_box_of_the_full_lattice(oracle):
             idx = [np.arange(o, o + B) % N for o in origin]
             ref = full[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]]
             assert np.array_equal(win, ref)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-1: potential-weighted <v^2>_V and the Lagrangian length estimator xi_L (L78-86)
+# ------------------------------------------------------------------------------------------------
+def test_potential_weighted_estimator_and_xi_L(oracle):
+    """(1) independent vectorised evaluation of sum K*Vp, sum G*Vp with Vp = (a^2 lambda(a)/4)(|phi|^2 - sigma^2)^2 on an
+    evolved state; (2) the boosted-profile identity R = v^2 holds for the potential weight as for any weight;
+    (3) xi_L = sqrt(-2 pi sigma^2 / mean Lag) (R20) on a hand-built state with a known mean Lagrangian;
+    (4) gauge invariance of the new sums."""
+    p = oracle.Params(N=12, m=2, s=0.5, e0=0.9, lambda0=1.7, dx=0.6, sigma=1.2)
+    f = oracle.initial_condition(p, seed=8)
+    oracle.step(p, f, 0, 25)
+    K, G, L = np_site_fields(p, f, 25)
+    phi = unpack(f)[0]
+    a = a_of(p, p.tau0 + 25 * p.dt)
+    Vp = p.lambda0 * a ** (2 * (p.s - 1)) * a ** 2 / 4 * (np.abs(phi) ** 2 - p.sigma ** 2) ** 2
+    Vo = oracle.site_fields4(p, f, 25)[3]
+    assert np.abs(Vp - Vo).max() < 1e-13 * max(1.0, Vp.max())
+    d = oracle.diagnostics(p, f, 25)
+    assert d["v2v_num"] == pytest.approx((K * Vp).sum(), rel=1e-11)
+    assert d["v2v_den"] == pytest.approx((G * Vp).sum(), rel=1e-11)
+    R = (K * Vp).sum() / (G * Vp).sum()
+    assert d["v2_V"] == pytest.approx(2 * R / (1 + R), rel=1e-10)
+    assert 0 < d["v2_V"] < 2                                   # a non-negative weight: the ratio is a proper average
+    if d["mean_lagrangian"] < 0:
+        assert d["xi_L"] == pytest.approx(math.sqrt(-TWO_PI * p.sigma ** 2 / d["mean_lagrangian"]), rel=1e-14)
+
+    # (2) rigidly translating profile: |phi-dot|^2 = v^2 |d_x phi|^2 pointwise -> R = v^2 for the potential weight too
+    N = 16
+    q = oracle.Params(N=N, m=0, s=1)
+    x = np.arange(N)[None, None, :] * np.ones((N, N, 1))
+    k = TWO_PI / N
+    prof = 1.0 + 0.3 * np.sin(k * x) + 0.2j * np.cos(2 * k * x)
+    v = 0.41
+    Pi = -v * (sh(prof, 0, 1) - prof) / q.dx
+    zero = np.zeros((N, N, N))
+    d = oracle.diagnostics(q, pack(prof, Pi, [zero] * 3, [zero] * 3), 0)
+    assert d["v2v_num"] / d["v2v_den"] == pytest.approx(v * v, rel=1e-12)
+    assert d["v2_V"] == pytest.approx(2 * v * v / (1 + v * v), rel=1e-12)
+
+    # (3) homogeneous phi = f0 (real), everything else zero: Lag = -Vp = -(lambda/4)(f0^2 - sigma^2)^2 at a = 1
+    f0 = 0.6
+    d = oracle.diagnostics(q, pack(np.full((N, N, N), f0 + 0j), zero + 0j, [zero] * 3, [zero] * 3), 0)
+    lag = -q.lambda0 / 4 * (f0 ** 2 - q.sigma ** 2) ** 2
+    assert d["mean_lagrangian"] == pytest.approx(lag, rel=1e-14)
+    assert d["xi_L"] == pytest.approx(math.sqrt(TWO_PI * q.sigma ** 2 / -lag), rel=1e-14)
+
+    # (4) random lattice gauge transformation leaves the new sums unchanged
+    rng = np.random.default_rng(11)
+    g = random_state(10, rng)
+    pg = oracle.Params(N=10, m=1, s=1)
+    phi, Pi, th, eps = unpack(g)
+    alpha = rng.uniform(-10, 10, (10, 10, 10))
+    g2 = pack(np.exp(1j * alpha) * phi, np.exp(1j * alpha) * Pi, [th[i] + (sh(alpha, i, 1) - alpha) for i in range(3)], eps)
+    d1, d2 = oracle.diagnostics(pg, g, 3), oracle.diagnostics(pg, g2, 3)
+    for key in ("v2v_num", "v2v_den", "v2_V", "xi_L"):
+        assert d1[key] == pytest.approx(d2[key], rel=1e-11, nan_ok=True)
