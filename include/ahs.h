@@ -103,6 +103,13 @@ typedef struct {
     double gauss_rhs_rms;     /* rms_x of the second term: the scale gauss_max is to be compared with      */
     int32_t nonfinite;        /* 1 if any stored field value is NaN or +-inf                               */
     int32_t reserved;
+    double v2v_num;           /* sum_x |Pi|^2 Vp^x, Vp = (a^2 lambda(a)/4)(|phi|^2 - sigma^2)^2: Eq. 10 with the
+                                 potential as the weight (L86, "two different weight functions")             */
+    double v2v_den;           /* sum_x |D phi|^2 Vp^x                                                      */
+    double v2_V;              /* 2R/(1+R), R = v2v_num / v2v_den: <v^2>_V (Eq. 9)                          */
+    double xi_L;              /* sqrt(-mu / mean_lagrangian), Eq. 9 (L78), with mu = 2 pi sigma^2 -- the paper
+                                 does not state mu; this is the Bogomolnyi tension at lambda = 2 e^2 (R20).
+                                 NaN when mean_lagrangian >= 0                                              */
 } ahs_diag;
 
 /* Bytes of device memory a simulation needs: 15 arrays of N^3 values (10 live + the phi', theta' shadow

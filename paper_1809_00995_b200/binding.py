@@ -42,7 +42,8 @@ class ahs_diag(C.Structure):
     _fields_ = [("step", C.c_int64), ("tau", C.c_double), ("n_pierced", C.c_uint64), ("sum_abs_w", C.c_uint64),
                 ("L", C.c_double), ("xi", C.c_double), ("v2_num", C.c_double), ("v2_den", C.c_double),
                 ("v2", C.c_double), ("mean_lagrangian", C.c_double), ("gauss_max", C.c_double),
-                ("gauss_rhs_rms", C.c_double), ("nonfinite", C.c_int32), ("reserved", C.c_int32)]
+                ("gauss_rhs_rms", C.c_double), ("nonfinite", C.c_int32), ("reserved", C.c_int32),
+                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double)]
 
 
 class AhsError(RuntimeError):

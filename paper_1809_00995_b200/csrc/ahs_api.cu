@@ -320,6 +320,11 @@ int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
     out->gauss_max = r.gmax;
     out->gauss_rhs_rms = std::sqrt(r.rhs2 / (double)s->nsites);
     out->nonfinite = r.nonfinite ? 1 : 0;
+    out->v2v_num = r.vnum;
+    out->v2v_den = r.vden;
+    const double Rv = r.vnum / r.vden;
+    out->v2_V = 2.0 * Rv / (1.0 + Rv);
+    out->xi_L = std::sqrt(-(2.0 * M_PI * p.sigma * p.sigma) / out->mean_lagrangian);   // mu = 2 pi sigma^2 (R20)
     s->diag_step = -1;
     if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "%llu sites hold a non-finite field value at step %lld",
                                     (unsigned long long)r.nonfinite, (long long)out->step);

@@ -189,7 +189,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         E2m = ldg_vec<T, V>(f.eps[2] + ((size_t)zm * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi));
     }
 
-    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, gmax = 0.0;
+    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, gmax = 0.0, vnum = 0.0, vden = 0.0;
     unsigned n_pierced = 0u, nonfinite = 0u;
     unsigned sum_abs_w = 0u;
     T gmax_t = T(0);
@@ -275,7 +275,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
 #pragma unroll
         for (int v = 0; v <= V; ++v) { n1c[v] = n1z[v]; a[v] = az[v]; ay[v] = azy[v]; }
 
-        T p_num = T(0), p_den = T(0), p_l = T(0), p_r2 = T(0);   // per thread and plane (V sites), then into the fp64 sums
+        T p_num = T(0), p_den = T(0), p_l = T(0), p_r2 = T(0), p_vn = T(0), p_vd = T(0);   // per thread and plane (V sites), then into the fp64 sums
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             const Cx<T> ph = { pr.v[v], pi.v[v] };
@@ -307,6 +307,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
             p_num += K * lag;
             p_den += Gd * lag;
             p_l += lag;
+            p_vn += K * Vp;   // potential-weighted estimator <v^2>_V (L86)
+            p_vd += Gd * Vp;
             nonfinite += finite_t(lag) ? 0u : 1u;   // every one of the ten values feeds lag: NaN or Inf in, NaN or Inf out
 
             // ---- Gauss residual ---------------------------------------------------------------------------------------------------
@@ -318,6 +320,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
             p_r2 += rhs * rhs;
         }
         num += (double)p_num; den += (double)p_den; lsum += (double)p_l; rhs2 += (double)p_r2;
+        vnum += (double)p_vn; vden += (double)p_vd;
         E2m = E2;
         // this warp is done with stage `sc` (plane it): release it to the copy-issuing thread
         __syncwarp();
@@ -325,7 +328,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     }
 
     gmax = (double)gmax_t;
-    DiagPartial acc = { (unsigned long long)n_pierced, (unsigned long long)sum_abs_w, num, den, lsum, gmax, rhs2, (unsigned long long)nonfinite };
+    DiagPartial acc = { (unsigned long long)n_pierced, (unsigned long long)sum_abs_w, num, den, lsum, gmax, rhs2, (unsigned long long)nonfinite, vnum, vden };
     block_reduce_store(acc, partials + blockIdx.x);
 }
 

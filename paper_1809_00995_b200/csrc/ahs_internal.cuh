@@ -37,7 +37,7 @@ struct DiagCoef {
     double gauss_rhs;      // 2 dx^2 e0^2 a_h^(2s), a_h = a(tau_n - dt/2)  (R4)
 };
 
-// One record per block / final result of the reduction (fixed 8 x 8 bytes).
+// One record per block / final result of the reduction (fixed 10 x 8 bytes).
 struct DiagPartial {
     unsigned long long n_pierced;
     unsigned long long sum_abs_w;
@@ -45,6 +45,7 @@ struct DiagPartial {
     double gmax;
     double rhs2;
     unsigned long long nonfinite;
+    double vnum, vden;     // potential-weighted sums: sum K Vp, sum G Vp
 };
 
 template <typename T>

@@ -54,6 +54,12 @@ def check_diag(O, p, sim, prec, snap, n):
     assert abs(d["v2_num"] - r["v2_num"]) <= rel * np.abs(K * Lg).sum() + 1e-300
     assert abs(d["v2_den"] - r["v2_den"]) <= rel * np.abs(G * Lg).sum() + 1e-300
     assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= rel * np.abs(Lg).mean() + 1e-300
+    Vp = O.site_fields4(p, snap, n)[3]                       # potential-weighted estimator and xi_L
+    floor = 1e-18 * Vp.size * max(1.0, G.max(), K.max())     # |phi| = sigma exactly (IC): Vp is rounding noise, ~1e-32
+    assert abs(d["v2v_num"] - r["v2v_num"]) <= rel * (K * Vp).sum() + floor
+    assert abs(d["v2v_den"] - r["v2v_den"]) <= rel * (G * Vp).sum() + floor
+    if r["mean_lagrangian"] < -1e-3 * np.abs(Lg).mean():
+        assert d["xi_L"] == pytest.approx(r["xi_L"], rel=50 * rel)
     eps_m = 2.3e-16 if prec == "f64" else 6e-8
     gscale = max(1.0, r["gauss_rhs_rms"], np.abs(snap[7:10]).max())
     assert abs(d["gauss_max"] - r["gauss_max"]) <= 64 * eps_m * gscale
