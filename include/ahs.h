@@ -73,6 +73,8 @@ enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
  *   device_buffer   DEVICE pointer, optional (NULL => the library calls cudaMalloc).  Must hold
  *                   ahs_required_bytes(N, precision) bytes, 256-byte aligned (e.g. torch.empty(...).data_ptr()).
  *   stream          cudaStream_t as void*, optional (NULL => the legacy default stream).
+ *   c_B             factor on the plaquette sum of Eq. 2 (L40) in the weight of <v^2>_L and in mean_lagrangian; 0 means 1, the
+ *                   value consistent with Eq. 5 (R2).  Eq. 2 as printed has 1/2; it does not enter the equations of motion.
  */
 typedef struct {
     int32_t N;
@@ -84,6 +86,7 @@ typedef struct {
     void* device_buffer;
     size_t device_buffer_bytes;
     void* stream;
+    double c_B;
 } ahs_params;
 
 /* Result of one diagnostics pass on the current snapshot (after `step` steps). */

@@ -35,7 +35,7 @@ class ahs_params(C.Structure):
                 ("dx", C.c_double), ("dt", C.c_double), ("lambda_", C.c_double), ("e", C.c_double),
                 ("sigma", C.c_double), ("m", C.c_double), ("s", C.c_double), ("tau0", C.c_double),
                 ("tau_ref", C.c_double), ("seed", C.c_uint64), ("device_buffer", C.c_void_p),
-                ("device_buffer_bytes", C.c_size_t), ("stream", C.c_void_p)]
+                ("device_buffer_bytes", C.c_size_t), ("stream", C.c_void_p), ("c_B", C.c_double)]
 
 
 class ahs_diag(C.Structure):
@@ -117,7 +117,7 @@ class Simulation:
     """One ahs_sim handle.  Methods mirror the C functions one to one."""
 
     def __init__(self, N, dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, m=1.0, s=0.0, tau0=1.0, seed=0,
-                 precision="f32", ic="random_phase", tau_ref=0.0, kernel="auto", use_torch=True):
+                 precision="f32", ic="random_phase", tau_ref=0.0, kernel="auto", use_torch=True, c_B=0.0):
         self._h = None
         lib = load()
         self.N = int(N)
@@ -129,6 +129,7 @@ class Simulation:
         p.N, p.precision, p.ic_kind, p.kernel = self.N, self.precision, _ICS[ic], _KERNELS[kernel]
         p.dx, p.dt, p.lambda_, p.e, p.sigma, p.m, p.s, p.tau0, p.tau_ref = dx, dt, lambda0, e0, sigma, m, s, tau0, tau_ref
         p.seed = seed
+        p.c_B = c_B
         self._buffer = None
         self.stream_handle = 0
         if use_torch:

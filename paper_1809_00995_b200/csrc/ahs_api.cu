@@ -112,7 +112,7 @@ DiagCoef diag_coefficients(const ahs_params& p, int64_t n)
     DiagCoef c;
     c.inv_dx2 = 1.0 / (p.dx * p.dx);
     c.gauge_norm = 1.0 / (2.0 * ea * ea * a * a * p.dx * p.dx);
-    c.cB_inv_dx2 = 1.0 / (p.dx * p.dx);
+    c.cB_inv_dx2 = (p.c_B != 0.0 ? p.c_B : 1.0) / (p.dx * p.dx);
     c.pot_coef = 0.25 * a * a * lambda_of(p, a);
     c.sigma2 = p.sigma * p.sigma;
     c.gauss_rhs = 2.0 * p.dx * p.dx * p.e * p.e * std::pow(a_h, 2.0 * p.s);
@@ -189,6 +189,7 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
         fail(AHS_ERR_INVALID_ARG, "m, s, tau0 must be finite and tau_ref >= 0"); return nullptr;
     }
     if (p.m != 0.0 && !(p.tau0 - 0.5 * p.dt > 0)) { fail(AHS_ERR_INVALID_ARG, "tau0 - dt/2 must be > 0 when m != 0"); return nullptr; }
+    if (!std::isfinite(p.c_B) || p.c_B < 0) { fail(AHS_ERR_INVALID_ARG, "c_B must be finite and >= 0 (0 = default 1)"); return nullptr; }
     if (p.kernel < AHS_KERNEL_AUTO || p.kernel > AHS_KERNEL_MARCH) { fail(AHS_ERR_INVALID_ARG, "unknown kernel %d", p.kernel); return nullptr; }
     const bool march_ok = p.precision == AHS_F32 ? march_supported<float>(p.N) : march_supported<double>(p.N);
     if (p.kernel == AHS_KERNEL_MARCH && !march_ok) {

@@ -424,3 +424,20 @@ def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
             out.append((hashlib.md5(sim.get_fields_native().tobytes()).hexdigest(), d["n_pierced"], d["v2_num"], d["gauss_max"]))
             assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"]), d
     assert out[0] == out[1]
+
+
+def test_c_B_parameter_reaches_the_weight(ahs, oracle):
+    """ahs_params.c_B (R2): the factor on the plaquette sum of Eq. 2 enters the Lagrangian weight only; 0.5 is Eq. 2 as printed."""
+    from paper_1809_00995_b200 import synthetic
+    N = 64
+    f = rounded(synthetic.random_snapshot(N, seed=5), "f64")
+    for cB in (0.5, 1.0):
+        p = oracle.Params(N=N, m=1.0, s=0.0, c_B=cB)
+        with ahs.Simulation(N=N, precision="f64", m=1.0, s=0.0, ic="none", c_B=cB) as sim:
+            sim.set_fields(f, 4)
+            d = sim.diagnostics()
+        r = oracle.diagnostics(p, f, 4)
+        K, G, Lg = oracle.site_fields(p, f, 4)
+        assert abs(d["v2_num"] - r["v2_num"]) <= 1e-10 * np.abs(K * Lg).sum()
+        assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= 1e-10 * np.abs(Lg).mean()
+        assert d["n_pierced"] == r["n_pierced"] and d["v2v_num"] == pytest.approx(r["v2v_num"], rel=1e-10)
