@@ -65,7 +65,7 @@ struct DiagPtrs {
 template <typename T> int launch_ic(T* phi_re, T* phi_im, int N, double sigma, uint64_t seed, int kind, cudaStream_t st);
 template <typename T> int launch_step_generic(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st);
 // TMA descriptors of the step march: the four-array stage and theta_2 of one (phi, theta) buffer, and the momenta
-struct StepMaps { CUtensorMap stage, th2, mom; };
+struct StepMaps { CUtensorMap stage, th2, mom, wstage, wth2; };   // w*: the V-wide wrapped halo column of x-edge tiles
 template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps /* HOST, may be NULL */, cudaStream_t st);
 template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi_re_base, int N, size_t array_bytes);
 template <typename T> bool march_supported(int N);

@@ -58,13 +58,18 @@ struct MarchCfg {
     static constexpr int XEX_ELEMS = 4 * TY;              // b0.re, b0.im, S01, S02 of the halo column (one parity)
     static constexpr int T2_STRIDE = (int)(((G::ARR_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
     static_assert(G::STAGE_BYTES % 128 == 0, "stages stay 128-byte aligned");
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * T2_STRIDE + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
+    // x-edge tiles under TMA: the wrapped halo column (V wide) of a plane lands in a side buffer, one tensor copy each
+    static constexpr int WRAP_ELEMS = (int)(((4 * G::ROWS * V * sizeof(T) + 127) & ~(size_t)127) / sizeof(T));   // phi_re, phi_im, theta_0, theta_1
+    static constexpr int WRAP2_STRIDE = (int)(((G::ROWS * V * sizeof(T) + 127) & ~(size_t)127) / sizeof(T));   // theta_2
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * G::STAGE_ELEMS + T2_SLOTS * T2_STRIDE + NSTAGE * WRAP_ELEMS +
+                                                              T2_SLOTS * WRAP2_STRIDE + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
 
 template <typename T, int TY, int MINB>
 __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB)
 step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
-                  const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_mom, int use_tma)
+                  const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_mom,
+                  const __grid_constant__ CUtensorMap map_wstage, const __grid_constant__ CUtensorMap map_wth2, int use_tma)
 {
     using C = MarchCfg<T, TY>;
     using G = typename C::G;
@@ -79,7 +84,9 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     uint64_t* xch = full + NS;   // exchange barrier: one phase per plane, every thread arrives
     T* stages = reinterpret_cast<T*>(smem + 128);
     T* th2ring = stages + NS * SE;
-    T* yex = th2ring + C::T2_SLOTS * C::T2_STRIDE;
+    T* wrapS = th2ring + C::T2_SLOTS * C::T2_STRIDE;      // side buffers of the wrapped halo column (x-edge tiles under TMA)
+    T* wrapT = wrapS + NS * C::WRAP_ELEMS;
+    T* yex = wrapT + C::T2_SLOTS * C::WRAP2_STRIDE;
     T* xex = yex + 2 * C::YEX_ELEMS;
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -106,14 +113,36 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     auto plane_of = [&](int i) { const int z = z0 - 1 + i; return z < 0 ? z + N : (z >= N ? z - N : z); };
     // Tiles that do not touch the periodic boundary fetch a plane with two tensor copies (UTMALDG: the four-array stage
     // and theta_2) instead of 30 row copies; the others keep the row copies (TMA zero-fills out of bounds, it does not wrap).
-    const bool tma_tile = (use_tma & 1) && x0 > 0 && x0 + TX < N && y0 > 0 && y0 + TY < N;
+    // x-edge tiles: the main box runs out of bounds on one side (zero-filled) and the wrapped halo column (x = N-V.. for the
+    // left edge, x = 0.. for the right edge) arrives by a second, V-wide tensor copy in a side buffer, which the few readers of
+    // that column use instead.  y-edge tiles (2 of N/TY tile rows) and lattices one tile wide keep the row copies.
+    const bool left_edge = x0 == 0, right_edge = x0 + TX == N;
+    const bool tma_tile = (use_tma & 1) && y0 > 0 && y0 + TY < N && !(left_edge && right_edge);
+    const bool wrapL = tma_tile && left_edge, wrapR = tma_tile && right_edge;
+    const int xw = left_edge ? N - V : 0;
+    const uint32_t wrap_tx = (wrapL || wrapR) ? (uint32_t)(4 * G::ROWS * V * sizeof(T)) : 0u, wrap2_tx = (wrapL || wrapR) ? (uint32_t)(G::ROWS * V * sizeof(T)) : 0u;
     auto issue_stage = [&](int s, int p) {   // phi_re, phi_im, theta_0, theta_1 of march plane p -> stage s
-        if (tma_tile) tma_load_4d(stages + s * SE, &map_stage, x0 - V, y0 - 1, plane_of(p), 0, &full[s]);
-        else issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+        if (tma_tile) {
+            tma_load_4d(stages + s * SE, &map_stage, x0 - V, y0 - 1, plane_of(p), 0, &full[s]);
+            if (wrapL || wrapR) tma_load_4d(wrapS + s * C::WRAP_ELEMS, &map_wstage, xw, y0 - 1, plane_of(p), 0, &full[s]);
+        } else {
+            issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+        }
     };
     auto issue_th2 = [&](int slot, int bar, int p) {   // theta_2 of march plane p -> ring slot, completion on full[bar]
-        if (tma_tile) tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &full[bar]);
-        else issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &full[bar], src2, N, x0, y0, plane_of(p));
+        if (tma_tile) {
+            tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &full[bar]);
+            if (wrapL || wrapR) tma_load_4d(wrapT + slot * C::WRAP2_STRIDE, &map_wth2, xw, y0 - 1, plane_of(p), 4, &full[bar]);
+        } else {
+            issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &full[bar], src2, N, x0, y0, plane_of(p));
+        }
+    };
+    // column x0-1 (array a, row r) of a staged plane / of a theta_2 slot, and the element right of this thread's vector
+    auto colL = [&](const T* st, const T* side, int a, int r) -> T {
+        return wrapL ? side[(a * G::ROWS + r + 1) * V + V - 1] : st[G::idx(a, r, -1)];
+    };
+    auto edgeR = [&](const T* st, const T* side, int a, int r, int c) -> T {   // c = column index of the element, <= TX
+        return (wrapR && c == TX) ? side[(a * G::ROWS + r + 1) * V] : st[G::idx(a, r, c)];
     };
     // the momenta of plane z (no halo) are asked into L2 one plane ahead of the streaming loads that consume them
     auto prefetch_momenta = [&](int z) {
@@ -127,7 +156,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         for (int i = 0; i < NS; ++i) {
             const bool t2 = i < C::T2_SLOTS;   // theta_2 of planes 0, 1 ride on the barriers of planes 0, 1
             if (elect_one()) {
-                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + (t2 ? G::ARR_BYTES : 0u));
+                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx + (t2 ? G::ARR_BYTES + wrap2_tx : 0u));
                 issue_stage(i, i);
                 if (t2) issue_th2(i, i, i);
                 if (i == 0) prefetch_momenta(z0);
@@ -149,7 +178,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(t2c + G::idx(0, w, xi));
         const VecT t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
-        const T t2x_edge = t2c[G::idx(0, w, xi + V)];
+        const T t2x_edge = edgeR(t2c, wrapT, 0, w, xi + V);
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             T s, c;
@@ -179,6 +208,9 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
         const T* t2c = th2ring + (it & 1) * C::T2_STRIDE;
+        const T* wsc = wrapS + (it % NS) * C::WRAP_ELEMS;
+        const T* wsn = wrapS + ((it + 1) % NS) * C::WRAP_ELEMS;
+        const T* wtc = wrapT + (it & 1) * C::WRAP2_STRIDE;
         T* yexp = yex + (it & 1) * C::YEX_ELEMS;
         T* xexp = xex + (it & 1) * C::XEX_ELEMS;
 
@@ -186,7 +218,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
             const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
             fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1: all reads of that stage are done)
-            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES);
+            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES + wrap_tx + wrap2_tx);
             issue_stage(s, it + 2);
             issue_th2((it + 1) & 1, s, it + 1);
         }
@@ -209,7 +241,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
                 const int x = 32 * (w / HSTRIDE) + lane;   // halo row y0-1: b_1, S_01, S_12 -> exchange row 0
                 const T pr = sc[G::idx(0, -1, x)], pi = sc[G::idx(1, -1, x)];
                 const T t0 = sc[G::idx(2, -1, x)], t1 = sc[G::idx(3, -1, x)], t2 = t2c[G::idx(0, -1, x)];
-                const T t1x = sc[G::idx(3, -1, x + 1)], t0y = sc[G::idx(2, 0, x)], t2y = t2c[G::idx(0, 0, x)], t1z = sn[G::idx(3, -1, x)];
+                const T t1x = edgeR(sc, wsc, 3, -1, x + 1), t0y = sc[G::idx(2, 0, x)], t2y = t2c[G::idx(0, 0, x)], t1z = sn[G::idx(3, -1, x)];
                 T s, c;
                 sincos_fast(t1, s, c);
                 const Cx<T> b = mulUc<T>(c, s, { pr, pi });
@@ -220,10 +252,10 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             }
             if (((w + it) % TY) == COLUMN && lane < TY) {   // halo column x0-1, row r = lane: b_0, S_01, S_02
                 const int r = lane;
-                const T pr = sc[G::idx(0, r, -1)], pi = sc[G::idx(1, r, -1)];
-                const T t0 = sc[G::idx(2, r, -1)], t1 = sc[G::idx(3, r, -1)], t2 = t2c[G::idx(0, r, -1)];
+                const T pr = colL(sc, wsc, 0, r), pi = colL(sc, wsc, 1, r);
+                const T t0 = colL(sc, wsc, 2, r), t1 = colL(sc, wsc, 3, r), t2 = colL(t2c, wtc, 0, r);
                 const T t1x = sc[G::idx(3, r, 0)], t2x = t2c[G::idx(0, r, 0)];
-                const T t0y = sc[G::idx(2, r + 1, -1)], t0z = sn[G::idx(2, r, -1)];
+                const T t0y = colL(sc, wsc, 2, r + 1), t0z = colL(sn, wsn, 2, r);
                 T s, c;
                 sincos_fast(t0, s, c);
                 const Cx<T> b = mulUc<T>(c, s, { pr, pi });
@@ -244,8 +276,8 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
             const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
             const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
-            const T prx_e = sc[G::idx(0, w, xi + V)], pix_e = sc[G::idx(1, w, xi + V)];
-            const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = t2c[G::idx(0, w, xi + V)];
+            const T prx_e = edgeR(sc, wsc, 0, w, xi + V), pix_e = edgeR(sc, wsc, 1, w, xi + V);
+            const T t1x_e = edgeR(sc, wsc, 3, w, xi + V), t2x_e = edgeR(t2c, wtc, 0, w, xi + V);
             T lfr[V], lfi[V], J0[V], J1[V], J2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], b2r[V], b2i[V];
             VecT yb1r, yb1i, yS01, yS12;
 #pragma unroll
@@ -386,11 +418,11 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* 
     // plane ahead (off: with the software-pipelined loads it only adds 5 % of DRAM reads, profiles/r2_step1024_f32_full.md)
     static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 3 : 1); }();
     if (maps && tma_mode) {
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, tma_mode);
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, maps->wstage, maps->wth2, tma_mode);
     } else {
         StepMaps none;
         memset(&none, 0, sizeof(none));
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, none.stage, none.th2, none.mom, 0);
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, none.stage, none.th2, none.mom, none.wstage, none.wth2, 0);
     }
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
@@ -431,7 +463,9 @@ bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi
     if (!march_supported<T>(N)) return false;
     return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
            make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
-           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, C::TY, 5);
+           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, C::TY, 5) &&
+           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 4) &&
+           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 1);
 }
 template bool make_step_march_maps<float>(StepMaps*, const void*, const void*, int, size_t);
 template bool make_step_march_maps<double>(StepMaps*, const void*, const void*, int, size_t);
