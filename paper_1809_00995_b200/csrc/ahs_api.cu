@@ -28,7 +28,7 @@ struct ahs_sim {
     DiagPartial* result_host;  // pinned host, 1 record
     int64_t diag_step;       // step the pending diagnostics launch refers to (-1: none)
     int device;
-    CUtensorMap diag_map[2];   // TMA descriptors of (phi, theta) buffer 0 / 1 for the diagnostics march
+    DiagMaps diag_map[2];      // TMA descriptors of (phi, theta) buffer 0 / 1 for the diagnostics march
     bool diag_map_ok;
     StepMaps step_maps[2];     // the same for the step march (buffer 0 / 1 as the level-n input)
     bool step_maps_ok;

@@ -46,7 +46,9 @@ struct DiagCfg {
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
     static constexpr int STAGE_STRIDE = (int)(((G::STAGE_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * STAGE_STRIDE);
+    // right-edge tiles under TMA: the wrapped forward halo column (x = 0 .. V-1) of a plane lands in a side buffer
+    static constexpr int WRAP_STRIDE = (int)(((5 * G::ROWS * V * sizeof(T) + 127) & ~(size_t)127) / sizeof(T));
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * (STAGE_STRIDE + WRAP_STRIDE));
 };
 
 // Link number of the link s -> t with angle th, fast path, all in fp32: t = (arg_t - arg_s - th) / 2 pi from the
@@ -105,7 +107,8 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
 template <typename T, int TY, int MINB, int NSTAGES>
 __global__ void __launch_bounds__(DiagCfg<T, TY, NSTAGES>::NTHREADS, MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
-                  unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap, int use_tma, int rotate)
+                  unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
+                  const __grid_constant__ CUtensorMap wmap, int use_tma, int rotate)
 {
     using C = DiagCfg<T, TY, NSTAGES>;
     using G = typename C::G;
@@ -116,6 +119,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
     uint64_t* empty = full + NS;                           // empty[s]: all TY warps have finished reading stage s
     T* stages = reinterpret_cast<T*>(smem + 128);
+    T* wraps = stages + NS * SE;                           // side buffers of the wrapped column (right-edge tiles under TMA)
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tiles_x = N / TX, tiles_y = N / TY;
@@ -139,12 +143,24 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
 
     // plane index p of this CTA's march = lattice plane z0 + p (periodic); planes 0 .. zlen are needed
     auto plane_of = [&](int p) { const int z = z0 + p; return z >= N ? z - N : z; };
-    // one tensor copy per plane for tiles that do not touch the periodic boundary, row copies for the others
-    const bool tma_tile = use_tma && (x0 + TX < N) && (y0 + TY < N);
+    // One tensor copy per plane for tiles away from the periodic boundary.  Tiles on the right edge get the main box
+    // (zero-filled out of bounds) plus a V-wide tensor copy of the wrapped column x = 0 .. V-1 into a side buffer, which the
+    // readers of column TX use instead; tiles on the top edge in y (2 of N/TY tile rows) keep the row copies.
+    const bool right_edge = x0 + TX == N;
+    const bool tma_tile = use_tma && (y0 + TY < N);
+    const bool wrapR = tma_tile && right_edge;
     auto issue_plane = [&](int s, int p) {
-        mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES);
-        if (tma_tile) tma_load_4d(stages + s * SE, &tmap, x0, y0, plane_of(p), 0, &full[s]);
-        else issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+        mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + (wrapR ? (uint32_t)(5 * G::ROWS * V * sizeof(T)) : 0u));
+        if (tma_tile) {
+            tma_load_4d(stages + s * SE, &tmap, x0, y0, plane_of(p), 0, &full[s]);
+            if (wrapR) tma_load_4d(wraps + s * C::WRAP_STRIDE, &wmap, 0, y0, plane_of(p), 0, &full[s]);
+        } else {
+            issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
+        }
+    };
+    // element (array a, row r) right of this thread's vector: column xi + V (= TX for the last lane)
+    auto edge = [&](const T* st, int a, int r) -> T {
+        return (wrapR && lane == 31) ? (wraps + (st - stages) / SE * C::WRAP_STRIDE)[(a * G::ROWS + r) * V] : st[G::idx(a, r, xi + V)];
     };
     if (w == 0 && elect_one()) {
 #pragma unroll
@@ -163,8 +179,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
             a0[v] = atan2_fast((float)pi.v[v], (float)pr.v[v]);
             a1[v] = atan2_fast((float)piy.v[v], (float)pry.v[v]);
         }
-        a0[V] = atan2_fast((float)st[G::idx(1, w, xi + V)], (float)st[G::idx(0, w, xi + V)]);
-        a1[V] = atan2_fast((float)st[G::idx(1, w + 1, xi + V)], (float)st[G::idx(0, w + 1, xi + V)]);
+        a0[V] = atan2_fast((float)edge(st, 1, w), (float)edge(st, 0, w));
+        a1[V] = atan2_fast((float)edge(st, 1, w + 1), (float)edge(st, 0, w + 1));
     };
 
     mbar_wait(&full[0], 0);
@@ -174,7 +190,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     args_of(stages, a, ay);
     {
         const VecT t0 = lds_vec<T, V>(stages + G::idx(2, w, xi)), t1 = lds_vec<T, V>(stages + G::idx(3, w, xi));
-        const T t1x_e = stages[G::idx(3, w, xi + V)];
+        const T t1x_e = edge(stages, 3, w);
 #pragma unroll
         for (int v = 0; v <= V; ++v) {
             n1c[v] = link_number(a[v], ay[v], (float)(v < V ? t1.v[v < V ? v : 0] : t1x_e), slack_c);
@@ -226,8 +242,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(sc + G::idx(4, w + 1, xi));
         const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
-        const T prx_e = sc[G::idx(0, w, xi + V)], pix_e = sc[G::idx(1, w, xi + V)];
-        const T t1x_e = sc[G::idx(3, w, xi + V)], t2x_e = sc[G::idx(4, w, xi + V)];
+        const T prx_e = edge(sc, 0, w), pix_e = edge(sc, 1, w);
+        const T t1x_e = edge(sc, 3, w), t2x_e = edge(sc, 4, w);
         // E0 of the site to the left: previous element, else lane-1's last element, else (lane 0) the halo value
         T e0_left = __shfl_up_sync(0xffffffffu, E0.v[V - 1], 1);
         if (lane == 0) e0_left = e0_halo;
@@ -238,7 +254,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         float n2[V + 1], n0y[V], n2y[V], n0z[V], n1z[V + 1];
         slack_c = 1.0f;
         {
-            const T t1z_e = sn[G::idx(3, w, xi + V)];
+            const T t1z_e = edge(sn, 3, w);
 #pragma unroll
             for (int v = 0; v <= V; ++v) {
                 n2[v] = link_number(a[v], az[v], (float)(v < V ? t2.v[v < V ? v : 0] : t2x_e), slack);
@@ -347,7 +363,7 @@ int pick_zlen(int N, int ctas_per_sm, int max_partials)
 
 template <typename T, int TY, int MINB, int NSTAGES = 4>
 int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-               void* list, size_t list_bytes, const CUtensorMap* tmap, cudaStream_t st)
+               void* list, size_t list_bytes, const DiagMaps* tmap, cudaStream_t st)
 {
     using C = DiagCfg<T, TY, NSTAGES>;
     auto kern = diag_march_kernel<T, TY, MINB, NSTAGES>;
@@ -366,10 +382,11 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
     if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
     static const bool tma_off = getenv("AHS_NO_TMA") != nullptr;
     static const int rot = [] { const char* e = getenv("AHS_DIAG_ROT"); return e ? atoi(e) : 1; }();
-    CUtensorMap none;
+    DiagMaps none;
     memset(&none, 0, sizeof(none));
     const bool use_tma = tmap && !tma_off;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, use_tma ? *tmap : none, use_tma ? 1 : 0, rot);
+    const DiagMaps& mp = use_tma ? *tmap : none;
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0, rot);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
@@ -381,7 +398,7 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
 
 template <typename T>
 int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-                      void* list, size_t list_bytes, const CUtensorMap* tmap, cudaStream_t st)
+                      void* list, size_t list_bytes, const DiagMaps* tmap, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
     // 4-row tiles (3 CTAs/SM) by default; AHS_DIAG_TY=8 selects 8-row tiles, two CTAs per SM (experiments)
@@ -395,16 +412,17 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartia
 
 // the tensor map of one (phi, theta) buffer for the default tile shape (4 rows): box (TX + V, TY + 1, 1, 5)
 template <typename T>
-bool make_diag_march_map(CUtensorMap* out, const void* phi_re_base, int N, size_t array_bytes)
+bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t array_bytes)
 {
     using G = typename DiagCfg<T, 4>::G;
     if (!march_supported<T>(N)) return false;
-    return make_tile_map<T>(out, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 5);
+    return make_tile_map<T>(&out->tile, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 5) &&
+           make_tile_map<T>(&out->wrap, phi_re_base, N, array_bytes, 5, G::V, G::ROWS, 5);
 }
-template bool make_diag_march_map<float>(CUtensorMap*, const void*, int, size_t);
-template bool make_diag_march_map<double>(CUtensorMap*, const void*, int, size_t);
+template bool make_diag_march_map<float>(DiagMaps*, const void*, int, size_t);
+template bool make_diag_march_map<double>(DiagMaps*, const void*, int, size_t);
 
-template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const CUtensorMap*, cudaStream_t);
-template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const CUtensorMap*, cudaStream_t);
+template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, cudaStream_t);
+template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, cudaStream_t);
 
 }  // namespace ahs

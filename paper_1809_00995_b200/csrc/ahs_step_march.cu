@@ -221,6 +221,12 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES + wrap_tx + wrap2_tx);
             issue_stage(s, it + 2);
             issue_th2((it + 1) & 1, s, it + 1);
+            if ((use_tma & 4) && tma_tile && it + 3 <= zlen + 1) {   // (experiment) the plane after that: into L2 only
+                asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_stage)),
+                             "r"(x0 - V), "r"(y0 - 1), "r"(plane_of(it + 3)), "r"(0) : "memory");
+                asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_th2)),
+                             "r"(x0 - V), "r"(y0 - 1), "r"(plane_of(it + 2)), "r"(4) : "memory");
+            }
         }
         if (((w + it) % TY) == ISSUER && it < zlen && elect_one()) prefetch_momenta(z0 + it);   // plane of iteration it+1
 
@@ -416,7 +422,7 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* 
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
     // AHS_STEP_TMA (experiments): bit 0 = tensor copies for the stages (default), bit 1 = L2 prefetch of the momenta one
     // plane ahead (off: with the software-pipelined loads it only adds 5 % of DRAM reads, profiles/r2_step1024_f32_full.md)
-    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 3 : 1); }();
+    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 7 : 1); }();
     if (maps && tma_mode) {
         kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, maps->wstage, maps->wth2, tma_mode);
     } else {
