@@ -40,9 +40,8 @@ FALLBACK_HBM_GBS = 6650.0                         # B200_PROFILING.md fallback i
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed `ncu --set full`
 # capture (profiles/); keyed by (kernel, precision, lattice).  None = no capture for that configuration.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r2_step1024_f32_full.md: 49.53 GB read + 42.90 GB written (capture taken with the momenta L2 prefetch still on;
-    # without it the r1 capture of the same stages read 47.08 GB)
-    ("march", "f32", 1024): 92.44e9,
+    # profiles/r3_step1024_f32_full.md: 48.35 GB read + 42.90 GB written per launch
+    ("march", "f32", 1024): 91.25e9,
 }
 
 
