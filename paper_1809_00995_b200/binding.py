@@ -60,7 +60,7 @@ def load(path: str | None = None):
     global _lib
     if _lib is not None:
         return _lib
-    path = path or _build.build_library()
+    path = path or os.environ.get("AHS_LIBRARY") or _build.build_library()   # AHS_LIBRARY: an already built libahs.so
     lib = C.CDLL(path)
     vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
     lib.ahs_required_bytes.argtypes = [i32, i32]; lib.ahs_required_bytes.restype = C.c_size_t

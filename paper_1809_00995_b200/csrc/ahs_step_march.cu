@@ -231,12 +231,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         if (((w + it) % TY) == ISSUER && it < zlen && elect_one()) prefetch_momenta(z0 + it);   // plane of iteration it+1
 
         const size_t g = gnext;                                         // plane z0 + it - 1
-#ifdef AHS_NO_PIPELINE
-        const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
-        const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
-#else
-        const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested right after the previous plane's barrier
-#endif
+        const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested one plane ago
 
         mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
 
@@ -353,12 +348,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             }
         }
         gnext = g + plane_stride;
-#ifndef AHS_NO_PIPELINE
-        if (it < zlen)
-#else
-        if (false)
-#endif
-        {
+        if (it < zlen) {
             nPr = ldg_vec<T, V>(f.pi_re + gnext); nPi = ldg_vec<T, V>(f.pi_im + gnext);
             nE0 = ldg_vec<T, V>(f.eps[0] + gnext); nE1 = ldg_vec<T, V>(f.eps[1] + gnext); nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
         }
