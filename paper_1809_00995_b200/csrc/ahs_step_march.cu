@@ -439,7 +439,7 @@ int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const Ste
     // 4-row tiles, four CTAs (barrier domains) per SM, measured fastest (profiles/); AHS_MARCH_TY=8 (experiments
     // only) selects 8-row tiles, two CTAs per SM
     static const int ty = [] { const char* e = getenv("AHS_MARCH_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, nullptr, st);
+    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, maps, st);   // (the maps are built for the same AHS_MARCH_TY)
     if (ty == 16 && N % 16 == 0) return launch_cfg<T, 16, 1>(f, N, c, nullptr, st);
     return launch_cfg<T, 4, 3>(f, N, c, maps, st);
 }
@@ -457,11 +457,13 @@ bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi
     using C = MarchCfg<T, 4>;
     using G = typename C::G;
     if (!march_supported<T>(N)) return false;
-    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
-           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
-           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, C::TY, 5) &&
-           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 4) &&
-           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 1);
+    const char* e = getenv("AHS_MARCH_TY");
+    const int rows = (e && atoi(e) == 8) ? 10 : G::ROWS, ty = rows - 2;   // experiments: 8-row tiles
+    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, rows, 4) &&
+           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, rows, 1) &&
+           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, ty, 5) &&
+           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, rows, 4) &&
+           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, rows, 1);
 }
 template bool make_step_march_maps<float>(StepMaps*, const void*, const void*, int, size_t);
 template bool make_step_march_maps<double>(StepMaps*, const void*, const void*, int, size_t);

@@ -37,10 +37,13 @@ __device__ __forceinline__ void sincos_fast(float x, float& s, float& c)
     pc = fmaf(z, pc, 0.04166662320494652f);
     pc = fmaf(z, pc, -0.5f);
     const float cr = fmaf(z, pc, 1.0f);
+    // quadrant k mod 4 = 0: (sr, cr), 1: (cr, -sr), 2: (-sr, -cr), 3: (-cr, sr): one sign word (bit 1 of k) on both, then
+    // the odd quadrants swap and negate -- the negation rides on the select
+    const int sgn = (q << 30) & 0x80000000;
+    const float X = __int_as_float(__float_as_int(sr) ^ sgn), Y = __int_as_float(__float_as_int(cr) ^ sgn);
     const bool odd = q & 1;
-    const float so = odd ? cr : sr, co = odd ? sr : cr;
-    s = __int_as_float(__float_as_int(so) ^ ((q << 30) & 0x80000000));
-    c = __int_as_float(__float_as_int(co) ^ (((q + 1) << 30) & 0x80000000));
+    s = odd ? Y : X;
+    c = odd ? -X : Y;
 }
 
 __device__ __forceinline__ float sin_fast(float x)
@@ -115,9 +118,10 @@ __device__ __forceinline__ void sincos_fast(double x, double& s, double& c)
     pc = fma(z, pc, -0.0013888888888873554);
     pc = fma(z, pc, 0.041666666666666595);
     const double cr = fma(z * z, pc, fma(z, -0.5, 1.0));
+    const double X = trig64::flip(sr, q), Y = trig64::flip(cr, q);   // same quadrant logic as the fp32 version
     const bool odd = q & 1;
-    s = trig64::flip(odd ? cr : sr, q);
-    c = trig64::flip(odd ? sr : cr, q + 1);
+    s = odd ? Y : X;
+    c = odd ? -X : Y;
 }
 
 __device__ __forceinline__ double sin_fast(double x)
