@@ -179,16 +179,18 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         const VecT t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
         const T t2x_edge = edgeR(t2c, wrapT, 0, w, xi + V);
+        T s2[V], c2[V], X02[V], X12[V];
+        sincos_vec<V>(t2.v, s2, c2);
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            T s, c;
-            sincos_fast(t2.v[v], s, c);
-            const Cx<T> b = mulUc<T>(c, s, { pr.v[v], pi.v[v] });
+            const Cx<T> b = mulUc<T>(c2[v], s2[v], { pr.v[v], pi.v[v] });
             cb2r[v] = b.re;
             cb2i[v] = b.im;
-            cS02[v] = sin_fast(t0.v[v] + next_x<T, V>(t2, v, t2x_edge) - t0z.v[v] - t2.v[v]);
-            cS12[v] = sin_fast(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
+            X02[v] = t0.v[v] + next_x<T, V>(t2, v, t2x_edge) - t0z.v[v] - t2.v[v];
+            X12[v] = t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v];
         }
+        sin_vec<V>(X02, cS02);
+        sin_vec<V>(X12, cS12);
     }
     __syncthreads();
     wait_barrier_resolved(full);   // the first in-loop copy re-fills the stage the prologue has just read
@@ -281,19 +283,33 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             const T t1x_e = edgeR(sc, wsc, 3, w, xi + V), t2x_e = edgeR(t2c, wtc, 0, w, xi + V);
             T lfr[V], lfi[V], J0[V], J1[V], J2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], b2r[V], b2i[V];
             VecT yb1r, yb1i, yS01, yS12;
+            // the six transcendental evaluations per site, V sites at once (fp32: packed two-lane arithmetic, ahs_trig.cuh)
+            T s0[V], c0[V], s1[V], c1[V], s2[V], c2[V];
+            sincos_vec<V>(t0.v, s0, c0);
+            sincos_vec<V>(t1.v, s1, c1);
+            sincos_vec<V>(t2.v, s2, c2);
+            {
+                // Xi_ij^x = th_i^x + th_j^{x+k_i} - th_i^{x+k_j} - th_j^x  (Eq. 3)
+                T X01[V], X02[V], X12[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    X01[v] = t0.v[v] + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - t1.v[v];
+                    X02[v] = t0.v[v] + next_x<T, V>(t2, v, t2x_e) - t0z.v[v] - t2.v[v];
+                    X12[v] = t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v];
+                }
+                sin_vec<V>(X01, S01);
+                sin_vec<V>(X02, S02);
+                sin_vec<V>(X12, S12);
+            }
 #pragma unroll
             for (int v = 0; v < V; ++v) {
                 const Cx<T> ph = { pr.v[v], pi.v[v] };
-                T s, c;
-                sincos_fast(t0.v[v], s, c);
-                const Cx<T> f0 = mulU<T>(c, s, { next_x<T, V>(pr, v, prx_e), next_x<T, V>(pi, v, pix_e) });
-                const Cx<T> b0 = mulUc<T>(c, s, ph);
-                sincos_fast(t1.v[v], s, c);
-                const Cx<T> f1 = mulU<T>(c, s, { pry.v[v], piy.v[v] });
-                const Cx<T> b1 = mulUc<T>(c, s, ph);
-                sincos_fast(t2.v[v], s, c);
-                const Cx<T> f2 = mulU<T>(c, s, { prz.v[v], piz.v[v] });
-                const Cx<T> b2 = mulUc<T>(c, s, ph);
+                const Cx<T> f0 = mulU<T>(c0[v], s0[v], { next_x<T, V>(pr, v, prx_e), next_x<T, V>(pi, v, pix_e) });
+                const Cx<T> b0 = mulUc<T>(c0[v], s0[v], ph);
+                const Cx<T> f1 = mulU<T>(c1[v], s1[v], { pry.v[v], piy.v[v] });
+                const Cx<T> b1 = mulUc<T>(c1[v], s1[v], ph);
+                const Cx<T> f2 = mulU<T>(c2[v], s2[v], { prz.v[v], piz.v[v] });
+                const Cx<T> b2 = mulUc<T>(c2[v], s2[v], ph);
                 lfr[v] = (f0.re + f1.re) + f2.re;
                 lfi[v] = (f0.im + f1.im) + f2.im;
                 // J_j = Im[conj(phi^x) U_j phi^{x+k_j}]  (Eq. 5, 2nd term)
@@ -303,10 +319,6 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
                 b0r[v] = b0.re; b0i[v] = b0.im;
                 yb1r.v[v] = b1.re; yb1i.v[v] = b1.im;
                 b2r[v] = b2.re; b2i[v] = b2.im;
-                // Xi_ij^x = th_i^x + th_j^{x+k_i} - th_i^{x+k_j} - th_j^x  (Eq. 3)
-                S01[v] = sin_fast(t0.v[v] + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - t1.v[v]);
-                S02[v] = sin_fast(t0.v[v] + next_x<T, V>(t2, v, t2x_e) - t0z.v[v] - t2.v[v]);
-                S12[v] = sin_fast(t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v]);
                 yS01.v[v] = S01[v];
                 yS12.v[v] = S12[v];
             }

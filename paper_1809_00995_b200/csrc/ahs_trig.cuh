@@ -22,44 +22,93 @@
 namespace ahs {
 
 // ---- fp32 ---------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void sincos_fast(float x, float& s, float& c)
+// The arithmetic is written once over a lane type W: float, or float2 evaluated with Blackwell's packed fp32
+// instructions (FFMA2 / FMUL2 / FADD2 on sm_100: two IEEE fp32 operations per issued instruction, constants broadcast from
+// immediates).  Both give bit-identical results per lane; the marching kernels use the packed form on pairs of sites,
+// which takes a quarter of the instructions out of the step kernel's trigonometry (profiles/r3).
+namespace lanes {
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float mul_(float a, float b) { return a * b; }
+__device__ __forceinline__ float add_(float a, float b) { return a + b; }
+__device__ __forceinline__ float2 fma_(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul_(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add_(float2 a, float2 b) { return __fadd2_rn(a, b); }
+template <typename W> __device__ __forceinline__ W all(float v);
+template <> __device__ __forceinline__ float all<float>(float v) { return v; }
+template <> __device__ __forceinline__ float2 all<float2>(float v) { return make_float2(v, v); }
+}  // namespace lanes
+
+// t = x * 2/pi + 1.5 * 2^23 (its low mantissa bits hold k = rint(x * 2/pi)); sr = sin(r), cr = cos(r), r = x - k pi/2
+template <typename W>
+__device__ __forceinline__ void sincos_core(W x, W& t, W& sr, W& cr)
 {
-    const float t = fmaf(x, 0.6366197466850281f, 12582912.0f);   // 1.5 * 2^23: the low mantissa bits hold rint(x * 2/pi)
+    using namespace lanes;
+    t = fma_(x, all<W>(0.6366197466850281f), all<W>(12582912.0f));
+    const W k = add_(t, all<W>(-12582912.0f));
+    W r = fma_(k, all<W>(-1.5707963705062866f), x);
+    r = fma_(k, all<W>(4.371138828673793e-08f), r);   // (a third term, 1.7e-15 k, is below fp32 resolution over the whole domain)
+    const W z = mul_(r, r);
+    W ps = fma_(z, all<W>(-0.00019513866573106498f), all<W>(0.00833214819431305f));
+    ps = fma_(z, ps, all<W>(-0.16666653752326965f));
+    sr = fma_(mul_(r, z), ps, r);
+    W pc = fma_(z, all<W>(2.438912088109646e-05f), all<W>(-0.0013886747183278203f));
+    pc = fma_(z, pc, all<W>(0.04166662320494652f));
+    pc = fma_(z, pc, all<W>(-0.5f));
+    cr = fma_(z, pc, all<W>(1.0f));
+}
+// quadrant k mod 4 = 0: (sr, cr), 1: (cr, -sr), 2: (-sr, -cr), 3: (-cr, sr): one sign word (bit 1 of k) on both, then the
+// odd quadrants swap and negate -- the negation rides on the select
+__device__ __forceinline__ void sincos_quadrant(float t, float sr, float cr, float& s, float& c)
+{
     const int q = __float_as_int(t);
-    const float k = t - 12582912.0f;
-    float r = fmaf(k, -1.5707963705062866f, x);
-    r = fmaf(k, 4.371138828673793e-08f, r);   // (a third term, 1.7e-15 k, is below fp32 resolution over the whole domain)
-    const float z = r * r;
-    float ps = fmaf(z, -0.00019513866573106498f, 0.00833214819431305f);
-    ps = fmaf(z, ps, -0.16666653752326965f);
-    const float sr = fmaf(r * z, ps, r);
-    float pc = fmaf(z, 2.438912088109646e-05f, -0.0013886747183278203f);
-    pc = fmaf(z, pc, 0.04166662320494652f);
-    pc = fmaf(z, pc, -0.5f);
-    const float cr = fmaf(z, pc, 1.0f);
-    // quadrant k mod 4 = 0: (sr, cr), 1: (cr, -sr), 2: (-sr, -cr), 3: (-cr, sr): one sign word (bit 1 of k) on both, then
-    // the odd quadrants swap and negate -- the negation rides on the select
     const int sgn = (q << 30) & 0x80000000;
     const float X = __int_as_float(__float_as_int(sr) ^ sgn), Y = __int_as_float(__float_as_int(cr) ^ sgn);
     const bool odd = q & 1;
     s = odd ? Y : X;
     c = odd ? -X : Y;
 }
+__device__ __forceinline__ void sincos_fast(float x, float& s, float& c)
+{
+    float t, sr, cr;
+    sincos_core<float>(x, t, sr, cr);
+    sincos_quadrant(t, sr, cr, s, c);
+}
+__device__ __forceinline__ void sincos_fast(float2 x, float2& s, float2& c)
+{
+    float2 t, sr, cr;
+    sincos_core<float2>(x, t, sr, cr);
+    sincos_quadrant(t.x, sr.x, cr.x, s.x, c.x);
+    sincos_quadrant(t.y, sr.y, cr.y, s.y, c.y);
+}
 
+// t = x / pi + 1.5 * 2^23; sr = sin(r), r = x - k pi in [-pi/2, pi/2]; sin x = (-1)^k sr
+template <typename W>
+__device__ __forceinline__ void sin_core(W x, W& t, W& sr)
+{
+    using namespace lanes;
+    t = fma_(x, all<W>(0.31830987334251404f), all<W>(12582912.0f));
+    const W k = add_(t, all<W>(-12582912.0f));
+    W r = fma_(k, all<W>(-3.1415927410125732f), x);
+    r = fma_(k, all<W>(8.742277657347586e-08f), r);
+    const W z = mul_(r, r);
+    W p = fma_(z, all<W>(-2.388586395341008e-08f), all<W>(2.752518867055187e-06f));
+    p = fma_(z, p, all<W>(-0.00019840864115394652f));
+    p = fma_(z, p, all<W>(0.008333330973982811f));
+    p = fma_(z, p, all<W>(-0.1666666716337204f));
+    sr = fma_(mul_(r, z), p, r);
+}
 __device__ __forceinline__ float sin_fast(float x)
 {
-    const float t = fmaf(x, 0.31830987334251404f, 12582912.0f);
-    const int q = __float_as_int(t);
-    const float k = t - 12582912.0f;
-    float r = fmaf(k, -3.1415927410125732f, x);
-    r = fmaf(k, 8.742277657347586e-08f, r);
-    const float z = r * r;
-    float p = fmaf(z, -2.388586395341008e-08f, 2.752518867055187e-06f);
-    p = fmaf(z, p, -0.00019840864115394652f);
-    p = fmaf(z, p, 0.008333330973982811f);
-    p = fmaf(z, p, -0.1666666716337204f);
-    const float sr = fmaf(r * z, p, r);
-    return __int_as_float(__float_as_int(sr) ^ (q << 31));
+    float t, sr;
+    sin_core<float>(x, t, sr);
+    return __int_as_float(__float_as_int(sr) ^ (__float_as_int(t) << 31));
+}
+__device__ __forceinline__ float2 sin_fast(float2 x)
+{
+    float2 t, sr;
+    sin_core<float2>(x, t, sr);
+    return make_float2(__int_as_float(__float_as_int(sr.x) ^ (__float_as_int(t.x) << 31)),
+                       __int_as_float(__float_as_int(sr.y) ^ (__float_as_int(t.y) << 31)));
 }
 
 // atan2 for the winding fast path (ahs_diag_march.cu): branch-free, absolute error <= 2.5e-7 rad in the fp32 emulation of
@@ -138,6 +187,40 @@ __device__ __forceinline__ double sin_fast(double x)
     const double base = odd ? fma(z, -0.5, 1.0) : r;
     const double mult = (odd ? z : r) * z;
     return trig64::flip(fma(mult, p, base), q);
+}
+
+// ---- V values at once (the V sites of a thread): fp32 goes through the packed two-lane form, fp64 one by one ------------
+template <int V>
+__device__ __forceinline__ void sincos_vec(const float (&x)[V], float (&s)[V], float (&c)[V])
+{
+    static_assert(V % 2 == 0, "pairs");
+#pragma unroll
+    for (int v = 0; v < V; v += 2) {
+        float2 s2, c2;
+        sincos_fast(make_float2(x[v], x[v + 1]), s2, c2);
+        s[v] = s2.x; s[v + 1] = s2.y; c[v] = c2.x; c[v + 1] = c2.y;
+    }
+}
+template <int V>
+__device__ __forceinline__ void sin_vec(const float (&x)[V], float (&y)[V])
+{
+#pragma unroll
+    for (int v = 0; v < V; v += 2) {
+        const float2 r = sin_fast(make_float2(x[v], x[v + 1]));
+        y[v] = r.x; y[v + 1] = r.y;
+    }
+}
+template <int V>
+__device__ __forceinline__ void sincos_vec(const double (&x)[V], double (&s)[V], double (&c)[V])
+{
+#pragma unroll
+    for (int v = 0; v < V; ++v) sincos_fast(x[v], s[v], c[v]);
+}
+template <int V>
+__device__ __forceinline__ void sin_vec(const double (&x)[V], double (&y)[V])
+{
+#pragma unroll
+    for (int v = 0; v < V; ++v) y[v] = sin_fast(x[v]);
 }
 
 }  // namespace ahs

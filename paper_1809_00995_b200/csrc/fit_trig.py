@@ -105,7 +105,7 @@ def main():
     print("sin(r)/r on [0, pi/2], even degree 10: max rel error %.2e" % e, c)
     # ---- the constants that are compiled in, emulated ------------------------------------------------------------------
     x = np.concatenate([rng.uniform(-20, 20, 2_000_000), rng.uniform(-1e3, 1e3, 200_000)]).astype(f32)
-    s, cc = emu_sincos(x, header_constants("void sincos_fast(float x"))
+    s, cc = emu_sincos(x, header_constants("void sincos_core(W x"))
     xs = x.astype(np.float64)
     print("sincos_fast fp32 emulation: max abs error sin %.2e cos %.2e" % (np.abs(s - np.sin(xs)).max(), np.abs(cc - np.cos(xs)).max()))
     ph = rng.uniform(-np.pi, np.pi, 4_000_000)

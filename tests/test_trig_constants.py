@@ -15,7 +15,7 @@ spec.loader.exec_module(fit_trig)
 def test_sincos_fast_fp32_constants():
     rng = np.random.default_rng(3)
     x = np.concatenate([rng.uniform(-20, 20, 400_000), rng.uniform(-1e3, 1e3, 100_000), [0.0, np.pi / 4, -np.pi / 4, 1e-8]]).astype(np.float32)
-    s, c = fit_trig.emu_sincos(x, fit_trig.header_constants("void sincos_fast(float x"))
+    s, c = fit_trig.emu_sincos(x, fit_trig.header_constants("void sincos_core(W x"))
     xs = x.astype(np.float64)
     assert np.abs(s - np.sin(xs)).max() < 1.2e-7 and np.abs(c - np.cos(xs)).max() < 1.2e-7
 
