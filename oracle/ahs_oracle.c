@@ -1,7 +1,7 @@
 /*
  * ahs_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
  *
- * Plain, slow, single-threaded fp64 CPU oracle for the hot path of arXiv 1809.00995
+ * Plain, slow fp64 CPU oracle for the hot path of arXiv 1809.00995
  * (Correia & Martins, "Abelian-Higgs Cosmic String Evolution with CUDA"): the damped
  * staggered-leapfrog update of (phi, Pi, A_i, E_i) and the network diagnostics
  * (plaquette winding, Lagrangian-weighted <v^2>, Gauss-law residual).
@@ -24,12 +24,36 @@
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): every function below is pinned by
  * something other than itself -- see the per-function "pinned by" notes and DESIGN.md.
  *
- * Build: gcc -O2 -ffp-contract=off -fPIC -shared -o libahs_oracle.so ahs_oracle.c -lm
+ * Threads.  The loops over sites are independent per site (the kicks read level-n phi, theta only and write
+ * the site's own Pi, eps), so their outer z loop carries an OpenMP "parallel for": the fields are bit-identical
+ * for any thread count.  Floating-point sums (diagnostics) are formed per z-plane in x-fastest order and the
+ * plane sums are added in z order, whatever the thread count, so every result is independent of it as well
+ * (pinned by test_oracle_is_independent_of_the_thread_count).  One thread unless aho_set_threads() says
+ * otherwise ("oracle, 1 core" and "oracle, all cores").
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -fPIC -shared -o libahs_oracle.so ahs_oracle.c -lm
  */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* number of threads the site loops use (default 1); returns the number actually in effect */
+static int aho_threads = 1;
+int32_t aho_set_threads(int32_t n)
+{
+#ifdef _OPENMP
+    if (n <= 0) n = omp_get_num_procs();
+    aho_threads = n;
+#else
+    (void)n;
+    aho_threads = 1;
+#endif
+    return aho_threads;
+}
 
 typedef struct {
     int32_t N;        /* lattice is N^3, periodic (any N >= 3)                                  */
@@ -138,6 +162,7 @@ void aho_ic(const aho_params* p, uint64_t seed, int32_t kind, double* f10)
     double* phi_re = f10;
     double* phi_im = f10 + V;
     uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t site = 0; site < V; ++site) aho_ic_site(p, key, site, kind, &phi_re[site], &phi_im[site]);
 }
 
@@ -242,6 +267,7 @@ static void aho_step_once(const aho_params* p, double* f10, int64_t n)
     const double c1 = c[0], c2 = c[1], c3 = c[2], d1 = c[3], d2 = c[4], d3 = c[5];
     const double sig2 = p->sigma * p->sigma;
 
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
@@ -291,6 +317,7 @@ static void aho_step_once(const aho_params* p, double* f10, int64_t n)
         eps[0][s0] = new_eps[0]; eps[1][s0] = new_eps[1]; eps[2][s0] = new_eps[2];
     }
     /* --- Eqs. 6-7: drift -------------------------------------------------------------------- */
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t s0 = 0; s0 < V; ++s0) {
         phr[s0]  += p->dt * pir[s0];
         phi_[s0] += p->dt * pii[s0];
@@ -329,7 +356,9 @@ void aho_winding(const aho_params* p, const double* f10, int32_t* W3, uint64_t* 
     const double* th[3] = { f10 + 4 * V, f10 + 5 * V, f10 + 6 * V };
     double* arg = (double*)malloc((size_t)V * sizeof(double));
     int32_t* nl = (int32_t*)malloc((size_t)(3 * V) * sizeof(int32_t));
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t s0 = 0; s0 < V; ++s0) arg[s0] = atan2(phi_[s0], phr[s0]);
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
@@ -344,6 +373,7 @@ void aho_winding(const aho_params* p, const double* f10, int32_t* W3, uint64_t* 
     uint64_t cnt = 0, tot = 0;
     for (int pl = 0; pl < 3; ++pl) {
         const int i = PI_[pl], j = PJ_[pl];
+#pragma omp parallel for num_threads(aho_threads) schedule(static) reduction(+ : cnt, tot)   /* integer sums: any order */
         for (int64_t z = 0; z < N; ++z)
         for (int64_t y = 0; y < N; ++y)
         for (int64_t x = 0; x < N; ++x) {
@@ -417,7 +447,7 @@ static void aho_site_lagrangian(const aho_params* p, const double* f10, double a
  *          string tension at lambda = 2 e^2 (the paper's couplings, L72) -- a labelled assumption (R20)
  *   Gauss residual (L72, L181; derived from Eqs. 4-7, R4), a_h = a(tau_n - dt/2):
  *     g^x = sum_i (eps_i^x - eps_i^{x-k_i}) - 2 q dx^2 e0^2 a_h^(2s) Im[conj(phi^x) Pi^x]
- * Sums are accumulated in fp64 in plain x-fastest order.
+ * Sums are accumulated in fp64: x-fastest within a z-plane, then the plane sums in z order.
  * pinned by: gauge invariance of W, <v^2>, g (P11); Gauss at roundoff after k steps for several
  * (m,s) (P1) -- the residual uses only this function's formula and the step's output, a dropped
  * factor or wrong a-level in either shows up as an O(1) residual; independent numpy evaluation of
@@ -445,25 +475,38 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
     const double a = aho_a(p, tau);
     const double ah = aho_a(p, tau - 0.5 * p->dt);
     const double grhs = 2.0 * q * p->dx * p->dx * p->e0 * p->e0 * pow(ah, 2.0 * p->s);
-    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
-    for (int64_t z = 0; z < N; ++z)
-    for (int64_t y = 0; y < N; ++y)
-    for (int64_t x = 0; x < N; ++x) {
-        const int64_t s0 = x + N * (y + N * z);
-        double kgl[4];
-        aho_site_lagrangian(p, f10, a, x, y, z, kgl);
-        num  += kgl[0] * kgl[2];
-        den  += kgl[1] * kgl[2];
-        lsum += kgl[2];
-        vnum += kgl[0] * kgl[3];
-        vden += kgl[1] * kgl[3];
-        double div = 0.0;
-        for (int i = 0; i < 3; ++i) div += eps[i][s0] - eps[i][aho_nb(N, x, y, z, i, -1)];
-        const double rhs = grhs * (phr[s0] * pii[s0] - phi_[s0] * pir[s0]);
-        const double g = fabs(div - rhs);
-        if (g > gmax || g != g) gmax = g;
-        rhs2 += rhs * rhs;
+    /* per z-plane sums in x-fastest order (planes are independent), then the planes added in z order */
+    double* plane = (double*)malloc((size_t)N * 7 * sizeof(double));
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
+    for (int64_t z = 0; z < N; ++z) {
+        double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+        for (int64_t y = 0; y < N; ++y)
+        for (int64_t x = 0; x < N; ++x) {
+            const int64_t s0 = x + N * (y + N * z);
+            double kgl[4];
+            aho_site_lagrangian(p, f10, a, x, y, z, kgl);
+            num  += kgl[0] * kgl[2];
+            den  += kgl[1] * kgl[2];
+            lsum += kgl[2];
+            vnum += kgl[0] * kgl[3];
+            vden += kgl[1] * kgl[3];
+            double div = 0.0;
+            for (int i = 0; i < 3; ++i) div += eps[i][s0] - eps[i][aho_nb(N, x, y, z, i, -1)];
+            const double rhs = grhs * (phr[s0] * pii[s0] - phi_[s0] * pir[s0]);
+            const double g = fabs(div - rhs);
+            if (g > gmax || g != g) gmax = g;
+            rhs2 += rhs * rhs;
+        }
+        double* o = plane + 7 * z;
+        o[0] = num; o[1] = den; o[2] = lsum; o[3] = gmax; o[4] = rhs2; o[5] = vnum; o[6] = vden;
     }
+    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+    for (int64_t z = 0; z < N; ++z) {
+        const double* o = plane + 7 * z;
+        num += o[0]; den += o[1]; lsum += o[2]; rhs2 += o[4]; vnum += o[5]; vden += o[6];
+        if (o[3] > gmax || o[3] != o[3]) gmax = o[3];
+    }
+    free(plane);
     out->v2_num = num;
     out->v2_den = den;
     {
@@ -487,6 +530,7 @@ void aho_site_fields4(const aho_params* p, const double* f10, int64_t n, double*
 {
     const int64_t N = p->N;
     const double a = aho_a(p, aho_tau(p, n));
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {

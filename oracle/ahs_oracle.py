@@ -2,7 +2,7 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this module.  It imports nothing from paper_1809_00995_b200 and the CUDA path imports nothing from
-here.  All arithmetic of the method lives in ahs_oracle.c (fp64, single-threaded); this file only
+here.  All arithmetic of the method lives in ahs_oracle.c (fp64; one thread unless set_threads); this file only
 builds the shared object with gcc, marshals numpy arrays and mirrors the two C structs.
 
 Field container ("f10"): float64 array of shape (10, N, N, N), C-contiguous, index [field, z, y, x]
@@ -27,11 +27,13 @@ IC_RANDOM_PHASE, IC_GAUSSIAN = 0, 1
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (no fast-math, no FMA contraction)."""
+    """Compile the oracle with gcc (no fast-math, no FMA contraction).  -fopenmp only marks the independent site loops
+    parallel (results do not depend on the thread count); without libgomp the pragmas are ignored: one thread."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c11",
-                               "-D_GNU_SOURCE", "-o", tmp, _SRC, "-lm"])
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c11", "-D_GNU_SOURCE", "-o", tmp, _SRC, "-lm"]
+        if subprocess.call(cmd[:1] + ["-fopenmp"] + cmd[1:], stderr=subprocess.DEVNULL) != 0:
+            subprocess.check_call(cmd)
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -93,9 +95,17 @@ def lib():
         for f in ("aho_philox4x32_10", "aho_ic", "aho_ic_window", "aho_coeffs", "aho_step", "aho_winding",
                   "aho_diag_compute", "aho_site_fields", "aho_site_fields4"):
             getattr(_lib, f).restype = None
+        _lib.aho_set_threads.argtypes = [C.c_int32]
+        _lib.aho_set_threads.restype = C.c_int32
         assert _lib.aho_sizeof_params() == C.sizeof(_Params)
         assert _lib.aho_sizeof_diag() == C.sizeof(_Diag)
     return _lib
+
+
+def set_threads(n: int = 0) -> int:
+    """Threads for the site loops (0 = all cores online; default at load time: 1).  Results do not depend on it.
+    Returns the count in effect (1 if the library was built without OpenMP)."""
+    return int(lib().aho_set_threads(int(n)))
 
 
 def _dptr(a: np.ndarray):

@@ -796,3 +796,34 @@ def test_potential_weighted_estimator_and_xi_L(oracle):
     d1, d2 = oracle.diagnostics(pg, g, 3), oracle.diagnostics(pg, g2, 3)
     for key in ("v2v_num", "v2v_den", "v2_V", "xi_L"):
         assert d1[key] == pytest.approx(d2[key], rel=1e-11, nan_ok=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# threads: the site loops are independent per site, the sums are per-plane in a fixed order
+# ---------------------------------------------------------------------------------------------------------
+def test_oracle_is_independent_of_the_thread_count(oracle):
+    """BASELINE.md section 3 ("oracle, all cores"): the OpenMP marking of the z loops must not change a single bit --
+    fields, integer counts and every fp64 sum (formed per z-plane, planes added in z order for any thread count)."""
+    from paper_1809_00995_b200 import synthetic
+    p = oracle.Params(N=20, m=2.0, s=0.5, tau0=2.0)
+    f0 = synthetic.random_snapshot(20, seed=3)
+    out = []
+    try:
+        for n in (1, 3, 0):
+            used = oracle.set_threads(n)
+            assert used >= 1
+            f = oracle.step(p, f0.copy(), 4, 3)
+            ic = oracle.initial_condition(p, 99, oracle.IC_GAUSSIAN)
+            out.append((f, ic, oracle.diagnostics(p, f, 7), oracle.winding(p, f), oracle.site_fields4(p, f, 7)))
+    finally:
+        oracle.set_threads(1)
+    for f, ic, d, w, sf in out[1:]:
+        assert np.array_equal(f, out[0][0]) and np.array_equal(ic, out[0][1])
+        assert w == out[0][3] and all(np.array_equal(d[k], out[0][2][k], equal_nan=True) for k in d)
+        assert all(np.array_equal(a, b) for a, b in zip(sf, out[0][4]))
+    # the per-plane order is a rounding-order change only: against a plain numpy sum of the per-site products
+    K, G, Lg, Vp = out[0][4]
+    d = out[0][2]
+    assert d["v2_num"] == pytest.approx(float((K * Lg).sum()), rel=1e-12)
+    assert d["v2_den"] == pytest.approx(float((G * Lg).sum()), rel=1e-12)
+    assert d["mean_lagrangian"] == pytest.approx(float(Lg.mean()), rel=1e-12)
