@@ -1,14 +1,20 @@
 """Parity of the CUDA path (through the C ABI) with the fp64 CPU oracle, element by element on the same
 seeded inputs.  Needs a B200: run with -m gpu.
 
-Tolerances (BASELINE.json north_star; definitions DESIGN.md "Tolerances"):
-  fp64 fields after 20 steps : max_x |gpu - oracle| / max(1, max_x |oracle|) <= 1e-12 per field array
-  fp32 fields after 20 steps : max_x |gpu - oracle| / max(1, max_x |oracle|) <= 2e-4 per field array
+Tolerances (BASELINE.json north_star; definitions DESIGN.md "Tolerances"), per field array, BOTH norms asserted:
+  fp64 fields after 20 steps : strict  max_x |gpu - oracle| / max_x |oracle| <= 1e-12
+                               R14     max_x |gpu - oracle| / max(1, max_x |oracle|) <= 1e-12
+  fp32 fields after 20 steps : strict  max_x |gpu - oracle| <= 2e-4                          (north_star, absolute)
+                               R14     max_x |gpu - oracle| / max(1, max_x |oracle|) <= 2e-4
+  (the one exception to the strict fp32 bound is config 3's physics, s = 1 in the matter era, where eps grows to ~30 in
+   20 steps and 2e-4 absolute is below fp32 resolution of the field itself: SURVEY 8(c) "Config consequences of G3")
   winding                    : bit-exact on identical snapshots (produced by the oracle, uploaded with ahs_set_fields)
   <v^2> sums                 : fp64 1e-10 relative, fp32 2e-5 relative to sum |K Lag|, sum |G Lag|
   Gauss residual             : at roundoff of the storage type on both paths
 """
+import json
 import math
+import os
 
 import numpy as np
 import pytest
@@ -16,6 +22,24 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-12, "f32": 2e-4}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def oracle_on_all_cores(oracle):
+    """The oracle's results do not depend on its thread count (test_oracle_is_independent_of_the_thread_count)."""
+    oracle.set_threads(0)
+    yield
+    oracle.set_threads(1)
+
+
+def record(test, **kw):
+    """Observed maxima: printed (pytest -s) and, if AHS_PARITY_LOG names a file, appended to it as JSON lines."""
+    line = json.dumps(dict(test=test, **kw))
+    print(line)
+    path = os.environ.get("AHS_PARITY_LOG")
+    if path:
+        with open(path, "a") as f:
+            f.write(line + "\n")
 
 
 @pytest.fixture(scope="module")
@@ -28,7 +52,28 @@ def ahs():
 
 
 def field_errors(got, ref):
+    """R14 norm per field array: max |d| / max(1, max |oracle|)."""
     return [np.abs(got[k] - ref[k]).max() / max(1.0, np.abs(ref[k]).max()) for k in range(10)]
+
+
+def strict_errors(got, ref, prec):
+    """north_star's norms as stated: fp64 max |d| / max |oracle| (relative), fp32 max |d| (absolute)."""
+    out = []
+    for k in range(10):
+        d, m = np.abs(got[k] - ref[k]).max(), np.abs(ref[k]).max()
+        out.append(d if prec == "f32" else (d / m if m > 0 else (0.0 if d == 0 else np.inf)))
+    return out
+
+
+def assert_fields(test, got, ref, prec, names, strict=True, tol=None, **ctx):
+    tol = TOL[prec] if tol is None else tol
+    r14, st = field_errors(got, ref), strict_errors(got, ref, prec)
+    record(test, prec=prec, strict_asserted=strict, max_r14=max(r14), max_strict=max(st),
+           strict_per_field={n: float("%.3g" % e) for n, e in zip(names, st)}, **ctx)
+    for k in range(10):
+        assert r14[k] <= tol, (names[k], "R14", r14[k], ctx)
+        if strict:
+            assert st[k] <= tol, (names[k], "strict", st[k], ctx)
 
 
 def oracle_params(O, sim):
@@ -103,16 +148,21 @@ CASES = [
     (20, "f64", 2.0, 0.5, "generic"),     # ragged: N not a multiple of the block size, several blocks
     (36, "f32", 2.0, 0.0, "generic"),
     (64, "f64", 1.0, 1.0, "auto"),
-    (128, "f32", 1.0, 0.0, "auto"),       # config 2 / 4 physics at an oracle-sized lattice
+    (128, "f32", 1.0, 0.0, "auto"),       # config 2 / 4 physics, one fp32 tile wide (row-copy staging)
     (128, "f32", 2.0, 1.0, "auto"),       # config 3 physics (matter, s=1), 20 steps are inside the stable window
     (192, "f64", 1.0, 0.0, "auto"),       # three fp64 tiles in x: left-edge, interior and right-edge tiles of the TMA path
+    (128, "f64", 1.0, 1.0, "auto"),       # config 5 physics, two fp64 tiles in x
+    (256, "f32", 1.0, 0.0, "auto"),       # two fp32 tiles in x: left- and right-edge tiles of the TMA path, z-chunks of 16
+    (384, "f32", 1.0, 0.0, "auto"),       # three fp32 tiles in x: left-edge, interior and right-edge TMA tiles
 ]
+# strict fp32 bound not applicable (see the module docstring): eps ~ 30 after 20 steps
+STRICT_EXEMPT = {(128, "f32", 2.0, 1.0)}
 
 
 @pytest.mark.parametrize("N,prec,m,s,kernel", CASES)
 def test_fields_after_20_steps(ahs, oracle, N, prec, m, s, kernel):
     from paper_1809_00995_b200 import synthetic
-    nsteps = 20 if N <= 64 else (6 if N <= 128 else 3)        # the oracle needs ~1 us per site-update
+    nsteps = 20                           # north_star's 20 steps; the oracle (all cores) needs ~0.05 us per site-update
     with ahs.Simulation(N=N, precision=prec, m=m, s=s, ic="none", kernel=kernel) as sim:
         p = oracle_params(oracle, sim)
         ref = rounded(oracle.initial_condition(p, synthetic.SEED_PRIMARY), prec)   # the oracle's IC, uploaded
@@ -121,9 +171,8 @@ def test_fields_after_20_steps(ahs, oracle, N, prec, m, s, kernel):
         got = sim.get_fields()
         assert sim.step_count == nsteps
         oracle.step(p, ref, 0, nsteps)
-        errs = field_errors(got, ref)
-        for k, e in enumerate(errs):
-            assert e <= TOL[prec], (oracle.FIELD_NAMES[k], e)
+        assert_fields("fields_after_20_steps", got, ref, prec, oracle.FIELD_NAMES, strict=(N, prec, m, s) not in STRICT_EXEMPT,
+                      N=N, m=m, s=s, kernel=sim.kernel_kind, nsteps=nsteps)
         # Gauss's law on the device trajectory itself
         d = sim.diagnostics()
         assert d["gauss_max"] <= (1e-12 if prec == "f64" else 2e-5) * max(1.0, d["gauss_rhs_rms"])
@@ -146,8 +195,8 @@ def test_step_from_generic_snapshot(ahs, oracle, N, prec, kernel):
         sim.step(nsteps)
         got = sim.get_fields()
         ref = oracle.step(p, f0.copy(), 7, nsteps)
-        for k, e in enumerate(field_errors(got, ref)):
-            assert e <= (1e-13 if prec == "f64" else 2e-5), (oracle.FIELD_NAMES[k], e)
+        assert_fields("step_from_generic_snapshot", got, ref, prec, oracle.FIELD_NAMES, tol=1e-13 if prec == "f64" else 2e-5,
+                      N=N, kernel=sim.kernel_kind, nsteps=nsteps)
         check_diag(oracle, p, sim, prec, ref, 7 + nsteps)
 
 
@@ -272,26 +321,45 @@ def test_gauge_transformation_leaves_diagnostics_unchanged(ahs, oracle, prec, N)
             assert d1["v2"] == pytest.approx(d0["v2"], rel=2e-3)
 
 
-def test_long_run_series_fp32_vs_oracle(ahs, oracle):
-    """north_star: long-run xi(tau) and <v^2> agree within 2 % (fp32 GPU vs fp64 oracle, config-2 physics, 48^3... here
-    at a size the oracle finishes in seconds; the 2 % criterion is applied to <v^2> where |den| is well away from 0)."""
-    N, nsteps, every = 48, 160, 20
-    with ahs.Simulation(N=N, precision="f32", ic="none", m=1.0, s=0.0, kernel="generic") as sim:
+@pytest.mark.parametrize("N,prec,kernel", [(48, "f32", "generic"), (128, "f32", "auto"), (128, "f64", "auto")])
+def test_long_run_series_vs_oracle(ahs, oracle, N, prec, kernel):
+    """north_star: long-run xi(tau) and <v^2> agree within 2 % (GPU trajectory vs the fp64 oracle's own trajectory from the
+    same initial condition, config-2 physics: radiation era, s = 0), to tau = 33, diagnostics every 20 steps.  The 128^3 cases run
+    the z-marching kernels (kernel="auto"), i.e. the kernels bench.py times.  <v^2>_L is a ratio with a sign-indefinite
+    weight (R16): the 2 % criterion is applied to it where |den| is well away from 0, and to <v^2>_V always."""
+    nsteps, every = 320, 20
+    with ahs.Simulation(N=N, precision=prec, ic="none", m=1.0, s=0.0, kernel=kernel) as sim:
+        if kernel == "auto":
+            assert sim.kernel_kind == "march"
         p = oracle_params(oracle, sim)
-        ref = rounded(oracle.initial_condition(p, 11), "f32")
+        ref = rounded(oracle.initial_condition(p, 11), prec)
         sim.set_fields(ref, 0)
+        series = []
         for n in range(every, nsteps + 1, every):
             sim.step(every)
             oracle.step(p, ref, n - every, every)
             d = sim.diagnostics()
             r = oracle.diagnostics(p, ref, n)
-            assert d["xi"] == pytest.approx(r["xi"], rel=0.02)
-            assert abs(int(d["n_pierced"]) - int(r["n_pierced"])) <= 0.02 * r["n_pierced"]
             K, G, Lg = oracle.site_fields(p, ref, n)
-            if abs(r["v2_den"]) > 0.05 * np.abs(G * Lg).sum():
-                assert d["v2"] == pytest.approx(r["v2"], rel=0.02)
-            assert d["gauss_max"] < 5e-5 * max(1.0, d["gauss_rhs_rms"])
-        assert max(field_errors(sim.get_fields(), ref)) < 5e-3
+            den_ok = abs(r["v2_den"]) > 0.05 * np.abs(G * Lg).sum()
+            series.append(dict(n=n, xi=(d["xi"], r["xi"]), n_pierced=(d["n_pierced"], r["n_pierced"]), v2_V=(d["v2_V"], r["v2_V"]),
+                               v2_L=(d["v2"], r["v2"]), den_ok=bool(den_ok), gauss=d["gauss_max"]))
+            assert d["xi"] == pytest.approx(r["xi"], rel=0.02), series
+            assert abs(int(d["n_pierced"]) - int(r["n_pierced"])) <= 0.02 * r["n_pierced"], series
+            assert d["v2_V"] == pytest.approx(r["v2_V"], rel=0.02), series
+            if den_ok:
+                assert d["v2"] == pytest.approx(r["v2"], rel=0.02), series
+            assert d["gauss_max"] < (5e-5 if prec == "f32" else 1e-12) * max(1.0, d["gauss_rhs_rms"]), series
+        got = sim.get_fields()
+        err = field_errors(got, ref)
+        rel = lambda a, b: abs(a - b) / abs(b)
+        record("long_run_series", N=N, prec=prec, kernel=sim.kernel_kind, nsteps=nsteps, max_field_err_r14=max(err),
+               max_dphi=float(np.abs(got[:2] - ref[:2]).max()),
+               max_rel_xi=max(rel(*x["xi"]) for x in series), max_rel_v2_V=max(rel(*x["v2_V"]) for x in series),
+               max_rel_v2_L_where_den_ok=max([rel(*x["v2_L"]) for x in series if x["den_ok"]] or [0.0]),
+               n_pierced_equal_at=sum(x["n_pierced"][0] == x["n_pierced"][1] for x in series), calls=len(series))
+        # SURVEY 8(d)(4): no chaotic divergence -- fp32 arithmetic drifts from fp64 by ~1e-4 in phi over 160-320 steps
+        assert max(err) < (5e-3 if prec == "f32" else 1e-10), err
 
 
 def test_native_transfer_and_device_pointers(ahs):
@@ -381,13 +449,16 @@ def _gather_window(sim, origin, B):
 
 
 def test_full_size_1024_sampled_windows_and_closed_forms(ahs, oracle):
-    """configs[3] at full size.  (1) Sampled outputs: the oracle generates the initial condition of small windows of the
-    1024^3 lattice from the Philox specification (aho_ic_window), steps each window as a periodic 22^3 lattice and is
-    compared on the 16^3 interior the wrong wrap cannot have reached after 3 steps -- windows sit on tile corners, on
-    z-chunk boundaries of the march and on the periodic corner of the lattice.  (2) Properties that hold at any size:
-    closed forms of the diagnostics on the random-phase initial condition, Gauss's law at fp32 roundoff after stepping."""
+    """configs[3] at full size, north_star's 20 steps, in the launch configuration bench.py times.  (1) Sampled outputs:
+    the oracle generates the initial condition of small windows of the 1024^3 lattice from the Philox specification
+    (aho_ic_window), steps each window 20 times as a periodic 56^3 lattice and is compared on the 16^3 interior that the
+    wrong wrap cannot have reached (one site per step, halo 20) -- interiors sit on tile corners of the march (x multiple
+    of 128, y multiple of 4), on its z-chunk boundaries (z multiple of 64) and on the periodic corner of the lattice, so
+    interior, left-edge and right-edge TMA tiles and the y-edge row-copy tiles are all sampled.  Strict norm: max |d| <= 2e-4.
+    (2) Properties that hold at any size: closed forms of the diagnostics on the random-phase initial condition, Gauss's
+    law at fp32 roundoff after stepping."""
     import torch
-    N, nsteps, halo, inner = 1024, 3, 3, 16
+    N, nsteps, halo, inner = 1024, 20, 20, 16
     free, _ = torch.cuda.mem_get_info()
     if free < ahs.required_bytes(N, "f32") + (2 << 30):
         pytest.skip("needs %.0f GB of free device memory" % (ahs.required_bytes(N, "f32") / 1e9))
@@ -404,17 +475,25 @@ def test_full_size_1024_sampled_windows_and_closed_forms(ahs, oracle):
         assert d0["v2_den"] / sites == pytest.approx(-672.0, rel=2e-3)
         sim.step(nsteps)
         rng = np.random.default_rng(5)
-        origins = [(-11, -11, -11), (128 - 11, 4 - 11, 64 - 11), (512 - 5, 700 - 2, 128 - 9), (1024 - 128 - 8, 1024 - 4 - 9, 960 - 3)]
-        origins += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(4)]
+        # first site of each compared 16^3 interior
+        interiors = [(-8, -8, -8), (128 - 8, 4 - 8, 64 - 8), (512 - 2, 700 + 1, 128 - 6), (1024 - 128 - 5, 1024 - 4 - 6, 960),
+                     (896 - 8, 512 - 8, 1024 - 64 - 8), (-8, 300, 448 - 8)]
+        interiors += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(4)]
         pw = oracle.Params(N=B, m=1.0, s=0.0)
         sl = slice(halo, halo + inner)
-        for origin in origins:
+        worst = np.zeros(10)
+        for io in interiors:
+            origin = tuple(v - halo for v in io)
             ref = rounded(oracle.initial_condition_window(pw, seed, N, origin), "f32")
             oracle.step(pw, ref, 0, nsteps)
             got = _gather_window(sim, origin, B)
             for k in range(10):
-                err = np.abs(got[k][sl, sl, sl] - ref[k][sl, sl, sl]).max() / max(1.0, np.abs(ref[k][sl, sl, sl]).max())
-                assert err <= TOL["f32"], (origin, oracle.FIELD_NAMES[k], err)
+                d = np.abs(got[k][sl, sl, sl] - ref[k][sl, sl, sl]).max()
+                worst[k] = max(worst[k], d)
+                assert d <= TOL["f32"], (io, oracle.FIELD_NAMES[k], d)                                          # strict: absolute
+                assert d / max(1.0, np.abs(ref[k][sl, sl, sl]).max()) <= TOL["f32"], (io, oracle.FIELD_NAMES[k], d)   # R14
+        record("full_size_1024_windows", nsteps=nsteps, windows=len(interiors), inner=inner, halo=halo, max_strict=float(worst.max()),
+               strict_per_field={n: float("%.3g" % e) for n, e in zip(oracle.FIELD_NAMES, worst)})
         d = sim.diagnostics()
         assert d["nonfinite"] == 0 and d["step"] == nsteps
         assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"])
