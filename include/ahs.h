@@ -27,6 +27,10 @@
  * ahs_step is asynchronous, every function that returns data to the host synchronises that stream.
  * A handle is not thread-safe; distinct handles are independent (replicas).
  *
+ * Devices.  A handle belongs to the device that was current when it was created (a caller-supplied device_buffer must
+ * live there).  Every later call makes that device current for its own duration and restores the caller's, so one host
+ * thread can drive handles on several GPUs without calling cudaSetDevice itself.
+ *
  * Errors.  Functions returning int return AHS_OK (0) or a negative code; ahs_last_error() returns a
  * thread-local, statically stored, human readable message for the last failure on the calling thread.
  * There is no CPU fallback and no other backend: without a CUDA device every call that needs one fails
@@ -54,11 +58,15 @@ enum { AHS_OK = 0, AHS_ERR_INVALID_ARG = -1, AHS_ERR_OOM = -2, AHS_ERR_CUDA = -3
 enum { AHS_F32 = 0, AHS_F64 = 1 };                                   /* storage AND arithmetic type of the step */
 enum { AHS_IC_RANDOM_PHASE = 0, AHS_IC_GAUSSIAN = 1, AHS_IC_NONE = 2 /* all fields zero; set them with ahs_set_fields */ };
 enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
+enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2 };   /* ahs_set_option */
+enum { AHS_STAGING_TENSOR = 0, AHS_STAGING_ROWS = 1 };
 
 /*
  * Parameters of a simulation (L36: lambda, e, sigma; L51: dx, dt; L68-70: s; L224: a ~ eta^m; L72: IC).
- *   N               lattice is N^3, periodic.  N >= 4 (ahs_create_ex); the z-marching kernel needs N % 128 == 0
- *                   (fp32) or N % 64 == 0 (fp64) and is chosen automatically when it applies.
+ *   N               lattice is N^3, periodic, 4 <= N <= 2048.  The z-marching kernels (TMA-staged tiles, the ones that run near
+ *                   the HBM roofline) need N % 128 == 0 (fp32) or N % 64 == 0 (fp64) and are chosen automatically when that
+ *                   holds.  Any other N runs on the one-thread-per-site kernels, which are about 6 x slower on the step and
+ *                   8 x slower on the diagnostics (profiles/r1_launches_1024.md); ahs_kernel_kind tells which one a handle uses.
  *   dx, dt          lattice spacing and conformal time step, > 0.
  *   lambda, e, sigma  lambda_0, e_0 of Eq. 8 and the vacuum expectation value, > 0.
  *   m               a(tau) = (tau/tau_ref)^m : 0 static, 1 radiation, 2 matter.
@@ -104,7 +112,8 @@ typedef struct {
     double gauss_max;         /* max_x |sum_i (eps_i^x - eps_i^{x-k_i}) - 2 dx^2 e0^2 a_h^(2s) Im[conj(phi) Pi]|,
                                  a_h = a(tau_n - dt/2)  (R4)                                               */
     double gauss_rhs_rms;     /* rms_x of the second term: the scale gauss_max is to be compared with      */
-    int32_t nonfinite;        /* 1 if any stored field value is NaN or +-inf                               */
+    int32_t nonfinite;        /* 1 if any stored field value is NaN or +-inf (finite values whose products
+                                 overflow the storage type make the sums non-finite but do not set this)   */
     int32_t reserved;
     double v2v_num;           /* sum_x |Pi|^2 Vp^x, Vp = (a^2 lambda(a)/4)(|phi|^2 - sigma^2)^2: Eq. 10 with the
                                  potential as the weight (L86, "two different weight functions")             */
@@ -163,6 +172,16 @@ AHS_API int32_t ahs_get_state(ahs_sim* sim, int64_t* step, double* tau, int64_t*
 
 /* Which implementation the handle uses: AHS_KERNEL_GENERIC or AHS_KERNEL_MARCH. */
 AHS_API int32_t ahs_kernel_kind(ahs_sim* sim);
+
+/* Tuning of the z-marching kernels (no effect on the one-thread-per-site kernels, none on any result beyond rounding order
+ * of the fp64 reduction, which follows the launch shape).  Takes effect at the next launch.
+ *   AHS_OPT_STAGING      AHS_STAGING_TENSOR (default): halo'd tiles of the level-n fields (Eq. 4-5's phi, theta) are staged in
+ *                        shared memory by tensor-map TMA copies wherever a tile does not straddle the periodic boundary in y;
+ *                        AHS_STAGING_ROWS: by one bulk copy per tile row everywhere (the path tiles on that boundary always take).
+ *   AHS_OPT_STEP_CHUNKS  number of z-chunks each (x, y) tile of the step march is cut into, 1..N (0 = the library's choice);
+ *   AHS_OPT_DIAG_CHUNKS  the same for the diagnostics march.  Chunks need not divide N.
+ * Returns AHS_ERR_INVALID_ARG for an unknown option or a value out of range. */
+AHS_API int32_t ahs_set_option(ahs_sim* sim, int32_t option, int32_t value);
 
 /* The six coefficients (c1, c2, c3, d1, d2, d3) of Eqs. 4-5 for the step n -> n+1, as the host computes
  * them. out6: HOST. */

@@ -18,6 +18,8 @@ AHS_OK, AHS_ERR_INVALID_ARG, AHS_ERR_OOM, AHS_ERR_CUDA, AHS_ERR_NONFINITE, AHS_E
 AHS_F32, AHS_F64 = 0, 1
 AHS_IC_RANDOM_PHASE, AHS_IC_GAUSSIAN, AHS_IC_NONE = 0, 1, 2
 AHS_KERNEL_AUTO, AHS_KERNEL_GENERIC, AHS_KERNEL_MARCH = 0, 1, 2
+AHS_OPT_STAGING, AHS_OPT_STEP_CHUNKS, AHS_OPT_DIAG_CHUNKS = 0, 1, 2
+AHS_STAGING_TENSOR, AHS_STAGING_ROWS = 0, 1
 
 FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "theta_0", "theta_1", "theta_2", "eps_0", "eps_1", "eps_2")
 
@@ -25,7 +27,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "theta_0", "theta_1", "thet
 SYMBOLS = (
     "ahs_required_bytes", "ahs_create", "ahs_create_ex", "ahs_step", "ahs_diagnostics", "ahs_diagnostics_ex",
     "ahs_diagnostics_launch", "ahs_diagnostics_fetch", "ahs_get_fields", "ahs_set_fields", "ahs_get_fields_native",
-    "ahs_set_fields_native", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_coefficients",
+    "ahs_set_fields_native", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_coefficients",
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
 )
 
@@ -78,6 +80,7 @@ def load(path: str | None = None):
     lib.ahs_field_device_ptr.argtypes = [vp, i32, C.POINTER(vp)]; lib.ahs_field_device_ptr.restype = i32
     lib.ahs_get_state.argtypes = [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64)]; lib.ahs_get_state.restype = i32
     lib.ahs_kernel_kind.argtypes = [vp]; lib.ahs_kernel_kind.restype = i32
+    lib.ahs_set_option.argtypes = [vp, i32, i32]; lib.ahs_set_option.restype = i32
     lib.ahs_coefficients.argtypes = [vp, i64, C.POINTER(dbl)]; lib.ahs_coefficients.restype = i32
     lib.ahs_synchronize.argtypes = [vp]; lib.ahs_synchronize.restype = i32
     lib.ahs_destroy.argtypes = [vp]; lib.ahs_destroy.restype = i32
@@ -245,6 +248,9 @@ class Simulation:
     @property
     def kernel_kind(self) -> str:
         return {AHS_KERNEL_GENERIC: "generic", AHS_KERNEL_MARCH: "march"}[load().ahs_kernel_kind(self._h)]
+
+    def set_option(self, option: int, value: int):
+        _check(load().ahs_set_option(self._h, int(option), int(value)))
 
     def coefficients(self, n: int) -> np.ndarray:
         out = (C.c_double * 6)()

@@ -32,6 +32,7 @@ struct ahs_sim {
     bool diag_map_ok;
     StepMaps step_maps[2];     // the same for the step march (buffer 0 / 1 as the level-n input)
     bool step_maps_ok;
+    MarchOptions opt;          // ahs_set_option
 };
 
 namespace {
@@ -133,7 +134,7 @@ int do_step(ahs_sim* s)
     }
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
     const StepCoef c = step_coefficients(s->p, s->step);
-    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->step_maps_ok ? &s->step_maps[s->cur] : nullptr, s->stream)
+    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->step_maps_ok ? &s->step_maps[s->cur] : nullptr, s->opt, s->stream)
                                          : launch_step_generic<T>(f, s->p.N, c, s->stream);
 }
 
@@ -149,7 +150,7 @@ int do_diag(ahs_sim* s)
     return s->kernel == AHS_KERNEL_MARCH
                ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result,
                                       slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1), 5 * s->array_bytes,
-                                      s->diag_map_ok ? &s->diag_map[s->cur] : nullptr, s->stream)   // shadow buffer: dead between steps
+                                      s->diag_map_ok ? &s->diag_map[s->cur] : nullptr, s->opt, s->stream)   // shadow buffer: dead between steps
                : launch_diag_generic<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream);
 }
 
@@ -158,6 +159,31 @@ int check_sim(const ahs_sim* s)
     if (!s) return fail(AHS_ERR_INVALID_ARG, "null handle");
     return AHS_OK;
 }
+
+// Every entry point runs on the handle's device whatever the caller's current device is, and puts the caller's device
+// back on return: one host thread may drive handles on several GPUs (replicas).
+class DeviceGuard {
+public:
+    explicit DeviceGuard(int device) : prev_(-1), ok_(true)
+    {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) { ok_ = false; return; }
+        if (cur != device) {
+            if (cudaSetDevice(device) != cudaSuccess) { ok_ = false; return; }
+            prev_ = cur;
+        }
+    }
+    ~DeviceGuard() { if (prev_ >= 0) cudaSetDevice(prev_); }
+    bool ok() const { return ok_; }
+private:
+    int prev_;
+    bool ok_;
+};
+
+#define AHS_ENTER(s)                                                                                         \
+    if (int r_ = check_sim(s)) return r_;                                                                    \
+    DeviceGuard guard_((s)->device);                                                                         \
+    if (!guard_.ok()) return fail(AHS_ERR_CUDA, "cannot make device %d current: %s", (s)->device, cudaGetErrorString(cudaGetLastError()))
 
 }  // namespace
 
@@ -211,11 +237,18 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     s->cur = 0; s->step = 0; s->launches = 0; s->diag_step = -1; s->device = dev;
     s->kernel = (p.kernel == AHS_KERNEL_AUTO) ? (march_ok ? AHS_KERNEL_MARCH : AHS_KERNEL_GENERIC) : p.kernel;
     s->result_host = nullptr;
+    s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0 };
 
     const size_t need = ahs_required_bytes(p.N, p.precision);
     if (p.device_buffer) {
         if (p.device_buffer_bytes < need || ((uintptr_t)p.device_buffer & 255)) {
             fail(AHS_ERR_INVALID_ARG, "device_buffer must hold %zu bytes and be 256-byte aligned", need);
+            delete s; return nullptr;
+        }
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, p.device_buffer) != cudaSuccess || pa.type != cudaMemoryTypeDevice || pa.device != dev) {
+            cudaGetLastError();
+            fail(AHS_ERR_INVALID_ARG, "device_buffer is not device memory of the current device (%d)", dev);
             delete s; return nullptr;
         }
         s->base = (char*)p.device_buffer; s->owns_buffer = false;
@@ -238,10 +271,10 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     s->step_maps_ok = false;
     if (s->kernel == AHS_KERNEL_MARCH) {
         s->step_maps_ok = p.precision == AHS_F32
-            ? make_step_march_maps<float>(&s->step_maps[0], slot<float>(s, PHI_RE0), slot<float>(s, PI_RE), p.N, s->array_bytes) &&
-              make_step_march_maps<float>(&s->step_maps[1], slot<float>(s, PHI_RE1), slot<float>(s, PI_RE), p.N, s->array_bytes)
-            : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), slot<double>(s, PI_RE), p.N, s->array_bytes) &&
-              make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), slot<double>(s, PI_RE), p.N, s->array_bytes);
+            ? make_step_march_maps<float>(&s->step_maps[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
+              make_step_march_maps<float>(&s->step_maps[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)
+            : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), p.N, s->array_bytes) &&
+              make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), p.N, s->array_bytes);
         s->diag_map_ok = p.precision == AHS_F32
             ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
               make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)
@@ -274,7 +307,7 @@ ahs_sim* ahs_create(int32_t N, double dx, double dt, double lambda, double e, do
 
 int32_t ahs_step(ahs_sim* s, int32_t n)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (n < 0) return fail(AHS_ERR_INVALID_ARG, "n must be >= 0");
     for (int32_t k = 0; k < n; ++k) {
         const int r = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
@@ -288,7 +321,7 @@ int32_t ahs_step(ahs_sim* s, int32_t n)
 
 int32_t ahs_diagnostics_launch(ahs_sim* s)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     const int r = s->p.precision == AHS_F32 ? do_diag<float>(s) : do_diag<double>(s);
     if (r < 0) return fail(r, "diagnostics kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     s->launches += r;
@@ -298,7 +331,7 @@ int32_t ahs_diagnostics_launch(ahs_sim* s)
 
 int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!out) return fail(AHS_ERR_INVALID_ARG, "out is NULL");
     if (s->diag_step < 0) return fail(AHS_ERR_STATE, "no diagnostics launch is pending");
     AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
@@ -327,8 +360,8 @@ int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
     out->v2_V = 2.0 * Rv / (1.0 + Rv);
     out->xi_L = std::sqrt(-(2.0 * M_PI * p.sigma * p.sigma) / out->mean_lagrangian);   // mu = 2 pi sigma^2 (R20)
     s->diag_step = -1;
-    if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "%llu sites hold a non-finite field value at step %lld",
-                                    (unsigned long long)r.nonfinite, (long long)out->step);
+    if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "the lattice holds non-finite field values at step %lld (%llu sites or thread-planes flagged)",
+                                    (long long)out->step, (unsigned long long)r.nonfinite);
     return AHS_OK;
 }
 
@@ -352,7 +385,7 @@ int32_t ahs_diagnostics(ahs_sim* s, double* L, double* v2, double* gauss)
 
 int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     const size_t bytes = (size_t)s->nsites * s->elem;
     for (int k = 0; k < 10; ++k)
@@ -364,7 +397,7 @@ int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
 
 int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
     const size_t bytes = (size_t)s->nsites * s->elem;
@@ -380,7 +413,7 @@ int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
 // the (currently dead) shadow buffer of phi/theta, two arrays of which hold one N^3 array of doubles.
 int32_t ahs_get_fields(ahs_sim* s, double* host10)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (s->p.precision == AHS_F64) return ahs_get_fields_native(s, host10);
     const int shadow = s->cur ? PHI_RE0 : PHI_RE1;   // 5 dead float arrays = room for 2 double arrays
@@ -398,7 +431,7 @@ int32_t ahs_get_fields(ahs_sim* s, double* host10)
 
 int32_t ahs_set_fields(ahs_sim* s, const double* host10, int64_t step)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
     if (s->p.precision == AHS_F64) return ahs_set_fields_native(s, host10, step);
@@ -418,7 +451,7 @@ int32_t ahs_set_fields(ahs_sim* s, const double* host10, int64_t step)
 
 int32_t ahs_field_device_ptr(ahs_sim* s, int32_t k, void** dev_ptr)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (k < 0 || k > 9 || !dev_ptr) return fail(AHS_ERR_INVALID_ARG, "field index must be 0..9 and dev_ptr non-NULL");
     *dev_ptr = s->base + (size_t)live_slot(s, k) * s->array_bytes;
     return AHS_OK;
@@ -426,7 +459,7 @@ int32_t ahs_field_device_ptr(ahs_sim* s, int32_t k, void** dev_ptr)
 
 int32_t ahs_get_state(ahs_sim* s, int64_t* step, double* tau, int64_t* kernel_launches)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (step) *step = s->step;
     if (tau) *tau = tau_of(s->p, s->step);
     if (kernel_launches) *kernel_launches = s->launches;
@@ -435,13 +468,13 @@ int32_t ahs_get_state(ahs_sim* s, int64_t* step, double* tau, int64_t* kernel_la
 
 int32_t ahs_kernel_kind(ahs_sim* s)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     return s->kernel;
 }
 
 int32_t ahs_coefficients(ahs_sim* s, int64_t n, double* out6)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     if (!out6 || n < 0) return fail(AHS_ERR_INVALID_ARG, "out6 is NULL or n < 0");
     const StepCoef c = step_coefficients(s->p, n);
     out6[0] = c.c1; out6[1] = c.c2; out6[2] = c.c3; out6[3] = c.d1; out6[4] = c.d2; out6[5] = c.d3;
@@ -450,14 +483,34 @@ int32_t ahs_coefficients(ahs_sim* s, int64_t n, double* out6)
 
 int32_t ahs_synchronize(ahs_sim* s)
 {
-    if (int r = check_sim(s)) return r;
+    AHS_ENTER(s);
     AHS_CUDA(cudaStreamSynchronize(s->stream));
     return AHS_OK;
+}
+
+int32_t ahs_set_option(ahs_sim* s, int32_t option, int32_t value)
+{
+    AHS_ENTER(s);
+    if (value < 0) return fail(AHS_ERR_INVALID_ARG, "option values are >= 0");
+    switch (option) {
+        case AHS_OPT_STAGING:
+            if (value != AHS_STAGING_TENSOR && value != AHS_STAGING_ROWS) return fail(AHS_ERR_INVALID_ARG, "AHS_OPT_STAGING takes AHS_STAGING_TENSOR or AHS_STAGING_ROWS");
+            s->opt.staging = value;
+            return AHS_OK;
+        case AHS_OPT_STEP_CHUNKS:
+        case AHS_OPT_DIAG_CHUNKS:
+            if (value > s->p.N) return fail(AHS_ERR_INVALID_ARG, "at most N = %d z-chunks per tile", s->p.N);
+            (option == AHS_OPT_STEP_CHUNKS ? s->opt.step_chunks : s->opt.diag_chunks) = value;
+            return AHS_OK;
+        default:
+            return fail(AHS_ERR_INVALID_ARG, "unknown option %d", option);
+    }
 }
 
 int32_t ahs_destroy(ahs_sim* s)
 {
     if (!s) return AHS_OK;
+    DeviceGuard guard_(s->device);
     cudaStreamSynchronize(s->stream);
     if (s->result_host) cudaFreeHost(s->result_host);
     if (s->owns_buffer && s->base) cudaFree(s->base);

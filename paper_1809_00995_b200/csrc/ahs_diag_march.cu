@@ -1,30 +1,38 @@
 // ahs_diag_march.cu -- the fused network diagnostics (winding Eq. 11, <v^2>_L Eqs. 9-10 with the weight of Eq. 2,
 // Gauss residual) as a 2.5D z-march for sm_100a: one read of the ten arrays per call.
 //
-// Same tile and staging as the step kernel (ahs_step_march.cu): a CTA owns TX x TY sites in (x, y) and marches over
-// `zlen` planes; phi_re, phi_im, theta_0..2 of plane k+3 are streamed by cp.async.bulk into a 4-stage ring of halo'd
-// shared-memory tiles (full / empty mbarrier pairs) while planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
+// Same tile and staging as the step kernel (ahs_step_march.cu): a CTA owns TX x TY sites in (x, y) and marches over a
+// z-chunk; phi_re, phi_im, theta_0..2 of plane k+3 are streamed by the copy engine (one tensor-map TMA copy per plane, row
+// copies on the periodic edge in y) into a 4-stage ring of halo'd shared-memory tiles (full / empty mbarrier pairs) while
+// planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
 // All the estimators need only FORWARD neighbours (x+k_i, x+k_i+k_j) of phi, theta -- except the divergence of eps,
 // whose -x / -y / -z terms come by shuffle, one extra row load and a carried register.
 //
-// Winding.  Every thread evaluates arg phi (branch-free atan2_fast) at the ten points of plane k+1 its V sites need and
-// carries them to the next plane in registers; there is NO exchange between warps and therefore no CTA barrier in the
+// The kernel is bound by instruction issue, not by HBM (profiles/r2_diag1024_f32_full.md: 85 % of the issue slots, 47 % of
+// the DRAM bandwidth), so ALL its arithmetic runs on pairs of neighbouring sites with sm_100's packed fp32 instructions
+// (ahs_pack.cuh; for fp64 lattices the same expressions element by element).
+//
+// Winding.  Every thread evaluates arg phi / 2 pi (branch-free atan2_turns) at the ten points of plane k+1 its V sites need
+// and carries them to the next plane in registers; there is NO exchange between warps and therefore no CTA barrier in the
 // march: the warps of a CTA drift freely and meet only at the stage ring's full / empty mbarriers (an earlier version
 // computed each phase once into a shared arg tile and lost 31 % of its issue slots at the per-plane barrier, profiles/r2).
-// The link numbers n_i^x = rint((arg^{x+k_i} - arg^x - theta_i^x) / 2 pi) are formed in fp32 and
+// The link numbers n_i^x = rint(t), t = arg^{x+k_i}/2pi - arg^x/2pi - theta_i^x/2pi, are formed in fp32 and
 // W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x) is summed exactly.  The decision is the fp64 one:
-// a phase is off by <= 6e-7 rad, a quotient by <= 3.5e-7 + 2.5e-7 |t| turns, and whenever a link of a thread-plane lies
-// within 4e-6 (1 + |t|) turns of a half-integer -- ten times that bound -- the thread redoes the plane's plaquettes with
-// fp64 atan2 in a second pass over a device-side doubt list (diag_resolve_kernel; ~4e-4 of the thread-planes), so every
-// rint is the one an all-fp64 evaluation takes and the march itself never diverges.
+//   |t - t_exact| <= 2 eps_a + 3e-8 + 1.6e-7 (1 + |t|) turns with eps_a <= 7.6e-8 turns per phase (atan2_turns, ahs_trig.cuh;
+//   the remaining terms: rounding of the difference, of the fma, of 1/2pi in fp32 and of theta when the lattice is fp64),
+//   i.e. <= 2.4e-7 + 1.6e-7 |t|;
+// whenever some link of a thread-plane lies within kTieMargin (1 + |t|) = 4e-6 (1 + |t|) turns of a half-integer -- more
+// than ten times that bound -- or a plaquette has |W| >= 2 (never seen on physical fields), the thread drops the plane's fast
+// count and appends it to a device-side doubt list, which diag_resolve_kernel redoes with fp64 atan2 (~4e-4 of the
+// thread-planes), so every rint is the one an all-fp64 evaluation takes and the march itself never diverges.
 // <v^2>_L sums: products and the sum over the 16-byte vector of a thread in the storage type, then fp64 accumulation.
 // The paper runs Winding and VelRWLag as two kernels over raw fields with a CUB block sum and a host-side final sum
 // (L140); this is a different design.
-#include <cstdlib>
 #include <cstring>
 
 #include "ahs_internal.cuh"
 #include "ahs_math.cuh"
+#include "ahs_pack.cuh"
 #include "ahs_reduce.cuh"
 #include "ahs_stage.cuh"
 #include "ahs_tma.cuh"
@@ -35,34 +43,40 @@ namespace ahs {
 namespace {
 
 constexpr double kInv2Pi = 0.15915494309189535;
-constexpr float kTieMargin = 4e-6f;   // in units of a full turn, relative to 1 + |t|: ten times the error bound
+constexpr float kTieMargin = 4e-6f;   // in units of a full turn, relative to 1 + |t|: more than ten times the error bound
 
-template <typename T, int TY_, int NS_ = 4>
+template <typename T>
 struct DiagCfg {
     static constexpr int V = 16 / sizeof(T);
-    static constexpr int TY = TY_;
-    static constexpr int NSTAGE = NS_;
+    static constexpr int TY = 4;                             // 4-row tiles (4 warps), three CTAs per SM
+    static constexpr int NSTAGE = 4;
     using G = TileGeom<T, V, TY, 5, NSTAGE, 0, 0>;           // a stage: phi_re, phi_im, theta_0..2 of one plane, forward halo only
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
     static constexpr int STAGE_STRIDE = (int)(((G::STAGE_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
     // right-edge tiles under TMA: the wrapped forward halo column (x = 0 .. V-1) of a plane lands in a side buffer
     static constexpr int WRAP_STRIDE = (int)(((5 * G::ROWS * V * sizeof(T) + 127) & ~(size_t)127) / sizeof(T));
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * (STAGE_STRIDE + WRAP_STRIDE));
+    static constexpr int SLOT_STRIDE = STAGE_STRIDE + WRAP_STRIDE;   // a ring slot = a stage followed by its side buffer
+    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * SLOT_STRIDE);
 };
 
-// Link number of the link s -> t with angle th, fast path, all in fp32: t = (arg_t - arg_s - th) / 2 pi from the
-// atan2_fast phases of the arg tile, n = rint(t) (ties to even) as a float.  |t - t_exact| <= 3.5e-7 + 2.5e-7 |t| turns
-// (6e-7 rad per phase, three roundings, the fp32 constant), so whenever |t - n| < 1/2 - kTieMargin (1 + |t|), n IS the
-// fp64 decision.  `slack` keeps the smallest margin seen; when it is not positive the caller drops the thread-plane's
-// fast count and appends the thread-plane to the doubt list (diag_resolve_kernel).  Everything here is branch-free.
-__device__ __forceinline__ float link_number(float as, float at, float th, float& slack)
+// Link numbers of two links s -> t with angles th, fast path, all in fp32 and in turns: t = (at - as) - th / 2 pi from the
+// atan2_turns phases, n = rint(t) (ties to even) as floats.  rmax / tmax collect max |t - n| and max |t| over the links of
+// a thread-plane: whenever rmax < 1/2 - kTieMargin (1 + tmax) every n IS the fp64 decision (error bound in the header).
+// Everything here is branch-free; NaN never raises rmax (fmaxf drops it) but makes the plaquette sums NaN, which the
+// caller tests.
+__device__ __forceinline__ float2 link_numbers(float2 as, float2 at, float2 th, float& rmax_x, float& rmax_y, float& tmax)
 {
-    const float t = ((at - as) - th) * 0.15915494309189535f;
-    const float n = (t + 12582912.0f) - 12582912.0f;   // 1.5 * 2^23
-    slack = fminf(slack, (0.5f - kTieMargin) - fmaf(kTieMargin, fabsf(t), fabsf(t - n)));
+    const float2 t = pk::fma(th, pk::splat(-0.15915494309189535f), pk::sub(at, as));
+    const float2 n = pk::add(pk::add(t, pk::splat(12582912.0f)), pk::splat(-12582912.0f));   // 1.5 * 2^23
+    const float2 r = pk::sub(t, n);
+    rmax_x = fmaxf(rmax_x, fabsf(r.x));
+    rmax_y = fmaxf(rmax_y, fabsf(r.y));
+    tmax = fmaxf(tmax, fmaxf(fabsf(t.x), fabsf(t.y)));
     return n;
 }
+__device__ __forceinline__ float2 to_float2(float2 v) { return v; }
+__device__ __forceinline__ float2 to_float2(double2 v) { return make_float2((float)v.x, (float)v.y); }
 
 // Second pass over the doubt list: the winding of the V sites of each listed (x/V, y, z), every phase and every quotient
 // in fp64 straight from global memory (same arithmetic as diag_generic_kernel), added to one extra partial record.
@@ -104,22 +118,23 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
     }
 }
 
-template <typename T, int TY, int MINB, int NSTAGES>
-__global__ void __launch_bounds__(DiagCfg<T, TY, NSTAGES>::NTHREADS, MINB)
-diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
+template <typename T>
+__global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, 3)
+diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
                   unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
-                  const __grid_constant__ CUtensorMap wmap, int use_tma, int rotate)
+                  const __grid_constant__ CUtensorMap wmap, int use_tma)
 {
-    using C = DiagCfg<T, TY, NSTAGES>;
+    using C = DiagCfg<T>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
-    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = C::STAGE_STRIDE;
+    using P = pk::Pair<T>;
+    constexpr int V = C::V, NP = V / 2, TX = C::TX, TY = C::TY, NS = C::NSTAGE, SE = C::SLOT_STRIDE;
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
     uint64_t* empty = full + NS;                           // empty[s]: all TY warps have finished reading stage s
-    T* stages = reinterpret_cast<T*>(smem + 128);
-    T* wraps = stages + NS * SE;                           // side buffers of the wrapped column (right-edge tiles under TMA)
+    T* stages = reinterpret_cast<T*>(smem + 128);          // ring slot s at stages + s SE: the stage, then (right-edge tiles under
+                                                           // TMA) the side buffer of the wrapped column at + STAGE_STRIDE
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int tiles_x = N / TX, tiles_y = N / TY;
@@ -127,12 +142,15 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     const int tx = bid % tiles_x;
     bid /= tiles_x;
     const int ty = bid % tiles_y, zc = bid / tiles_y;
-    const int x0 = tx * TX, y0 = ty * TY, z0 = zc * zlen;
+    // z-chunk zc of nchunks: planes [zc N / nchunks, (zc + 1) N / nchunks)
+    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * N / nchunks);
+    const int zlen = (int)((long long)(zc + 1) * N / nchunks) - z0;
     const int xi = V * lane;
 
     const T* const src[5] = { f.phi_re, f.phi_im, f.th[0], f.th[1], f.th[2] };
-    const T inv_dx2 = (T)kd.inv_dx2, gauge_norm = (T)kd.gauge_norm, cB = (T)kd.cB_inv_dx2, pot = (T)kd.pot_coef;
-    const T sigma2 = (T)kd.sigma2, grhs = (T)kd.gauss_rhs;
+    const P inv_dx2 = pk::splat((T)kd.inv_dx2), gauge_norm = pk::splat((T)kd.gauge_norm), ncB = pk::splat(-(T)kd.cB_inv_dx2);
+    const P pot = pk::splat((T)kd.pot_coef), nsigma2 = pk::splat(-(T)kd.sigma2), grhs = pk::splat((T)kd.gauss_rhs);
+    const P half = pk::splat(T(0.5)), four = pk::splat(T(4));
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -145,7 +163,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
     auto plane_of = [&](int p) { const int z = z0 + p; return z >= N ? z - N : z; };
     // One tensor copy per plane for tiles away from the periodic boundary.  Tiles on the right edge get the main box
     // (zero-filled out of bounds) plus a V-wide tensor copy of the wrapped column x = 0 .. V-1 into a side buffer, which the
-    // readers of column TX use instead; tiles on the top edge in y (2 of N/TY tile rows) keep the row copies.
+    // readers of column TX use instead; tiles on the top edge in y (1 of N/TY tile rows) keep the row copies.
     const bool right_edge = x0 + TX == N;
     const bool tma_tile = use_tma && (y0 + TY < N);
     const bool wrapR = tma_tile && right_edge;
@@ -153,240 +171,271 @@ diag_march_kernel(DiagPtrs<T> f, int N, int zlen, DiagCoef kd, DiagPartial* __re
         mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + (wrapR ? (uint32_t)(5 * G::ROWS * V * sizeof(T)) : 0u));
         if (tma_tile) {
             tma_load_4d(stages + s * SE, &tmap, x0, y0, plane_of(p), 0, &full[s]);
-            if (wrapR) tma_load_4d(wraps + s * C::WRAP_STRIDE, &wmap, 0, y0, plane_of(p), 0, &full[s]);
+            if (wrapR) tma_load_4d(stages + s * SE + C::STAGE_STRIDE, &wmap, 0, y0, plane_of(p), 0, &full[s]);
         } else {
             issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
         }
     };
-    // element (array a, row r) right of this thread's vector: column xi + V (= TX for the last lane)
-    auto edge = [&](const T* st, int a, int r) -> T {
-        return (wrapR && lane == 31) ? (wraps + (st - stages) / SE * C::WRAP_STRIDE)[(a * G::ROWS + r) * V] : st[G::idx(a, r, xi + V)];
-    };
+    // element (array a, row w + dr) right of this thread's vector: column xi + V (= TX for the last lane, which on a
+    // right-edge tile under TMA reads the side buffer instead).  The offsets from the slot base are per-thread constants.
+    const bool side = wrapR && lane == 31;
+    auto edge_off = [&](int a, int r) { return side ? C::STAGE_STRIDE + (a * G::ROWS + r) * V : G::idx(a, r, xi + V); };
+    const int eo_re = edge_off(0, w), eo_im = edge_off(1, w), eo_rey = edge_off(0, w + 1), eo_imy = edge_off(1, w + 1);
+    const int eo_t1 = edge_off(3, w), eo_t2 = edge_off(4, w);
     if (w == 0 && elect_one()) {
 #pragma unroll
         for (int p = 0; p < NS - 1; ++p)
             if (p <= zlen) issue_plane(p, p);
     }
 
-    // arg phi at the V sites of this thread and at the site right of them, rows w and w+1 of a staged plane.  Every
-    // thread evaluates the ten phases it needs itself (2.5 per site instead of 1): no exchange, hence no CTA barrier
-    // anywhere in the march -- the warps of a CTA drift freely and only meet at the stage ring's mbarriers.
-    auto args_of = [&](const T* st, float (&a0)[V + 1], float (&a1)[V + 1]) {
+    // arg phi / 2 pi at the V sites of this thread (pairs p0: row w, p1: row w+1) and at the site right of them (pe = rows
+    // w, w+1).  Every thread evaluates the ten phases it needs itself (2.5 per site instead of 1): no exchange, hence no CTA
+    // barrier anywhere in the march -- the warps of a CTA drift freely and only meet at the stage ring's mbarriers.
+    auto phases_of = [&](const T* st, float2 (&p0)[NP], float2 (&p1)[NP], float2& pe) {
         const VecT pr = lds_vec<T, V>(st + G::idx(0, w, xi)), pi = lds_vec<T, V>(st + G::idx(1, w, xi));
         const VecT pry = lds_vec<T, V>(st + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(st + G::idx(1, w + 1, xi));
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-            a0[v] = atan2_fast((float)pi.v[v], (float)pr.v[v]);
-            a1[v] = atan2_fast((float)piy.v[v], (float)pry.v[v]);
+        for (int h = 0; h < NP; ++h) {
+            p0[h] = atan2_turns(to_float2(pk::at<T, V>(pi.v, h)), to_float2(pk::at<T, V>(pr.v, h)));
+            p1[h] = atan2_turns(to_float2(pk::at<T, V>(piy.v, h)), to_float2(pk::at<T, V>(pry.v, h)));
         }
-        a0[V] = atan2_fast((float)edge(st, 1, w), (float)edge(st, 0, w));
-        a1[V] = atan2_fast((float)edge(st, 1, w + 1), (float)edge(st, 0, w + 1));
+        pe = atan2_turns(make_float2((float)st[eo_im], (float)st[eo_imy]), make_float2((float)st[eo_re], (float)st[eo_rey]));
     };
+    // the pair of phases one site to the right of pair h: (p[2h+1], p[2h+2]), the last one being the edge phase
+    auto shifted = [&](const float2 (&p)[NP], int h, float e) { return make_float2(p[h].y, h + 1 < NP ? p[h + 1 < NP ? h + 1 : h].x : e); };
 
     mbar_wait(&full[0], 0);
     // phases of the current plane and n_0, n_1 of its links (own sites; n_1 also right of the vector), carried along
-    // the march together with the smallest margin of those link numbers
-    float a[V + 1], ay[V + 1], n0c[V], n1c[V + 1], slack_c = 1.0f;
-    args_of(stages, a, ay);
+    // the march together with the margins of those link numbers
+    float2 a[NP], ay[NP], ae, n0c[NP], n1c[NP];
+    float n1c_e, rmax_c = 0.0f, tmax_c = 0.0f;
+    phases_of(stages, a, ay, ae);
     {
         const VecT t0 = lds_vec<T, V>(stages + G::idx(2, w, xi)), t1 = lds_vec<T, V>(stages + G::idx(3, w, xi));
-        const T t1x_e = edge(stages, 3, w);
+        float dummy = 0.0f;
 #pragma unroll
-        for (int v = 0; v <= V; ++v) {
-            n1c[v] = link_number(a[v], ay[v], (float)(v < V ? t1.v[v < V ? v : 0] : t1x_e), slack_c);
-            if (v < V) n0c[v < V ? v : 0] = link_number(a[v], a[v < V ? v + 1 : v], (float)t0.v[v < V ? v : 0], slack_c);
+        for (int h = 0; h < NP; ++h) {
+            n1c[h] = link_numbers(a[h], ay[h], to_float2(pk::at<T, V>(t1.v, h)), rmax_c, rmax_c, tmax_c);
+            n0c[h] = link_numbers(a[h], shifted(a, h, ae.x), to_float2(pk::at<T, V>(t0.v, h)), rmax_c, rmax_c, tmax_c);
         }
+        const float th_e = (float)stages[eo_t1];
+        n1c_e = link_numbers(make_float2(ae.x, ae.x), make_float2(ae.y, ae.y), make_float2(th_e, th_e), rmax_c, dummy, tmax_c).x;
     }
 
+    // The momenta (no halo) come straight from global memory: g = element offset of this thread's vector in plane z0 + it, a
+    // running offset; the row below (eps_1^{x-k_1}) and the site left of the tile (eps_0^{x-k_0}, lane 0) sit at fixed distances.
+    const size_t plane_stride = (size_t)N * N;
+    size_t g = ((size_t)z0 * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+    const ptrdiff_t d_row_below = (y0 + w == 0) ? (ptrdiff_t)(N - 1) * N : -(ptrdiff_t)N;
+    const ptrdiff_t d_site_left = (x0 == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;   // (lane 0 only: xi = 0)
     // eps_2 of the plane below, carried in registers along the march
-    VecT E2m;
-    {
-        const int zm = z0 == 0 ? N - 1 : z0 - 1;
-        E2m = ldg_vec<T, V>(f.eps[2] + ((size_t)zm * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi));
-    }
+    VecT E2m = ldg_vec<T, V>(f.eps[2] + (z0 == 0 ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));
 
-    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, gmax = 0.0, vnum = 0.0, vden = 0.0;
-    unsigned n_pierced = 0u, nonfinite = 0u;
-    unsigned sum_abs_w = 0u;
+    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+    float pierced_f = 0.0f;   // plaquettes with W != 0 on the fast path (all |W| <= 1 there, so this is sum |W| as well); exact below 2^24
+    unsigned nonfinite = 0u;
     T gmax_t = T(0);
 
+    const T* sc = stages;             // slot of plane it (walks the ring with running pointers: no index arithmetic per plane)
+    int ring = 0;                     // it % NS
     for (int it = 0; it < zlen; ++it) {
-        const T* sc = stages + (it % NS) * SE;
-        const T* sn = stages + ((it + 1) % NS) * SE;
+        const int ring_n = ring + 1 == NS ? 0 : ring + 1;
+        const T* sn = ring_n ? sc + SE : stages;
 
-        // plane it+3 -> the stage that held plane it-1, once all TY warps have released it
-        if (w == (rotate ? it % TY : 0) && it + NS - 1 <= zlen && elect_one()) {
-            const int s = (it + NS - 1) % NS;
+        // plane it+3 -> the stage that held plane it-1, once all TY warps have released it (the issuing warp rotates)
+        static_assert(TY == NS, "the issuing warp rotates with the ring");
+        if (w == ring && it + NS - 1 <= zlen && elect_one()) {
+            const int s = ring == 0 ? NS - 1 : ring - 1;   // (it + NS - 1) % NS
             if (it > 0) mbar_wait(&empty[s], ((it - 1) / NS) & 1);
             issue_plane(s, it + NS - 1);
         }
 
-        const int z = z0 + it, y = y0 + w;
-        const size_t grow = ((size_t)z * N + (size_t)y) * N;
-        const size_t g = grow + (size_t)(x0 + xi);
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
         const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
-        const int ym = y == 0 ? N - 1 : y - 1;
-        const VecT E1m = ldg_vec<T, V>(f.eps[1] + ((size_t)z * N + (size_t)ym) * N + (size_t)(x0 + xi));
+        const VecT E1m = ldg_vec<T, V>(f.eps[1] + (g + d_row_below));
         T e0_halo = T(0);
-        if (lane == 0) e0_halo = f.eps[0][grow + (size_t)(x0 == 0 ? N - 1 : x0 - 1)];
+        if (lane == 0) e0_halo = f.eps[0][g + d_site_left];
 
-        mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
-        float az[V + 1], azy[V + 1];
-        args_of(sn, az, azy);
+        mbar_wait(&full[ring_n], ((it + 1) / NS) & 1);
+        float2 az[NP], azy[NP], aze;
+        phases_of(sn, az, azy, aze);
 
-        // ---- phase B: everything of plane `it` ---------------------------------------------------------------------------
         const VecT pr = lds_vec<T, V>(sc + G::idx(0, w, xi)), pi = lds_vec<T, V>(sc + G::idx(1, w, xi));
         const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(sc + G::idx(4, w, xi));
         const VecT pry = lds_vec<T, V>(sc + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(sc + G::idx(1, w + 1, xi));
         const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(sc + G::idx(4, w + 1, xi));
         const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
-        const T prx_e = edge(sc, 0, w), pix_e = edge(sc, 1, w);
-        const T t1x_e = edge(sc, 3, w), t2x_e = edge(sc, 4, w);
+        const T prx_e = sc[eo_re], pix_e = sc[eo_im];
+        const T t1x_e = sc[eo_t1], t2x_e = sc[eo_t2];
         // E0 of the site to the left: previous element, else lane-1's last element, else (lane 0) the halo value
         T e0_left = __shfl_up_sync(0xffffffffu, E0.v[V - 1], 1);
         if (lane == 0) e0_left = e0_halo;
 
         // ---- winding (Eq. 11), fast path: the link numbers this thread-plane needs.  n_0, n_1 of this plane were formed
         //      one iteration ago (as the +z links); n_1, n_2 are also taken at the site right of the vector (n_j^{x+k_0}).
-        float slack = slack_c;                               // margins of the carried n0c, n1c
-        float n2[V + 1], n0y[V], n2y[V], n0z[V], n1z[V + 1];
-        slack_c = 1.0f;
+        float rmax = rmax_c, tmax = tmax_c;                  // margins of the carried n0c, n1c
+        float2 n2[NP], n0y[NP], n2y[NP], n0z[NP], n1z[NP];
+        rmax_c = 0.0f;
+        tmax_c = 0.0f;
+#pragma unroll
+        for (int h = 0; h < NP; ++h) {
+            n2[h] = link_numbers(a[h], az[h], to_float2(pk::at<T, V>(t2.v, h)), rmax, rmax, tmax);
+            n2y[h] = link_numbers(ay[h], azy[h], to_float2(pk::at<T, V>(t2y.v, h)), rmax, rmax, tmax);
+            n0y[h] = link_numbers(ay[h], shifted(ay, h, ae.y), to_float2(pk::at<T, V>(t0y.v, h)), rmax, rmax, tmax);
+            n1z[h] = link_numbers(az[h], azy[h], to_float2(pk::at<T, V>(t1z.v, h)), rmax_c, rmax_c, tmax_c);
+            n0z[h] = link_numbers(az[h], shifted(az, h, aze.x), to_float2(pk::at<T, V>(t0z.v, h)), rmax_c, rmax_c, tmax_c);
+        }
+        // right of the vector: (n_2 of this plane, n_1 of the next) in one packed evaluation
+        float tmax_e = 0.0f;
+        const float2 ne = link_numbers(make_float2(ae.x, aze.x), make_float2(aze.x, aze.y), make_float2((float)t2x_e, (float)sn[eo_t1]),
+                                       rmax, rmax_c, tmax_e);
+        tmax = fmaxf(tmax, tmax_e);
+        tmax_c = fmaxf(tmax_c, tmax_e);
+        float2 sabs = pk::splat(0.0f), ssq = pk::splat(0.0f);   // small integers: exact in fp32
+#pragma unroll
+        for (int h = 0; h < NP; ++h) {
+            const float2 n1x = make_float2(n1c[h].y, h + 1 < NP ? n1c[h + 1 < NP ? h + 1 : h].x : n1c_e);   // n_1^{x+k_0}
+            const float2 n2x = make_float2(n2[h].y, h + 1 < NP ? n2[h + 1 < NP ? h + 1 : h].x : ne.x);      // n_2^{x+k_0}
+            const float2 W01 = pk::sub(pk::add(n0c[h], n1x), pk::add(n0y[h], n1c[h]));   // -W_ij
+            const float2 W02 = pk::sub(pk::add(n0c[h], n2x), pk::add(n0z[h], n2[h]));
+            const float2 W12 = pk::sub(pk::add(n1c[h], n2y[h]), pk::add(n1z[h], n2[h]));
+            sabs = pk::add(pk::add(sabs, pk::absv(W01)), pk::add(pk::absv(W02), pk::absv(W12)));
+            ssq = pk::fma(W01, W01, pk::fma(W02, W02, pk::fma(W12, W12, ssq)));
+        }
         {
-            const T t1z_e = edge(sn, 3, w);
-#pragma unroll
-            for (int v = 0; v <= V; ++v) {
-                n2[v] = link_number(a[v], az[v], (float)(v < V ? t2.v[v < V ? v : 0] : t2x_e), slack);
-                n1z[v] = link_number(az[v], azy[v], (float)(v < V ? t1z.v[v < V ? v : 0] : t1z_e), slack_c);
+            const float cnt = sabs.x + sabs.y;
+            // sure: every link is far from a tie and every |W| <= 1 (integers: sum W^2 == sum |W|); NaN fails both
+            // (n_0, n_1 of the next plane enter this plane's W_02, W_12 as the +z links: their margins count here too)
+            const bool sure = (fmaxf(rmax, rmax_c) < 0.5f - kTieMargin * (1.0f + fmaxf(tmax, tmax_c))) && (ssq.x + ssq.y == cnt);
+            if (!sure) {   // fp64 decides (diag_resolve_kernel)
+                const unsigned long long e = atomicAdd(doubt_count, 1ull);
+                doubt_list[e] = (unsigned)((x0 + xi) / V) | ((unsigned)(y0 + w) << 10) | ((unsigned)(z0 + it) << 21);   // N <= 2048
             }
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-                n0y[v] = link_number(ay[v], ay[v + 1], (float)t0y.v[v], slack);
-                n2y[v] = link_number(ay[v], azy[v], (float)t2y.v[v], slack);
-                n0z[v] = link_number(az[v], az[v + 1], (float)t0z.v[v], slack_c);
-            }
+            pierced_f += sure ? cnt : 0.0f;
         }
-        unsigned pierced = 0u;
-        float abs_w = 0.0f;                              // small integers: exact in fp32
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const float W01 = (n0c[v] + n1c[v + 1]) - (n0y[v] + n1c[v]);   // -W_ij
-            const float W02 = (n0c[v] + n2[v + 1]) - (n0z[v] + n2[v]);
-            const float W12 = (n1c[v] + n2y[v]) - (n1z[v] + n2[v]);
-            pierced += (W01 != 0.0f) + (W02 != 0.0f) + (W12 != 0.0f);
-            abs_w += (fabsf(W01) + fabsf(W02)) + fabsf(W12);
-        }
-        unsigned absw_u = (unsigned)abs_w;
-        if (!(fminf(slack, slack_c) > 0.0f) || !(abs_w < 1.0e6f)) {   // a link too close to a tie (or NaN / huge): fp64 decides
-            const unsigned long long e = atomicAdd(doubt_count, 1ull);
-            doubt_list[e] = (unsigned)((x0 + xi) / V) | ((unsigned)(y0 + w) << 10) | ((unsigned)(z0 + it) << 21);
-            pierced = 0u;
-            absw_u = 0u;
-        }
-        n_pierced += pierced;
-        sum_abs_w += absw_u;
-#pragma unroll
-        for (int v = 0; v < V; ++v) n0c[v] = n0z[v];
-#pragma unroll
-        for (int v = 0; v <= V; ++v) { n1c[v] = n1z[v]; a[v] = az[v]; ay[v] = azy[v]; }
+        for (int h = 0; h < NP; ++h) { n0c[h] = n0z[h]; n1c[h] = n1z[h]; a[h] = az[h]; ay[h] = azy[h]; }
+        n1c_e = ne.y;
+        ae = aze;
 
-        T p_num = T(0), p_den = T(0), p_l = T(0), p_r2 = T(0), p_vn = T(0), p_vd = T(0);   // per thread and plane (V sites), then into the fp64 sums
+        // ---- Eq. 2 pieces, <v^2> sums and the Gauss residual, two sites at a time --------------------------------------------
+        P p_num = pk::splat(T(0)), p_den = p_num, p_l = p_num, p_r2 = p_num, p_vn = p_num, p_vd = p_num;   // per thread and plane, then into the fp64 sums
 #pragma unroll
-        for (int v = 0; v < V; ++v) {
-            const Cx<T> ph = { pr.v[v], pi.v[v] };
-            const Cx<T> pm = { Pr.v[v], Pi.v[v] };
-            const T th0 = t0.v[v], th1 = t1.v[v], th2 = t2.v[v];
-            const T ep0 = E0.v[v], ep1 = E1.v[v], ep2 = E2.v[v];
-            // ---- Eq. 2 pieces ---------------------------------------------------------------------------------------------------
-            T s, c;
-            sincos_fast(th0, s, c);
-            const Cx<T> f0 = mulU<T>(c, s, { next_x<T, V>(pr, v, prx_e), next_x<T, V>(pi, v, pix_e) });
-            sincos_fast(th1, s, c);
-            const Cx<T> f1 = mulU<T>(c, s, { pry.v[v], piy.v[v] });
-            sincos_fast(th2, s, c);
-            const Cx<T> f2 = mulU<T>(c, s, { prz.v[v], piz.v[v] });
-            T Gd = (f0.re - ph.re) * (f0.re - ph.re) + (f0.im - ph.im) * (f0.im - ph.im);
-            Gd += (f1.re - ph.re) * (f1.re - ph.re) + (f1.im - ph.im) * (f1.im - ph.im);
-            Gd += (f2.re - ph.re) * (f2.re - ph.re) + (f2.im - ph.im) * (f2.im - ph.im);
-            Gd *= inv_dx2;
-            const T K = pm.re * pm.re + pm.im * pm.im;
-            const T dm = ph.re * ph.re + ph.im * ph.im - sigma2;
-            const T Vp = pot * dm * dm;
+        for (int h = 0; h < NP; ++h) {
+            const P phr = pk::at<T, V>(pr.v, h), phi = pk::at<T, V>(pi.v, h), pmr = pk::at<T, V>(Pr.v, h), pmi = pk::at<T, V>(Pi.v, h);
+            const P th0 = pk::at<T, V>(t0.v, h), th1 = pk::at<T, V>(t1.v, h), th2 = pk::at<T, V>(t2.v, h);
+            const P ep0 = pk::at<T, V>(E0.v, h), ep1 = pk::at<T, V>(E1.v, h), ep2 = pk::at<T, V>(E2.v, h);
+            P s0, c0, s1, c1, s2, c2;
+            sincos_pair(th0, s0, c0);
+            sincos_pair(th1, s1, c1);
+            sincos_pair(th2, s2, c2);
+            // forward hops U_j phi^{x+k_j} - phi^x, U = cos - i sin:  (c re + s im, c im - s re)
+            const P nxr = pk::next<T, V>(pr.v, h, prx_e), nxi = pk::next<T, V>(pi.v, h, pix_e);
+            const P d0r = pk::sub(pk::fma(c0, nxr, pk::mul(s0, nxi)), phr), d0i = pk::sub(pk::fma(pk::neg(s0), nxr, pk::mul(c0, nxi)), phi);
+            const P nyr = pk::at<T, V>(pry.v, h), nyi = pk::at<T, V>(piy.v, h);
+            const P d1r = pk::sub(pk::fma(c1, nyr, pk::mul(s1, nyi)), phr), d1i = pk::sub(pk::fma(pk::neg(s1), nyr, pk::mul(c1, nyi)), phi);
+            const P nzr = pk::at<T, V>(prz.v, h), nzi = pk::at<T, V>(piz.v, h);
+            const P d2r = pk::sub(pk::fma(c2, nzr, pk::mul(s2, nzi)), phr), d2i = pk::sub(pk::fma(pk::neg(s2), nzr, pk::mul(c2, nzi)), phi);
+            P Gd = pk::fma(d0r, d0r, pk::mul(d0i, d0i));
+            Gd = pk::fma(d1r, d1r, pk::fma(d1i, d1i, Gd));
+            Gd = pk::fma(d2r, d2r, pk::fma(d2i, d2i, Gd));
+            Gd = pk::mul(Gd, inv_dx2);
+            const P K = pk::fma(pmr, pmr, pk::mul(pmi, pmi));
+            const P dm = pk::fma(phr, phr, pk::fma(phi, phi, nsigma2));
+            const P Vp = pk::mul(pot, pk::mul(dm, dm));
             // 1 - cos Xi = 2 sin^2(Xi/2), without the cancellation of the literal form at small Xi
-            const T h01 = sin_fast(T(0.5) * (th0 + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - th1));
-            const T h02 = sin_fast(T(0.5) * (th0 + next_x<T, V>(t2, v, t2x_e) - t0z.v[v] - th2));
-            const T h12 = sin_fast(T(0.5) * (th1 + t2y.v[v] - t1z.v[v] - th2));
-            const T mag = T(4) * (h01 * h01 + h02 * h02 + h12 * h12);   // ordered pairs: 2 x [2 sin^2] per plaquette (R12)
-            const T e2 = ep0 * ep0 + ep1 * ep1 + ep2 * ep2;
-            const T lag = (e2 - cB * mag) * gauge_norm + K - Gd - Vp;
-            p_num += K * lag;
-            p_den += Gd * lag;
-            p_l += lag;
-            p_vn += K * Vp;   // potential-weighted estimator <v^2>_V (L86)
-            p_vd += Gd * Vp;
-            nonfinite += finite_t(lag) ? 0u : 1u;   // every one of the ten values feeds lag: NaN or Inf in, NaN or Inf out
+            const P X01 = pk::sub(pk::add(th0, pk::next<T, V>(t1.v, h, t1x_e)), pk::add(pk::at<T, V>(t0y.v, h), th1));
+            const P X02 = pk::sub(pk::add(th0, pk::next<T, V>(t2.v, h, t2x_e)), pk::add(pk::at<T, V>(t0z.v, h), th2));
+            const P X12 = pk::sub(pk::add(th1, pk::at<T, V>(t2y.v, h)), pk::add(pk::at<T, V>(t1z.v, h), th2));
+            const P h01 = sin_pair(pk::mul(half, X01)), h02 = sin_pair(pk::mul(half, X02)), h12 = sin_pair(pk::mul(half, X12));
+            const P mag = pk::mul(four, pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12))));   // ordered pairs: 2 x [2 sin^2] per plaquette (R12)
+            const P e2 = pk::fma(ep0, ep0, pk::fma(ep1, ep1, pk::mul(ep2, ep2)));
+            const P lag = pk::sub(pk::sub(pk::fma(pk::fma(ncB, mag, e2), gauge_norm, K), Gd), Vp);
+            p_num = pk::fma(K, lag, p_num);
+            p_den = pk::fma(Gd, lag, p_den);
+            p_l = pk::add(p_l, lag);
+            p_vn = pk::fma(K, Vp, p_vn);   // potential-weighted estimator <v^2>_V (L86)
+            p_vd = pk::fma(Gd, Vp, p_vd);
 
-            // ---- Gauss residual ---------------------------------------------------------------------------------------------------
-            const T e0m = v > 0 ? E0.v[v > 0 ? v - 1 : 0] : e0_left;
-            const T div = ((ep0 - e0m) + (ep1 - E1m.v[v])) + (ep2 - E2m.v[v]);
-            const T rhs = grhs * (ph.re * pm.im - ph.im * pm.re);
-            const T gabs = fabs(div - rhs);
-            gmax_t = gabs > gmax_t ? gabs : gmax_t;   // (a NaN residual is reported through `nonfinite`)
-            p_r2 += rhs * rhs;
+            // ---- Gauss residual: sum_i (eps_i^x - eps_i^{x-k_i}) - gauss_rhs Im[conj(phi) Pi] ----------------------------------
+            const P e0m = pk::mk(h > 0 ? E0.v[h > 0 ? 2 * h - 1 : 0] : e0_left, E0.v[2 * h]);
+            const P div = pk::add(pk::add(pk::sub(ep0, e0m), pk::sub(ep1, pk::at<T, V>(E1m.v, h))), pk::sub(ep2, pk::at<T, V>(E2m.v, h)));
+            const P rhs = pk::mul(grhs, pk::fma(phr, pmi, pk::neg(pk::mul(phi, pmr))));
+            const P gabs = pk::absv(pk::sub(div, rhs));
+            const T g2 = gabs.x > gabs.y ? gabs.x : gabs.y;
+            gmax_t = g2 > gmax_t ? g2 : gmax_t;   // (a NaN residual is reported through `nonfinite`)
+            p_r2 = pk::fma(rhs, rhs, p_r2);
         }
-        num += (double)p_num; den += (double)p_den; lsum += (double)p_l; rhs2 += (double)p_r2;
-        vnum += (double)p_vn; vden += (double)p_vd;
+        const T l_plane = p_l.x + p_l.y;
+        num += (double)(p_num.x + p_num.y); den += (double)(p_den.x + p_den.y); lsum += (double)l_plane; rhs2 += (double)(p_r2.x + p_r2.y);
+        vnum += (double)(p_vn.x + p_vn.y); vden += (double)(p_vd.x + p_vd.y);
+        // Non-finite values.  Every one of the ten stored values feeds the Lagrangian (NaN or Inf in, NaN or Inf out), so a
+        // finite plane sum clears all of them at once; otherwise the stored values themselves are examined (a finite value
+        // whose square overflows the storage type is not an error: include/ahs.h "nonfinite").
+        if (!finite_t(l_plane)) {
+            bool bad = false;
+#pragma unroll
+            for (int v = 0; v < V; ++v)
+                bad = bad || !finite_t(pr.v[v]) || !finite_t(pi.v[v]) || !finite_t(Pr.v[v]) || !finite_t(Pi.v[v]) || !finite_t(t0.v[v]) ||
+                      !finite_t(t1.v[v]) || !finite_t(t2.v[v]) || !finite_t(E0.v[v]) || !finite_t(E1.v[v]) || !finite_t(E2.v[v]);
+            // (the forward neighbours that also feed this plane's sum are the own sites of other threads)
+            nonfinite += bad ? 1u : 0u;
+        }
         E2m = E2;
         // this warp is done with stage `sc` (plane it): release it to the copy-issuing thread
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[it % NS]);
+        if (lane == 0) mbar_arrive(&empty[ring]);
+        sc = sn;
+        ring = ring_n;
+        g += plane_stride;
     }
 
-    gmax = (double)gmax_t;
-    DiagPartial acc = { (unsigned long long)n_pierced, (unsigned long long)sum_abs_w, num, den, lsum, gmax, rhs2, (unsigned long long)nonfinite, vnum, vden };
+    const unsigned long long n_fast = (unsigned long long)pierced_f;
+    DiagPartial acc = { n_fast, n_fast, num, den, lsum, (double)gmax_t, rhs2, (unsigned long long)nonfinite, vnum, vden };
     block_reduce_store(acc, partials + blockIdx.x);
 }
 
-template <typename T, int TY>
-int pick_zlen(int N, int ctas_per_sm, int max_partials)
+// z-chunks per tile: the fewest (longest marches; a chunk start costs one extra staged plane) that still give >= 4 waves of
+// resident CTAs and fit the partials buffer; chunk lengths 128 ... 8 as far as N allows
+template <typename T>
+int pick_chunks(int N, int ctas_per_sm, int max_partials)
 {
-    using C = DiagCfg<T, TY>;
-    const long tiles = (long)(N / C::TX) * (N / TY);
+    using C = DiagCfg<T>;
+    const long tiles = (long)(N / C::TX) * (N / C::TY);
     const int cands[5] = { 128, 64, 32, 16, 8 };
-    for (int c : cands)   // the longest march that still gives >= 4 waves of resident CTAs (the prologue costs one plane)
-        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials && tiles * (N / c) >= 4L * ctas_per_sm * 148) return c;
     for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials) return c;
-    return N;
+        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials && tiles * (N / c) >= 4L * ctas_per_sm * 148) return N / c;
+    for (int c : cands)
+        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials) return N / c;
+    return 1;
 }
 
-template <typename T, int TY, int MINB, int NSTAGES = 4>
-int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-               void* list, size_t list_bytes, const DiagMaps* tmap, cudaStream_t st)
+}  // namespace
+
+template <typename T>
+int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
+                      void* list, size_t list_bytes, const DiagMaps* tmap, const MarchOptions& opt, cudaStream_t st)
 {
-    using C = DiagCfg<T, TY, NSTAGES>;
-    auto kern = diag_march_kernel<T, TY, MINB, NSTAGES>;
-    static bool configured = false;
-    if (!configured) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return AHS_ERR_CUDA;
-        configured = true;
-    }
-    static const int zlen_env = [] { const char* e = getenv("AHS_DIAG_ZLEN"); return e ? atoi(e) : 0; }();
-    const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB, max_partials);
-    const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
+    using C = DiagCfg<T>;
+    if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
+    auto kern = diag_march_kernel<T>;
+    static SmemAttribute attr;   // per device
+    if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
+    const long tiles = (long)(N / C::TX) * (N / C::TY);
+    int nchunks = pick_chunks<T>(N, 3, max_partials);
+    if (opt.diag_chunks > 0 && opt.diag_chunks <= N && tiles * opt.diag_chunks + 2 <= max_partials) nchunks = opt.diag_chunks;
+    const long blocks = tiles * nchunks;
     // partials[blocks] collects the second pass, partials[blocks + 1].n_pierced is the length of the doubt list
     if (blocks + 2 > max_partials || list_bytes < sizeof(unsigned) * ((size_t)N * N * N / C::V)) return AHS_ERR_INVALID_ARG;
     DiagPartial* extra = partials + blocks;
     unsigned long long* count = &partials[blocks + 1].n_pierced;
     if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
-    static const bool tma_off = getenv("AHS_NO_TMA") != nullptr;
-    static const int rot = [] { const char* e = getenv("AHS_DIAG_ROT"); return e ? atoi(e) : 1; }();
     DiagMaps none;
     memset(&none, 0, sizeof(none));
-    const bool use_tma = tmap && !tma_off;
+    const bool use_tma = tmap && opt.staging == AHS_STAGING_TENSOR;
     const DiagMaps& mp = use_tma ? *tmap : none;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0, rot);
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
@@ -394,27 +443,11 @@ int launch_cfg(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* part
     return r < 0 ? r : 3;
 }
 
-}  // namespace
-
-template <typename T>
-int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
-                      void* list, size_t list_bytes, const DiagMaps* tmap, cudaStream_t st)
-{
-    if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
-    // 4-row tiles (3 CTAs/SM) by default; AHS_DIAG_TY=8 selects 8-row tiles, two CTAs per SM (experiments)
-    static const int ty = [] { const char* e = getenv("AHS_DIAG_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, partials, max_partials, result, list, list_bytes, nullptr, st);
-    static const int ns = [] { const char* e = getenv("AHS_DIAG_NS"); return e ? atoi(e) : 4; }();
-    if (ns == 5) return launch_cfg<T, 4, 3, 5>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
-    if (ns == 3) return launch_cfg<T, 4, 3, 3>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
-    return launch_cfg<T, 4, 3>(f, N, c, partials, max_partials, result, list, list_bytes, tmap, st);
-}
-
-// the tensor map of one (phi, theta) buffer for the default tile shape (4 rows): box (TX + V, TY + 1, 1, 5)
+// the tensor map of one (phi, theta) buffer for the tile shape above: box (TX + V, TY + 1, 1, 5)
 template <typename T>
 bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t array_bytes)
 {
-    using G = typename DiagCfg<T, 4>::G;
+    using G = typename DiagCfg<T>::G;
     if (!march_supported<T>(N)) return false;
     return make_tile_map<T>(&out->tile, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 5) &&
            make_tile_map<T>(&out->wrap, phi_re_base, N, array_bytes, 5, G::V, G::ROWS, 5);
@@ -422,7 +455,7 @@ bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t a
 template bool make_diag_march_map<float>(DiagMaps*, const void*, int, size_t);
 template bool make_diag_march_map<double>(DiagMaps*, const void*, int, size_t);
 
-template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, cudaStream_t);
-template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, cudaStream_t);
+template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
+template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
 
 }  // namespace ahs

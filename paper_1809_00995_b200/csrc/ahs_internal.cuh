@@ -6,6 +6,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/ahs.h"
 
 namespace ahs {
@@ -61,13 +63,37 @@ struct DiagPtrs {
     const T* pi_re; const T* pi_im; const T* eps[3];
 };
 
+// Tuning of the marching kernels, set per handle through ahs_set_option (include/ahs.h); 0 = the library's choice.
+struct MarchOptions {
+    int staging;       // AHS_STAGING_TENSOR (tensor-map TMA where a tile allows it) or AHS_STAGING_ROWS (row copies only)
+    int step_chunks;   // z-chunks per tile of the step march
+    int diag_chunks;   // z-chunks per tile of the diagnostics march
+};
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: set it once on every device a kernel is launched on
+// (one static instance per kernel instantiation; handles on different GPUs of one process share the kernels).
+struct SmemAttribute {
+    std::atomic<unsigned long long> done{ 0ull };
+    template <typename K> bool ensure(K kernel, size_t bytes)
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return false;
+        const unsigned long long bit = dev < 64 ? 1ull << dev : 0ull;
+        if (bit && (done.load(std::memory_order_acquire) & bit)) return true;
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) return false;
+        done.fetch_or(bit, std::memory_order_release);
+        return true;
+    }
+};
+
 // ---- kernel launchers (each returns the number of kernels it launched, or a negative ahs error) -------------
 template <typename T> int launch_ic(T* phi_re, T* phi_im, int N, double sigma, uint64_t seed, int kind, cudaStream_t st);
 template <typename T> int launch_step_generic(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st);
-// TMA descriptors of the step march: the four-array stage and theta_2 of one (phi, theta) buffer, and the momenta
-struct StepMaps { CUtensorMap stage, th2, mom, wstage, wth2; };   // w*: the V-wide wrapped halo column of x-edge tiles
-template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps /* HOST, may be NULL */, cudaStream_t st);
-template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi_re_base, int N, size_t array_bytes);
+// TMA descriptors of the step march: the four-array stage and theta_2 of one (phi, theta) buffer
+struct StepMaps { CUtensorMap stage, th2, wstage, wth2; };   // w*: the V-wide wrapped halo column of x-edge tiles
+template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps /* HOST, may be NULL */,
+                                            const MarchOptions& opt, cudaStream_t st);
+template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, size_t array_bytes);
 template <typename T> bool march_supported(int N);
 template <typename T> int launch_diag_generic(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
                                               int max_partials, DiagPartial* result, cudaStream_t st);
@@ -76,7 +102,8 @@ struct DiagMaps { CUtensorMap tile, wrap; };
 // `list`: DEVICE scratch of >= 4 N^3 / (16 / sizeof(T)) bytes for the winding doubt list (the dead phi', theta' shadow buffer)
 template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
                                             int max_partials, DiagPartial* result, void* list, size_t list_bytes,
-                                            const DiagMaps* tmap /* HOST, may be NULL: row copies only */, cudaStream_t st);
+                                            const DiagMaps* tmap /* HOST, may be NULL: row copies only */, const MarchOptions& opt,
+                                            cudaStream_t st);
 // tensor map (TMA descriptor) of the five level-n arrays of one (phi, theta) buffer for the diagnostics march; false if unavailable
 template <typename T> bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t array_bytes);
 int launch_diag_finish(const DiagPartial* partials, int n, DiagPartial* result, cudaStream_t st);

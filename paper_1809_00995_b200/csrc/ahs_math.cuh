@@ -18,9 +18,12 @@ __device__ __forceinline__ bool finite_t(double x) { return isfinite(x); }
 // complex helpers on (re, im) pairs; U = cos(theta) - i sin(theta)  (q = +1, R1)
 template <typename T> struct Cx { T re, im; };
 
+// The contraction into fused multiply-adds is written out (one rounded product, one fma) so that a hop is rounded the same
+// way wherever the compiler inlines it: the step march forms conj(U_2) phi both in a chunk's prologue and in its loop, and
+// the fields must not depend on where the chunk boundaries fall.
 // U * z = (c - i s)(re + i im) = (c re + s im) + i (c im - s re)
-template <typename T> __device__ __forceinline__ Cx<T> mulU(T c, T s, Cx<T> z) { return { c * z.re + s * z.im, c * z.im - s * z.re }; }
+template <typename T> __device__ __forceinline__ Cx<T> mulU(T c, T s, Cx<T> z) { return { fma(c, z.re, s * z.im), fma(c, z.im, -(s * z.re)) }; }
 // conj(U) * z = (c + i s)(re + i im) = (c re - s im) + i (c im + s re)
-template <typename T> __device__ __forceinline__ Cx<T> mulUc(T c, T s, Cx<T> z) { return { c * z.re - s * z.im, c * z.im + s * z.re }; }
+template <typename T> __device__ __forceinline__ Cx<T> mulUc(T c, T s, Cx<T> z) { return { fma(c, z.re, -(s * z.im)), fma(c, z.im, s * z.re) }; }
 
 }  // namespace ahs

@@ -30,7 +30,6 @@
 // double-buffered by plane parity so that the barrier of plane k+1 also orders "everyone has read plane k's
 // exchange" before it is overwritten at plane k+2.
 // The paper's kernels stage raw fields per kernel and recompute every phase (L107-109); this is a different design.
-#include <cstdlib>
 #include <cstring>
 
 #include "ahs_internal.cuh"
@@ -67,9 +66,9 @@ struct MarchCfg {
 
 template <typename T, int TY, int MINB>
 __global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB)
-step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
-                  const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_mom,
-                  const __grid_constant__ CUtensorMap map_wstage, const __grid_constant__ CUtensorMap map_wth2, int use_tma)
+step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
+                  const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_wstage,
+                  const __grid_constant__ CUtensorMap map_wth2, int use_tma)
 {
     using C = MarchCfg<T, TY>;
     using G = typename C::G;
@@ -95,7 +94,9 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     const int tx = bid % tiles_x;
     bid /= tiles_x;
     const int ty = bid % tiles_y, zc = bid / tiles_y;
-    const int x0 = tx * TX, y0 = ty * TY, z0 = zc * zlen;
+    // z-chunk zc of nchunks: planes [zc N / nchunks, (zc + 1) N / nchunks) -- the chunks need not be of equal length
+    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * N / nchunks);
+    const int zlen = (int)((long long)(zc + 1) * N / nchunks) - z0;
     const int xi = V * lane;
 
     const T* const src[4] = { f.phi_re, f.phi_im, f.th[0], f.th[1] };
@@ -117,7 +118,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     // left edge, x = 0.. for the right edge) arrives by a second, V-wide tensor copy in a side buffer, which the few readers of
     // that column use instead.  y-edge tiles (2 of N/TY tile rows) and lattices one tile wide keep the row copies.
     const bool left_edge = x0 == 0, right_edge = x0 + TX == N;
-    const bool tma_tile = (use_tma & 1) && y0 > 0 && y0 + TY < N && !(left_edge && right_edge);
+    const bool tma_tile = use_tma && y0 > 0 && y0 + TY < N && !(left_edge && right_edge);
     const bool wrapL = tma_tile && left_edge, wrapR = tma_tile && right_edge;
     const int xw = left_edge ? N - V : 0;
     const uint32_t wrap_tx = (wrapL || wrapR) ? (uint32_t)(4 * G::ROWS * V * sizeof(T)) : 0u, wrap2_tx = (wrapL || wrapR) ? (uint32_t)(G::ROWS * V * sizeof(T)) : 0u;
@@ -144,13 +145,6 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     auto edgeR = [&](const T* st, const T* side, int a, int r, int c) -> T {   // c = column index of the element, <= TX
         return (wrapR && c == TX) ? side[(a * G::ROWS + r + 1) * V] : st[G::idx(a, r, c)];
     };
-    // the momenta of plane z (no halo) are asked into L2 one plane ahead of the streaming loads that consume them
-    auto prefetch_momenta = [&](int z) {
-        if (use_tma & 2)
-            asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_mom)),
-                         "r"(x0), "r"(y0), "r"(z), "r"(0)
-                         : "memory");
-    };
     if (w == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
@@ -159,7 +153,6 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
                 mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx + (t2 ? G::ARR_BYTES + wrap2_tx : 0u));
                 issue_stage(i, i);
                 if (t2) issue_th2(i, i, i);
-                if (i == 0) prefetch_momenta(z0);
             }
         }
     }
@@ -192,8 +185,13 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         sin_vec<V>(X02, cS02);
         sin_vec<V>(X12, cS12);
     }
-    __syncthreads();
-    wait_barrier_resolved(full);   // the first in-loop copy re-fills the stage the prologue has just read
+    // Hand stage 0 and theta_2 slot 0 over to the copy engine with the protocol the march uses: every thread signals the
+    // exchange barrier once its prologue reads have been issued (the arrive travels down the same shared-memory pipe
+    // behind them, release semantics) and waits for the phase to complete, so the thread that re-fills the stage at plane 1
+    // has synchronised with every reader before its fence.proxy.async.  (A __syncthreads() here was not enough on sm_100:
+    // profiles/r2_race.md.)  Phase 0 of `xch` = prologue, phase it = plane it.
+    mbar_arrive(xch);
+    mbar_wait(xch, 0);
 
     const T dtc2 = k.dt * k.c2, dtd3 = k.dt * k.d3;
 
@@ -219,18 +217,11 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
         // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
         if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
             const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
-            fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1: all reads of that stage are done)
+            fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1 / of the prologue: all reads of that stage are done)
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES + wrap_tx + wrap2_tx);
             issue_stage(s, it + 2);
             issue_th2((it + 1) & 1, s, it + 1);
-            if ((use_tma & 4) && tma_tile && it + 3 <= zlen + 1) {   // (experiment) the plane after that: into L2 only
-                asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_stage)),
-                             "r"(x0 - V), "r"(y0 - 1), "r"(plane_of(it + 3)), "r"(0) : "memory");
-                asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(reinterpret_cast<uint64_t>(&map_th2)),
-                             "r"(x0 - V), "r"(y0 - 1), "r"(plane_of(it + 2)), "r"(4) : "memory");
-            }
         }
-        if (((w + it) % TY) == ISSUER && it < zlen && elect_one()) prefetch_momenta(z0 + it);   // plane of iteration it+1
 
         const size_t g = gnext;                                         // plane z0 + it - 1
         const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested one plane ago
@@ -364,7 +355,7 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
             nPr = ldg_vec<T, V>(f.pi_re + gnext); nPi = ldg_vec<T, V>(f.pi_im + gnext);
             nE0 = ldg_vec<T, V>(f.eps[0] + gnext); nE1 = ldg_vec<T, V>(f.eps[1] + gnext); nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
         }
-        mbar_wait(xch, (it - 1) & 1);   // all 128 threads have signalled plane `it`: exchange rows complete, stages no longer read
+        mbar_wait(xch, it & 1);   // all 128 threads have signalled plane `it`: exchange rows complete, stages no longer read
         {
             // ---- phase 2: the terms that crossed a warp or tile boundary, then the stores ----------------------------
             const VecT yb1r = lds_vec<T, V>(yexp + (0 * TY + w) * TX + xi), yb1i = lds_vec<T, V>(yexp + (1 * TY + w) * TX + xi);
@@ -397,40 +388,35 @@ step_march_kernel(FieldPtrs<T> f, int N, int zlen, StepCoefT<T> k, const __grid_
     }
 }
 
+// Number of z-chunks per tile: the fewest (longest marches: a chunk start costs one extra staged plane and the trigonometry of
+// its -z products) that still gives >= 4 waves of resident CTAs; chunk lengths 64, 32, 16, 8 as far as N allows.
 template <typename T, int TY>
-int pick_zlen(int N, int ctas_per_sm)
+int pick_chunks(int N, int ctas_per_sm)
 {
     using C = MarchCfg<T, TY>;
     const long tiles = (long)(N / C::TX) * (N / TY);
     const int cands[4] = { 64, 32, 16, 8 };
     for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) >= 4L * ctas_per_sm * 148) return c;   // >= 4 waves of resident CTAs
-    return 8;
+        if (N % c == 0 && tiles * (N / c) >= 4L * ctas_per_sm * 148) return N / c;
+    return N / 8;
 }
 
 template <typename T, int TY, int MINB>
-int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, cudaStream_t st)
+int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
 {
     using C = MarchCfg<T, TY>;
     auto kern = step_march_kernel<T, TY, MINB>;
-    static bool configured = false;
-    if (!configured) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return AHS_ERR_CUDA;
-        configured = true;
-    }
-    static const int zlen_env = [] { const char* e = getenv("AHS_MARCH_ZLEN"); return e ? atoi(e) : 0; }();
-    const int zlen = (zlen_env > 0 && N % zlen_env == 0) ? zlen_env : pick_zlen<T, TY>(N, MINB);
-    const long blocks = (long)(N / C::TX) * (N / TY) * (N / zlen);
+    static SmemAttribute attr;   // per device: the kernel needs more than the default 48 KB of dynamic shared memory
+    if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
+    const int nchunks = (opt.step_chunks > 0 && opt.step_chunks <= N) ? opt.step_chunks : pick_chunks<T, TY>(N, MINB);
+    const long blocks = (long)(N / C::TX) * (N / TY) * nchunks;
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
-    // AHS_STEP_TMA (experiments): bit 0 = tensor copies for the stages (default), bit 1 = L2 prefetch of the momenta one
-    // plane ahead (off: with the software-pipelined loads it only adds 5 % of DRAM reads, profiles/r2_step1024_f32_full.md)
-    static const int tma_mode = [] { const char* e = getenv("AHS_STEP_TMA"); return getenv("AHS_NO_TMA") ? 0 : (e ? atoi(e) & 7 : 1); }();
-    if (maps && tma_mode) {
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, maps->stage, maps->th2, maps->mom, maps->wstage, maps->wth2, tma_mode);
+    if (maps && opt.staging == AHS_STAGING_TENSOR) {
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, k, maps->stage, maps->th2, maps->wstage, maps->wth2, 1);
     } else {
         StepMaps none;
         memset(&none, 0, sizeof(none));
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zlen, k, none.stage, none.th2, none.mom, none.wstage, none.wth2, 0);
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, k, none.stage, none.th2, none.wstage, none.wth2, 0);
     }
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
@@ -440,44 +426,37 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* 
 template <typename T>
 bool march_supported(int N)
 {
-    using C = MarchCfg<T, 8>;
-    return N >= C::TX && N % C::TX == 0 && N % 8 == 0;
+    using C = MarchCfg<T, 4>;
+    return N >= C::TX && N % C::TX == 0;
 }
 
+// 4-row tiles (4 warps), three CTAs per SM: measured fastest (profiles/r2, r3)
 template <typename T>
-int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, cudaStream_t st)
+int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
-    // 4-row tiles, four CTAs (barrier domains) per SM, measured fastest (profiles/); AHS_MARCH_TY=8 (experiments
-    // only) selects 8-row tiles, two CTAs per SM
-    static const int ty = [] { const char* e = getenv("AHS_MARCH_TY"); return e ? atoi(e) : 4; }();
-    if (ty == 8) return launch_cfg<T, 8, 2>(f, N, c, maps, st);   // (the maps are built for the same AHS_MARCH_TY)
-    if (ty == 16 && N % 16 == 0) return launch_cfg<T, 16, 1>(f, N, c, nullptr, st);
-    return launch_cfg<T, 4, 3>(f, N, c, maps, st);
+    return launch_cfg<T, 4, 3>(f, N, c, maps, opt, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu
 template bool march_supported<float>(int);
 template bool march_supported<double>(int);
-template int launch_step_march<float>(const FieldPtrs<float>&, int, const StepCoef&, const StepMaps*, cudaStream_t);
-template int launch_step_march<double>(const FieldPtrs<double>&, int, const StepCoef&, const StepMaps*, cudaStream_t);
+template int launch_step_march<float>(const FieldPtrs<float>&, int, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
+template int launch_step_march<double>(const FieldPtrs<double>&, int, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
 
-// tensor maps of one (phi, theta) buffer and of the momenta for the default tile shape (4 rows)
+// tensor maps of one (phi, theta) buffer for the tile shape above
 template <typename T>
-bool make_step_march_maps(StepMaps* out, const void* phi_re_base, const void* pi_re_base, int N, size_t array_bytes)
+bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, size_t array_bytes)
 {
     using C = MarchCfg<T, 4>;
     using G = typename C::G;
     if (!march_supported<T>(N)) return false;
-    const char* e = getenv("AHS_MARCH_TY");
-    const int rows = (e && atoi(e) == 8) ? 10 : G::ROWS, ty = rows - 2;   // experiments: 8-row tiles
-    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, rows, 4) &&
-           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, rows, 1) &&
-           make_tile_map<T>(&out->mom, pi_re_base, N, array_bytes, 5, C::TX, ty, 5) &&
-           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, rows, 4) &&
-           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, rows, 1);
+    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
+           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
+           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 4) &&
+           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 1);
 }
-template bool make_step_march_maps<float>(StepMaps*, const void*, const void*, int, size_t);
-template bool make_step_march_maps<double>(StepMaps*, const void*, const void*, int, size_t);
+template bool make_step_march_maps<float>(StepMaps*, const void*, int, size_t);
+template bool make_step_march_maps<double>(StepMaps*, const void*, int, size_t);
 
 }  // namespace ahs

@@ -3,18 +3,19 @@
 // Why not libdevice sincosf/sinf: the step is issue-bound as much as HBM-bound, six
 // transcendental evaluations per site are half of its instructions, and every libdevice call carries a
 // Payne-Hanek slow path whose branch (BSSY/BSYNC) stalls instruction fetch and bloats the loop past the
-// instruction cache (profiles/r1_step512_march_v1.md).  Why not the __sinf/__cosf intrinsics: their absolute
+// instruction cache (seen on the first marching kernel of round 1; no profile of that version was kept).  Why not
+// the __sinf/__cosf intrinsics: their absolute
 // error (2^-21) is what PAPER.md L142 reports as degrading the diagnostics.  So: Cody-Waite reduction with a
 // two-term (fp32) / three-term (fp64) split of pi/2 (or pi) carried by FMAs, then minimax-style polynomials on the reduced interval.
 //
 //   sincos_fast(x): k = rint(x * 2/pi), r = x - k*pi/2 in [-pi/4, pi/4]; sin and cos polynomials; quadrant fix-up.
 //   sin_fast(x)   : fp32: k = rint(x / pi), r in [-pi/2, pi/2], odd polynomial, sign (-1)^k;
 //                   fp64: the quadrant form with the coefficient set chosen by the parity of k.
-// Measured against fp64 references (csrc/fit_trig.py): fp32 sincos <= 0.9 ulp, fp32 sin <= 1.9 ulp
+// Measured against fp64 references (tests/tools/fit_trig.py): fp32 sincos <= 0.9 ulp, fp32 sin <= 1.9 ulp
 // (abs 1.2e-7), fp64 <= 1.3 ulp.  Domain: |x| < 2^22 * pi/2 (fp32: 6.5e6; fp64: |x| < 2^30); beyond it the result
 // is finite garbage or NaN (a link angle that large has no phase information left in fp32 anyway); NaN and Inf
 // inputs give NaN, so blown-up lattices still reach the diagnostics' non-finite flag.
-// The polynomial coefficients were fitted by csrc/fit_trig.py (least squares on Chebyshev nodes, relative
+// The polynomial coefficients were fitted by tests/tools/fit_trig.py (least squares on Chebyshev nodes, relative
 // weighting), not copied from a library.
 #pragma once
 #include <cuda_runtime.h>
@@ -25,7 +26,7 @@ namespace ahs {
 // The arithmetic is written once over a lane type W: float, or float2 evaluated with Blackwell's packed fp32
 // instructions (FFMA2 / FMUL2 / FADD2 on sm_100: two IEEE fp32 operations per issued instruction, constants broadcast from
 // immediates).  Both give bit-identical results per lane; the marching kernels use the packed form on pairs of sites,
-// which takes a quarter of the instructions out of the step kernel's trigonometry (profiles/r3).
+// which takes a quarter of the instructions out of the step kernel's trigonometry (profiles/r3_step1024_f32_full.md).
 namespace lanes {
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ float mul_(float a, float b) { return a * b; }
@@ -111,25 +112,37 @@ __device__ __forceinline__ float2 sin_fast(float2 x)
                        __int_as_float(__float_as_int(sr.y) ^ (__float_as_int(t.y) << 31)));
 }
 
-// atan2 for the winding fast path (ahs_diag_march.cu): branch-free, absolute error <= 2.5e-7 rad in the fp32 emulation of
-// fit_trig.py (the fast path's error budget assumes <= 4.8e-7).  q = min/max in [0, 1], odd polynomial of degree 15, then
-// the octant fix-ups.  atan2_fast(0, 0) and non-finite inputs give NaN, which sends the link to the fp64 evaluation.
-__device__ __forceinline__ float atan2_fast(float y, float x)
+// arg(x + i y) / 2 pi, in turns, for the winding fast path (ahs_diag_march.cu): two values at once, branch-free.
+// q = min/max in [0, 1] (MUFU.RCP and a multiply), odd polynomial of degree 15 in q fitted to atan(q) / 2 pi, then the
+// octant fix-ups, whose constants 1/4 and 1/2 are exact in turns.  Absolute error <= 5e-8 turns in the fp32 emulation of
+// tests/tools/fit_trig.py (the fast path's error budget assumes <= 7.6e-8 turns = 4.8e-7 rad).  atan2_turns(0, 0) and
+// non-finite inputs give NaN, which sends the link to the fp64 evaluation.
+__device__ __forceinline__ float rcp_approx(float x)
 {
-    const float ax = fabsf(x), ay = fabsf(y);
-    const float q = __fdividef(fminf(ax, ay), fmaxf(ax, ay));
-    const float z = q * q;
-    float p = fmaf(z, -0.004054565913975239f, 0.021862955763936043f);
-    p = fmaf(z, p, -0.055912330746650696f);
-    p = fmaf(z, p, 0.096421979367733f);
-    p = fmaf(z, p, -0.1390863060951233f);
-    p = fmaf(z, p, 0.19946566224098206f);
-    p = fmaf(z, p, -0.33329859375953674f);
-    p = fmaf(z, p, 0.9999993443489075f);
-    float r = q * p;
-    r = ay > ax ? 1.5707963705062866f - r : r;
-    r = x < 0 ? 3.1415927410125732f - r : r;
-    return copysignf(r, y);
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float2 atan2_turns(float2 y, float2 x)
+{
+    using namespace lanes;
+    const float ax0 = fabsf(x.x), ay0 = fabsf(y.x), ax1 = fabsf(x.y), ay1 = fabsf(y.y);
+    const float2 mn = make_float2(fminf(ax0, ay0), fminf(ax1, ay1));
+    const float2 q = mul_(mn, make_float2(rcp_approx(fmaxf(ax0, ay0)), rcp_approx(fmaxf(ax1, ay1))));
+    const float2 z = mul_(q, q);
+    float2 p = fma_(z, all<float2>(-0.00064530421514064074f), all<float2>(0.0034795976243913174f));
+    p = fma_(z, p, all<float2>(-0.0088987238705158234f));
+    p = fma_(z, p, all<float2>(0.015346035361289978f));
+    p = fma_(z, p, all<float2>(-0.022136272862553596f));
+    p = fma_(z, p, all<float2>(0.031745944172143936f));
+    p = fma_(z, p, all<float2>(-0.053046122193336487f));
+    p = fma_(z, p, all<float2>(0.15915483236312866f));
+    float2 r = mul_(q, p);
+    const float2 r4 = add_(all<float2>(0.25f), make_float2(-r.x, -r.y));
+    r = make_float2(ay0 > ax0 ? r4.x : r.x, ay1 > ax1 ? r4.y : r.y);
+    const float2 r2 = add_(all<float2>(0.5f), make_float2(-r.x, -r.y));
+    r = make_float2(x.x < 0.0f ? r2.x : r.x, x.y < 0.0f ? r2.y : r.y);
+    return make_float2(copysignf(r.x, y.x), copysignf(r.y, y.y));
 }
 
 // ---- fp64 ---------------------------------------------------------------------------------------------------------------
@@ -222,5 +235,15 @@ __device__ __forceinline__ void sin_vec(const double (&x)[V], double (&y)[V])
 #pragma unroll
     for (int v = 0; v < V; ++v) y[v] = sin_fast(x[v]);
 }
+
+// ---- pairs of sites (ahs_pack.cuh): fp32 through the packed form, fp64 element by element ------------------------------
+__device__ __forceinline__ void sincos_pair(float2 x, float2& s, float2& c) { sincos_fast(x, s, c); }
+__device__ __forceinline__ float2 sin_pair(float2 x) { return sin_fast(x); }
+__device__ __forceinline__ void sincos_pair(double2 x, double2& s, double2& c)
+{
+    sincos_fast(x.x, s.x, c.x);
+    sincos_fast(x.y, s.y, c.y);
+}
+__device__ __forceinline__ double2 sin_pair(double2 x) { return make_double2(sin_fast(x.x), sin_fast(x.y)); }
 
 }  // namespace ahs

@@ -530,3 +530,97 @@ def test_c_B_parameter_reaches_the_weight(ahs, oracle):
         assert abs(d["v2_num"] - r["v2_num"]) <= 1e-10 * np.abs(K * Lg).sum()
         assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= 1e-10 * np.abs(Lg).mean()
         assert d["n_pierced"] == r["n_pierced"] and d["v2v_num"] == pytest.approx(r["v2v_num"], rel=1e-10)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# tuning options (ahs_set_option), several handles, the non-finite flag
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,N", [("f32", 256), ("f64", 128)])
+def test_options_change_the_launch_shape_not_the_result(ahs, prec, N):
+    """Every accepted value of ahs_set_option: row-copy staging instead of tensor-map TMA, and z-chunk counts from one chunk
+    per tile to chunks of 2 and 3 planes (uneven: 100 and 37 do not divide N), which multiplies the chunk starts where the
+    march hands its first stages over to the copy engine.  Fields must be bit-identical to the default launch shape
+    (each site's arithmetic does not depend on the tiling); the integer counts equal; the fp64 sums equal to reduction order."""
+    with ahs.Simulation(N=N, precision=prec, seed=21) as ref:
+        ref.step(6)
+        want, dref = ref.get_fields_native(), ref.diagnostics()
+    settings = [{ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS}, {ahs.AHS_OPT_STEP_CHUNKS: 1, ahs.AHS_OPT_DIAG_CHUNKS: 1},
+                {ahs.AHS_OPT_STEP_CHUNKS: 100, ahs.AHS_OPT_DIAG_CHUNKS: 37}, {ahs.AHS_OPT_STEP_CHUNKS: N // 2, ahs.AHS_OPT_DIAG_CHUNKS: N // 4},
+                {ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS, ahs.AHS_OPT_STEP_CHUNKS: 37, ahs.AHS_OPT_DIAG_CHUNKS: 5}]
+    for opts in settings:
+        with ahs.Simulation(N=N, precision=prec, seed=21) as sim:
+            for k, v in opts.items():
+                sim.set_option(k, v)
+            sim.step(6)
+            assert np.array_equal(sim.get_fields_native(), want), opts
+            d = sim.diagnostics()
+            assert (d["n_pierced"], d["sum_abs_w"], d["nonfinite"]) == (dref["n_pierced"], dref["sum_abs_w"], 0), opts
+            for key in ("v2_num", "v2_den", "v2v_num", "v2v_den", "mean_lagrangian", "gauss_rhs_rms"):
+                assert d[key] == pytest.approx(dref[key], rel=1e-11, abs=1e-11 * abs(dref["v2_den"])), (opts, key)
+            assert d["gauss_max"] == dref["gauss_max"], opts
+    with ahs.Simulation(N=N, precision=prec) as sim:
+        for bad in ((99, 0), (ahs.AHS_OPT_STAGING, 2), (ahs.AHS_OPT_STEP_CHUNKS, N + 1), (ahs.AHS_OPT_DIAG_CHUNKS, -1)):
+            with pytest.raises(ahs.AhsError) as e:
+                sim.set_option(*bad)
+            assert e.value.code == ahs.AHS_ERR_INVALID_ARG
+
+
+def test_two_handles_on_two_streams_interleaved(ahs):
+    """Distinct handles are independent (include/ahs.h): two replicas on two streams, their steps and asynchronous
+    diagnostics interleaved from one host thread, give what each gives alone."""
+    import torch
+    N = 256
+    alone = []
+    for seed in (1, 2):
+        with ahs.Simulation(N=N, precision="f32", seed=seed) as sim:
+            sim.step(8)
+            alone.append((sim.diagnostics(), sim.get_fields_native()))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    sims = []
+    for seed, st in zip((1, 2), streams):
+        with torch.cuda.stream(st):
+            sims.append(ahs.Simulation(N=N, precision="f32", seed=seed))
+    assert sims[0].stream_handle != sims[1].stream_handle
+    for _ in range(4):
+        for sim in sims:
+            sim.step(1)
+        for sim in sims:
+            sim.diagnostics_launch()
+        for sim in reversed(sims):
+            sim.step(1)
+    got = [sim.diagnostics_fetch() for sim in sims]          # the record of the LAST launch (step 7)
+    for sim, (d_alone, f_alone), g in zip(sims, alone, got):
+        assert g["step"] == 7
+        d = sim.diagnostics()
+        assert d["step"] == 8 and d["n_pierced"] == d_alone["n_pierced"] and d["v2_num"] == d_alone["v2_num"]
+        assert np.array_equal(sim.get_fields_native(), f_alone)
+        sim.destroy()
+
+
+@pytest.mark.parametrize("prec,N,kernel", [("f32", 128, "auto"), ("f32", 128, "generic"), ("f64", 64, "auto"), ("f64", 24, "generic")])
+def test_nonfinite_flag_means_a_stored_value_is_not_finite(ahs, oracle, prec, N, kernel):
+    """include/ahs.h: `nonfinite` is about the ten stored arrays, on both diagnostics implementations and on the oracle: a NaN
+    or an infinity in any one of them sets it; a finite value whose square overflows the storage type does not."""
+    from paper_1809_00995_b200 import synthetic
+    base = rounded(synthetic.random_snapshot(N, seed=8), prec)
+    p = oracle.Params(N=N, m=1.0, s=0.0)
+    rng = np.random.default_rng(0)
+    with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.0, ic="none", kernel=kernel) as sim:
+        for k in range(10):
+            f = base.copy()
+            z, y, x = (int(v) for v in rng.integers(0, N, 3))
+            f[k, z, y, x] = np.nan if k % 2 else np.inf
+            sim.set_fields(f, 0)
+            assert sim.diagnostics()["nonfinite"] == 1, oracle.FIELD_NAMES[k]
+            if k in (0, 5, 9):
+                assert oracle.diagnostics(p, f, 0)["nonfinite"] == 1
+        big = 1e20 if prec == "f32" else 1e160
+        for k in (0, 2, 7):
+            f = base.copy()
+            f[k, N // 2, 1, N - 1] = big
+            sim.set_fields(f, 0)
+            d = sim.diagnostics()
+            assert d["nonfinite"] == 0 and not math.isfinite(d["mean_lagrangian"]), oracle.FIELD_NAMES[k]
+            assert oracle.diagnostics(p, f, 0)["nonfinite"] == 0
+        sim.set_fields(base, 0)
+        assert sim.diagnostics()["nonfinite"] == 0
