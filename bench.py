@@ -38,10 +38,11 @@ BYTES_PER_SITE = {"f32": 80, "f64": 160}          # 10 values read + 10 written 
 FALLBACK_HBM_GBS = 6650.0                         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the committed `ncu --set full`
-# capture (profiles/); keyed by (kernel, precision, lattice).  None = no capture for that configuration.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r3_step1024_f32_full.md: 48.35 GB read + 42.90 GB written per launch
-    ("march", "f32", 1024): 91.25e9,
+# captures (profiles/); keyed by (kernel, precision, lattice) -> (bytes, capture).  Absent = no capture for that configuration:
+# the line then carries "traffic": null.  A capture is only listed while the kernel it was taken on is the one that ships
+# (the capture names its commit).
+NCU_TRAFFIC = {
+    ("march", "f32", 1024): (91.25e9, "profiles/r3_step1024_f32_full.md (48.35 GB read + 42.90 GB written per launch)"),
 }
 
 
@@ -121,12 +122,14 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------------------------
 # the oracle on the host cores: cpu_baseline leg and the --impl reference arm (the only places bench.py runs oracle/)
 # ------------------------------------------------------------------------------------------------------------------
-def oracle_sample(args, steps: int = 1, warmup: int = 0) -> dict:
-    """Time the fp64 oracle, as it stands (single thread), on a bounded sample of the workload: a cpu_lattice^3
-    lattice with the same physics, `cpu_leapfrog` leapfrog steps + one diagnostics pass per bench step."""
+def oracle_sample(args, steps: int = 1, warmup: int = 0, threads: int = 1, lattice: int = 0) -> dict:
+    """Time the fp64 oracle, as it stands, on a bounded sample of the workload: a lattice^3 lattice with the same physics,
+    `cpu_leapfrog` leapfrog steps + one diagnostics pass per bench step, on `threads` host threads (0 = all cores online;
+    the oracle's results do not depend on the thread count)."""
     import numpy as np
     from oracle import ahs_oracle as O
-    N, L = args.cpu_lattice, args.cpu_leapfrog
+    N, L = lattice or args.cpu_lattice, args.cpu_leapfrog
+    used = O.set_threads(threads)
     p = O.Params(N=N, m=args.m, s=args.s, tau_ref=args.tau_ref, **COMMON)
     f = O.initial_condition(p, SEED)
     if args.precision == "f32":
@@ -140,23 +143,34 @@ def oracle_sample(args, steps: int = 1, warmup: int = 0) -> dict:
         O.step(p, f, n, L); n += L
         d = O.diagnostics(p, f, n)
     dt = time.perf_counter() - t0
-    return {"value": N ** 3 * L * steps / dt, "unit": "site-updates/s", "cores": 1, "kind": "oracle",
-            "sample": "%d^3 lattice, same physics (m=%g, s=%g), %d x (%d leapfrog steps + 1 diagnostics), fp64, 1 thread, %.1f s"
-                      % (N, args.m, args.s, steps, L, dt),
-            "seconds": dt, "n_pierced": int(d["n_pierced"]), "host_cores_online": os.cpu_count()}
+    O.set_threads(1)
+    return {"value": N ** 3 * L * steps / dt, "unit": "site-updates/s", "cores": used, "kind": "oracle",
+            "sample": "%d^3 lattice, same physics (m=%g, s=%g), %d x (%d leapfrog steps + 1 diagnostics), fp64, %d thread%s, %.1f s"
+                      % (N, args.m, args.s, steps, L, used, "" if used == 1 else "s", dt),
+            "seconds": dt, "n_pierced": int(d["n_pierced"]), "host_cores_online": os.cpu_count(), "cpu_model": cpu_model()}
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def run_reference(args):
     """--impl reference: for this tier the reference arm is the oracle on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    steps, warm = max(1, args.steps), max(0, min(args.warmup, 1))
-    # bound the whole run to a few minutes: ~1 us per site-update
-    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 1.5e8 and args.cpu_leapfrog > 1:
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    # bound the whole run to a few minutes: ~0.3 us per site-update on one core, all cores are used
+    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 6e8 and args.cpu_leapfrog > 1:
         args.cpu_leapfrog = max(1, args.cpu_leapfrog // 2)
-    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 1.5e8 and args.cpu_lattice > 32:
+    while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 6e8 and args.cpu_lattice > 32:
         args.cpu_lattice //= 2
-    r = oracle_sample(args, steps=steps, warmup=warm)
+    r = oracle_sample(args, steps=steps, warmup=warm, threads=0)     # all host cores
     line = {
         "impl": "reference", "metric": "lattice site-updates/sec per leapfrog step", "value": r["value"], "unit": "site-updates/s",
         "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * r["seconds"] / steps,
@@ -268,7 +282,8 @@ def run_ours(args):
     peak, peak_src = measured_peak()
     achieved = BYTES_PER_SITE[args.precision] * sites / launch_s / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get((sim.kernel_kind, args.precision, N)),
+                "traffic": NCU_TRAFFIC.get((sim.kernel_kind, args.precision, N), (None, None))[0],
+                "traffic_source": NCU_TRAFFIC.get((sim.kernel_kind, args.precision, N), (None, "no ncu capture for this configuration"))[1],
                 "kernel": "fused leapfrog step (%s)" % sim.kernel_kind, "peak_source": peak_src,
                 "bytes_per_launch": BYTES_PER_SITE[args.precision] * sites, "launch_ms": launch_s * 1e3,
                 "frac_of_nominal_8TBps": achieved / 8000.0,
@@ -293,8 +308,11 @@ def run_ours(args):
         line["e2e"] = e2e
     sim.destroy()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = oracle_sample(args)
-        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores_online")}
+        # the oracle on all host cores (a sample twice as wide: ~10 s) and, beside it, on one core
+        r = oracle_sample(args, threads=0, lattice=2 * args.cpu_lattice)
+        one = oracle_sample(args, threads=1)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample", "host_cores_online", "cpu_model")}
+        line["cpu_baseline"]["one_core"] = {k: one[k] for k in ("value", "unit", "cores", "sample")}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
