@@ -48,7 +48,8 @@ constexpr float kTieMargin = 4e-6f;   // in units of a full turn, relative to 1 
 template <typename T>
 struct DiagCfg {
     static constexpr int V = 16 / sizeof(T);
-    static constexpr int TY = 4;                             // 4-row tiles (4 warps), three CTAs per SM
+    static constexpr int TY = 4;                             // 4-row tiles (4 warps)
+    static constexpr int MINB = sizeof(T) == 8 ? 2 : 3;      // CTAs per SM the register budget is cut for (fp64: 255 registers, no spills)
     static constexpr int NSTAGE = 4;
     using G = TileGeom<T, V, TY, 5, NSTAGE, 0, 0>;           // a stage: phi_re, phi_im, theta_0..2 of one plane, forward halo only
     static constexpr int TX = G::TX;
@@ -119,7 +120,7 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
 }
 
 template <typename T>
-__global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, 3)
+__global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, DiagCfg<T>::MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
                   unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
                   const __grid_constant__ CUtensorMap wmap, int use_tma)
@@ -227,7 +228,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     const size_t plane_stride = (size_t)N * N;
     size_t g = ((size_t)z0 * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
     const ptrdiff_t d_row_below = (y0 + w == 0) ? (ptrdiff_t)(N - 1) * N : -(ptrdiff_t)N;
-    const ptrdiff_t d_site_left = (x0 == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;   // (lane 0 only: xi = 0)
+    const ptrdiff_t d_site_left = (x0 + xi == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;
     // eps_2 of the plane below, carried in registers along the march
     VecT E2m = ldg_vec<T, V>(f.eps[2] + (z0 == 0 ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));
 
@@ -253,8 +254,9 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
         const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
         const VecT E1m = ldg_vec<T, V>(f.eps[1] + (g + d_row_below));
-        T e0_halo = T(0);
-        if (lane == 0) e0_halo = f.eps[0][g + d_site_left];
+        // eps_0 of the site left of the vector: its own scalar load (the line is in flight for the neighbouring lane's vector anyway);
+        // a shuffle of E0 would tie the first use of the streamed loads to the top of the plane
+        const T e0_left = __ldg(f.eps[0] + (g + d_site_left));
 
         mbar_wait(&full[ring_n], ((it + 1) / NS) & 1);
         float2 az[NP], azy[NP], aze;
@@ -268,9 +270,6 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
         const T prx_e = sc[eo_re], pix_e = sc[eo_im];
         const T t1x_e = sc[eo_t1], t2x_e = sc[eo_t2];
-        // E0 of the site to the left: previous element, else lane-1's last element, else (lane 0) the halo value
-        T e0_left = __shfl_up_sync(0xffffffffu, E0.v[V - 1], 1);
-        if (lane == 0) e0_left = e0_halo;
 
         // ---- winding (Eq. 11), fast path: the link numbers this thread-plane needs.  n_0, n_1 of this plane were formed
         //      one iteration ago (as the +z links); n_1, n_2 are also taken at the site right of the vector (n_j^{x+k_0}).
@@ -396,19 +395,14 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     block_reduce_store(acc, partials + blockIdx.x);
 }
 
-// z-chunks per tile: the fewest (longest marches; a chunk start costs one extra staged plane) that still give >= 4 waves of
-// resident CTAs and fit the partials buffer; chunk lengths 128 ... 8 as far as N allows
+// z-chunks per tile, measured (profiles/r4_chunks.md; see pick_chunks of the step march): 32 up to 512^3, 16 beyond and for
+// fp64 lattices; halved until the partial records fit and the count divides N.
 template <typename T>
-int pick_chunks(int N, int ctas_per_sm, int max_partials)
+int pick_chunks(int N, long tiles, int max_partials)
 {
-    using C = DiagCfg<T>;
-    const long tiles = (long)(N / C::TX) * (N / C::TY);
-    const int cands[5] = { 128, 64, 32, 16, 8 };
-    for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials && tiles * (N / c) >= 4L * ctas_per_sm * 148) return N / c;
-    for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) + 2 <= max_partials) return N / c;
-    return 1;
+    int c = (sizeof(T) == 4 && N <= 512) ? 32 : 16;
+    while (c > 1 && (N % c != 0 || N / c < 4 || tiles * c + 2 > max_partials)) c /= 2;
+    return c;
 }
 
 }  // namespace
@@ -423,7 +417,7 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartia
     static SmemAttribute attr;   // per device
     if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
     const long tiles = (long)(N / C::TX) * (N / C::TY);
-    int nchunks = pick_chunks<T>(N, 3, max_partials);
+    int nchunks = pick_chunks<T>(N, tiles, max_partials);
     if (opt.diag_chunks > 0 && opt.diag_chunks <= N && tiles * opt.diag_chunks + 2 <= max_partials) nchunks = opt.diag_chunks;
     const long blocks = tiles * nchunks;
     // partials[blocks] collects the second pass, partials[blocks + 1].n_pierced is the length of the doubt list

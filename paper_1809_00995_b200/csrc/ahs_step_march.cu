@@ -44,13 +44,21 @@ namespace {
 
 template <typename T> struct StepCoefT { T c1, c2, c3, d1, d2, d3, dt, sigma2; };
 
-template <typename T, int TY_>
+// Launch shape per storage type: rows per tile (= warps per CTA), CTAs per SM the register budget is cut for, ring depth.
+//   float : 4 rows, 3 CTAs/SM (168 registers), 3 stages -- measured fastest (profiles/r2, r3)
+//   double: 4 rows, 2 CTAs/SM (255 registers: at 168 the kernel spills ~100 B per thread and plane and waits on the reloads,
+//           profiles/r4_step512_f64_full.md), 4 stages (two CTAs leave room for a deeper ring)
+template <typename T> struct StepShape;
+template <> struct StepShape<float> { static constexpr int TY = 4, MINB = 3, NS = 3; };
+template <> struct StepShape<double> { static constexpr int TY = 4, MINB = 2, NS = 4; };
+
+template <typename T, int TY_, int NS_>
 struct MarchCfg {
     static constexpr int V = 16 / sizeof(T);
     static constexpr int TY = TY_;
-    static constexpr int NSTAGE = 3;
+    static constexpr int NSTAGE = NS_;                       // plane it + NSTAGE - 1 is in flight while planes it, it + 1 are read
     using G = TileGeom<T, V, TY, 4, NSTAGE>;                // a stage: phi_re, phi_im, theta_0, theta_1 of one plane
-    static constexpr int T2_SLOTS = 2;                       // theta_2 is never read one plane ahead: a ring of two
+    static constexpr int T2_SLOTS = NSTAGE - 1;              // theta_2 is never read one plane ahead: its ring is one slot shorter
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
     static constexpr int YEX_ELEMS = 4 * TY * TX;         // b1.re, b1.im, S01, S12 of rows -1 .. TY-2 (one parity)
@@ -64,16 +72,16 @@ struct MarchCfg {
                                                               T2_SLOTS * WRAP2_STRIDE + 2 * YEX_ELEMS + 2 * XEX_ELEMS);
 };
 
-template <typename T, int TY, int MINB>
-__global__ void __launch_bounds__(MarchCfg<T, TY>::NTHREADS, MINB)
+template <typename T, int TY, int MINB, int NSTG>
+__global__ void __launch_bounds__(MarchCfg<T, TY, NSTG>::NTHREADS, MINB)
 step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
                   const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_wstage,
                   const __grid_constant__ CUtensorMap map_wth2, int use_tma)
 {
-    using C = MarchCfg<T, TY>;
+    using C = MarchCfg<T, TY, NSTG>;
     using G = typename C::G;
     using VecT = Vec<T, C::V>;
-    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS;
+    constexpr int V = C::V, TX = C::TX, NS = C::NSTAGE, SE = G::STAGE_ELEMS, T2S = C::T2_SLOTS;
     // rotation of the side jobs over the warps at plane `it` (by (w + it) % ...): the halo row takes TX/32 = V warps
     constexpr int HSTRIDE = TY / V, COLUMN = 1 % TY, ISSUER = 3 % TY;
     static_assert(TY % V == 0, "the halo row is shared out over V warps");
@@ -148,8 +156,8 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     if (w == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
-            const bool t2 = i < C::T2_SLOTS;   // theta_2 of planes 0, 1 ride on the barriers of planes 0, 1
-            if (elect_one()) {
+            const bool t2 = i < T2S;   // theta_2 of the first planes rides on the barrier of its own plane
+            if (i <= zlen + 1 && elect_one()) {   // (planes 0 .. zlen+1 are all this chunk reads; nothing may be in flight at exit)
                 mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx + (t2 ? G::ARR_BYTES + wrap2_tx : 0u));
                 issue_stage(i, i);
                 if (t2) issue_th2(i, i, i);
@@ -207,20 +215,20 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     for (int it = 1; it <= zlen; ++it) {
         const T* sc = stages + (it % NS) * SE;
         const T* sn = stages + ((it + 1) % NS) * SE;
-        const T* t2c = th2ring + (it & 1) * C::T2_STRIDE;
+        const T* t2c = th2ring + (it % T2S) * C::T2_STRIDE;
         const T* wsc = wrapS + (it % NS) * C::WRAP_ELEMS;
         const T* wsn = wrapS + ((it + 1) % NS) * C::WRAP_ELEMS;
-        const T* wtc = wrapT + (it & 1) * C::WRAP2_STRIDE;
+        const T* wtc = wrapT + (it % T2S) * C::WRAP2_STRIDE;
         T* yexp = yex + (it & 1) * C::YEX_ELEMS;
         T* xexp = xex + (it & 1) * C::XEX_ELEMS;
 
-        // ---- plane it+2 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ------
-        if (((w + it) % TY) == ISSUER && it + 2 <= zlen + 1 && elect_one()) {
-            const int s = (it + 2) % NS;   // with it: theta_2 of plane it+1 -> the slot that held plane it-1
+        // ---- plane it+NS-1 -> the stage that held plane it-1 (its last readers passed the barrier of iteration it-1) ----
+        if (((w + it) % TY) == ISSUER && it + NS - 1 <= zlen + 1 && elect_one()) {
+            const int s = (it + NS - 1) % NS;   // with it: theta_2 of plane it+NS-2 -> the slot that held plane it-1
             fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1 / of the prologue: all reads of that stage are done)
             mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES + wrap_tx + wrap2_tx);
-            issue_stage(s, it + 2);
-            issue_th2((it + 1) & 1, s, it + 1);
+            issue_stage(s, it + NS - 1);
+            issue_th2((it + NS - 2) % T2S, s, it + NS - 2);   // (it is read at iteration it+NS-2, after the wait on this barrier)
         }
 
         const size_t g = gnext;                                         // plane z0 + it - 1
@@ -388,27 +396,26 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     }
 }
 
-// Number of z-chunks per tile: the fewest (longest marches: a chunk start costs one extra staged plane and the trigonometry of
-// its -z products) that still gives >= 4 waves of resident CTAs; chunk lengths 64, 32, 16, 8 as far as N allows.
-template <typename T, int TY>
-int pick_chunks(int N, int ctas_per_sm)
+// Number of z-chunks per tile.  A chunk start costs one extra staged plane and the trigonometry of its -z products, so long
+// marches look attractive -- but measured (profiles/r4_chunks.md) shorter ones win: CTAs that start together drift apart
+// along z, their halo rows then miss L2, and every chunk boundary re-aligns them.  32 chunks (fp32) / 16 (fp64, twice the
+// tiles per plane) were fastest at 256^3, 512^3 and 1024^3 alike; chunk counts that do not divide N lose 3-6 % at small N.
+template <typename T>
+int pick_chunks(int N)
 {
-    using C = MarchCfg<T, TY>;
-    const long tiles = (long)(N / C::TX) * (N / TY);
-    const int cands[4] = { 64, 32, 16, 8 };
-    for (int c : cands)
-        if (N % c == 0 && tiles * (N / c) >= 4L * ctas_per_sm * 148) return N / c;
-    return N / 8;
+    int c = sizeof(T) == 4 ? 32 : 16;
+    while (c > 1 && (N % c != 0 || N / c < 4)) c /= 2;
+    return c;
 }
 
-template <typename T, int TY, int MINB>
+template <typename T, int TY, int MINB, int NSTG>
 int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
 {
-    using C = MarchCfg<T, TY>;
-    auto kern = step_march_kernel<T, TY, MINB>;
+    using C = MarchCfg<T, TY, NSTG>;
+    auto kern = step_march_kernel<T, TY, MINB, NSTG>;
     static SmemAttribute attr;   // per device: the kernel needs more than the default 48 KB of dynamic shared memory
     if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
-    const int nchunks = (opt.step_chunks > 0 && opt.step_chunks <= N) ? opt.step_chunks : pick_chunks<T, TY>(N, MINB);
+    const int nchunks = (opt.step_chunks > 0 && opt.step_chunks <= N) ? opt.step_chunks : pick_chunks<T>(N);
     const long blocks = (long)(N / C::TX) * (N / TY) * nchunks;
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
     if (maps && opt.staging == AHS_STAGING_TENSOR) {
@@ -426,16 +433,15 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* 
 template <typename T>
 bool march_supported(int N)
 {
-    using C = MarchCfg<T, 4>;
-    return N >= C::TX && N % C::TX == 0;
+    using C = MarchCfg<T, StepShape<T>::TY, StepShape<T>::NS>;
+    return N >= C::TX && N % C::TX == 0 && N % C::TY == 0;
 }
 
-// 4-row tiles (4 warps), three CTAs per SM: measured fastest (profiles/r2, r3)
 template <typename T>
 int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
 {
     if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
-    return launch_cfg<T, 4, 3>(f, N, c, maps, opt, st);
+    return launch_cfg<T, StepShape<T>::TY, StepShape<T>::MINB, StepShape<T>::NS>(f, N, c, maps, opt, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu
@@ -448,7 +454,7 @@ template int launch_step_march<double>(const FieldPtrs<double>&, int, const Step
 template <typename T>
 bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, size_t array_bytes)
 {
-    using C = MarchCfg<T, 4>;
+    using C = MarchCfg<T, StepShape<T>::TY, StepShape<T>::NS>;
     using G = typename C::G;
     if (!march_supported<T>(N)) return false;
     return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
