@@ -3,8 +3,8 @@
 //
 // Same tile and staging as the step kernel (ahs_step_march.cu): a CTA owns TX x TY sites in (x, y) and marches over a
 // z-chunk; phi_re, phi_im, theta_0..2 of plane k+3 are streamed by the copy engine (one tensor-map TMA copy per plane, row
-// copies on the periodic edge in y) into a 4-stage ring of halo'd shared-memory tiles (full / empty mbarrier pairs) while
-// planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
+// copies on the periodic edge in y) into a 4-stage ring of halo'd shared-memory tiles (one `full` mbarrier per stage; the last
+// warp to finish with a stage re-fills it) while planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
 // All the estimators need only FORWARD neighbours (x+k_i, x+k_i+k_j) of phi, theta -- except the divergence of eps,
 // whose -x / -y / -z terms come by shuffle, one extra row load and a carried register.
 //
@@ -14,7 +14,7 @@
 //
 // Winding.  Every thread evaluates arg phi / 2 pi (branch-free atan2_turns) at the ten points of plane k+1 its V sites need
 // and carries them to the next plane in registers; there is NO exchange between warps and therefore no CTA barrier in the
-// march: the warps of a CTA drift freely and meet only at the stage ring's full / empty mbarriers (an earlier version
+// march: the warps of a CTA drift freely and meet only at the stage ring's `full` mbarriers (an earlier version
 // computed each phase once into a shared arg tile and lost 31 % of its issue slots at the per-plane barrier, profiles/r2).
 // The link numbers n_i^x = rint(t), t = arg^{x+k_i}/2pi - arg^x/2pi - theta_i^x/2pi, are formed in fp32 and
 // W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x) is summed exactly.  The decision is the fp64 one:
@@ -133,7 +133,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
-    uint64_t* empty = full + NS;                           // empty[s]: all TY warps have finished reading stage s
+    unsigned* released = reinterpret_cast<unsigned*>(full + NS);   // released[s]: how many of the TY warps have finished reading stage s
     T* stages = reinterpret_cast<T*>(smem + 128);          // ring slot s at stages + s SE: the stage, then (right-edge tiles under
                                                            // TMA) the side buffer of the wrapped column at + STAGE_STRIDE
 
@@ -155,7 +155,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
 
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], TY); }
+        for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); released[s] = 0u; }
         mbar_fence_init();
     }
     __syncthreads();
@@ -185,7 +185,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     const int eo_t1 = edge_off(3, w), eo_t2 = edge_off(4, w);
     if (w == 0 && elect_one()) {
 #pragma unroll
-        for (int p = 0; p < NS - 1; ++p)
+        for (int p = 0; p < NS; ++p)
             if (p <= zlen) issue_plane(p, p);
     }
 
@@ -242,14 +242,6 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     for (int it = 0; it < zlen; ++it) {
         const int ring_n = ring + 1 == NS ? 0 : ring + 1;
         const T* sn = ring_n ? sc + SE : stages;
-
-        // plane it+3 -> the stage that held plane it-1, once all TY warps have released it (the issuing warp rotates)
-        static_assert(TY == NS, "the issuing warp rotates with the ring");
-        if (w == ring && it + NS - 1 <= zlen && elect_one()) {
-            const int s = ring == 0 ? NS - 1 : ring - 1;   // (it + NS - 1) % NS
-            if (it > 0) mbar_wait(&empty[s], ((it - 1) / NS) & 1);
-            issue_plane(s, it + NS - 1);
-        }
 
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
         const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
@@ -382,9 +374,23 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
             nonfinite += bad ? 1u : 0u;
         }
         E2m = E2;
-        // this warp is done with stage `sc` (plane it): release it to the copy-issuing thread
+        // This warp is done with stage `ring` (plane it).  The LAST of the TY warps to say so re-fills it with plane it + NS: nobody
+        // ever waits for a stage to become free.  (An earlier version let a rotating warp spin on an `empty` mbarrier before issuing:
+        // its elected lane and its 31 siblings then ran the rest of the plane as two groups, every instruction issued twice, and a
+        // __syncwarp() there made the whole warp wait instead -- profiles/r4_diag1024_f32_full.md.)  The acq_rel counter orders all
+        // warps' reads of the stage before the last one's fence.proxy.async and copy.
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[ring]);
+        if (lane == 0) {
+            unsigned before;
+            asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(before) : "r"(smem_u32(&released[ring])) : "memory");
+            if (before == TY - 1) {
+                released[ring] = 0u;
+                if (it + NS <= zlen) {
+                    fence_proxy_async();
+                    issue_plane(ring, it + NS);
+                }
+            }
+        }
         sc = sn;
         ring = ring_n;
         g += plane_stride;
