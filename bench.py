@@ -9,8 +9,9 @@ Gauss residual) whose record is read back.  Default K = 10 -> the config's 500-s
 by rank 0 follows the driver's contract; see DESIGN.md "Measurement" for every field.
 
   value       site-updates/s, whole job, state resident in HBM, CUDA events on the handle's stream, max over ranks
-  e2e         same metric through the C ABI with HOST buffers: ahs_set_fields_native (H2D of the 10 fields from pinned
-              memory) + the same step + ahs_get_fields_native of ... the diagnostics record (D2H), all inside the timing
+  e2e         same metric through the C ABI with HOST buffers: ahs_set_fields_native_async (H2D of the 10 fields from pinned
+              memory) + the same step + the diagnostics record read back (D2H), all inside the timing; two handles alternate so
+              that one step's upload overlaps the other's evolution
   roofline    step kernel: 80 B (fp32) / 160 B (fp64) per site per launch / average launch duration (events around the
               back-to-back launches of each step), against MEASURED_PEAKS.json hbm_gbs
   cpu_baseline  the fp64 oracle (oracle/, test infrastructure) as it stands on this box's host cores, bounded sample
@@ -60,7 +61,7 @@ def parse_args():
     ap.add_argument("--tau-ref", type=float, default=0.0, help="a = (tau/tau_ref)^m; 0 = tau0 (DESIGN.md R3: s != 0 runs leave the "
                     "stability region after ~80 steps at m=1 unless tau_ref is the end time)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "march"])
-    ap.add_argument("--e2e-steps", type=int, default=2, help="timed end-to-end steps (each uploads the full state)")
+    ap.add_argument("--e2e-steps", type=int, default=4, help="timed end-to-end steps (each uploads the full state)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-lattice", type=int, default=128, help="lattice of the oracle's bounded sample")
@@ -320,8 +321,11 @@ def run_ours(args):
 
 
 def run_e2e(args, sim, torch, max_over_ranks, barrier, world):
-    """The same step through the C ABI with HOST buffers: every timed step uploads the 10 fields from pinned memory
-    (ahs_set_fields_native), runs L leapfrog launches + diagnostics and reads the diagnostics record back."""
+    """The same step through the C ABI with HOST buffers: every timed step uploads its 10 input fields from pinned host memory
+    (ahs_set_fields_native_async), runs L leapfrog launches + diagnostics and reads the diagnostics record back to the host.
+    With room for a second lattice in HBM the steps alternate between two handles on two streams, so the upload of step k+1
+    overlaps the evolution of step k (an input pipeline through the public API); otherwise they run back to back on one handle."""
+    from paper_1809_00995_b200 import binding as ahs
     N, L, E = args.lattice, args.leapfrog, max(1, args.e2e_steps)
     sites = N ** 3
     tdtype = torch.float32 if args.precision == "f32" else torch.float64
@@ -333,28 +337,47 @@ def run_e2e(args, sim, torch, max_over_ranks, barrier, world):
     sim.get_fields_native(host.data_ptr())            # the resident state, downloaded once (untimed)
     h2d = host.numel() * host.element_size()
     import ctypes
-    d2h = ctypes.sizeof(__import__("paper_1809_00995_b200.binding", fromlist=["ahs_diag"]).ahs_diag)
+    d2h = ctypes.sizeof(ahs.ahs_diag)
 
-    def one():
-        sim.set_fields_native(host.data_ptr(), step=n0)
-        sim.step(L)
-        return sim.diagnostics()
+    sims = [sim]
+    free, _ = torch.cuda.mem_get_info()
+    if free > ahs.required_bytes(N, args.precision) + (4 << 30):
+        with torch.cuda.stream(torch.cuda.Stream()):
+            sims.append(ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, ic="none", kernel=args.kernel,
+                                       tau_ref=args.tau_ref, **COMMON))
 
-    one()                                             # warm-up
+    def submit(k):
+        sm = sims[k % len(sims)]
+        sm.set_fields_native(host.data_ptr(), step=n0, wait=False)   # H2D of this step's inputs, asynchronous on the handle's stream
+        sm.step(L)
+        sm.diagnostics_launch()
+
+    def collect(k):
+        return sims[k % len(sims)].diagnostics_fetch()               # D2H of the record; synchronises that handle's stream
+
+    def run(n):
+        submit(0)
+        for k in range(1, n):
+            submit(k)
+            collect(k - 1)
+        return collect(n - 1)
+
+    run(len(sims))                                    # warm-up on every handle
     barrier()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     w0 = time.perf_counter()
-    a.record()
-    for _ in range(E):
-        one()
-    b.record()
-    barrier()
+    last = run(E)
+    torch.cuda.synchronize()
     wall = time.perf_counter() - w0
-    ms = max_over_ranks(max(a.elapsed_time(b), 0.0))
+    barrier()
+    ms = max_over_ranks(1e3 * wall)                   # host clock between two device synchronisations: the copies are part of it
+    for sm in sims[1:]:
+        sm.destroy()
     del host
     return {"value": world * sites * L * E / (ms * 1e-3), "unit": "site-updates/s", "h2d_bytes_per_step": h2d,
-            "d2h_bytes_per_step": d2h, "steps": E, "ms_per_step": ms / E, "wall_ms_per_step": 1e3 * wall / E,
-            "what": "ahs_set_fields_native (pinned host -> HBM) + %d x ahs_step + ahs_diagnostics_ex (record -> host) per step" % L}
+            "d2h_bytes_per_step": d2h, "steps": E, "ms_per_step": ms / E, "handles": len(sims), "n_pierced_last": int(last["n_pierced"]),
+            "what": "per step: ahs_set_fields_native_async (pinned host -> HBM) + %d x ahs_step + ahs_diagnostics_launch/_fetch (record -> host); "
+                    "%s" % (L, "two handles on two streams, upload of one step overlapping the evolution of the other"
+                            if len(sims) == 2 else "one handle, back to back (no room for a second lattice)")}
 
 
 def main():

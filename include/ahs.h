@@ -162,6 +162,11 @@ AHS_API int32_t ahs_set_fields(ahs_sim* sim, const double* host10, int64_t step)
  * the copies run at PCIe speed. */
 AHS_API int32_t ahs_get_fields_native(ahs_sim* sim, void* host10);
 AHS_API int32_t ahs_set_fields_native(ahs_sim* sim, const void* host10, int64_t step);
+/* The same upload without the final synchronise: the ten copies are enqueued on the handle's stream and the call returns; later
+ * work of the handle (ahs_step, diagnostics) is ordered behind them.  host10 (HOST, pinned for a truly asynchronous copy) must stay
+ * valid and unchanged until a synchronising call of this handle has returned.  With two handles on two streams the upload of one
+ * state overlaps the evolution of the other (bench.py's end-to-end leg). */
+AHS_API int32_t ahs_set_fields_native_async(ahs_sim* sim, const void* host10, int64_t step);
 
 /* DEVICE pointer to live field k (0..9, order above) in the storage type; valid until the next ahs_step
  * (phi and theta alternate between two buffers).  For zero-copy views from PyTorch. */

@@ -27,7 +27,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "theta_0", "theta_1", "thet
 SYMBOLS = (
     "ahs_required_bytes", "ahs_create", "ahs_create_ex", "ahs_step", "ahs_diagnostics", "ahs_diagnostics_ex",
     "ahs_diagnostics_launch", "ahs_diagnostics_fetch", "ahs_get_fields", "ahs_set_fields", "ahs_get_fields_native",
-    "ahs_set_fields_native", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_coefficients",
+    "ahs_set_fields_native", "ahs_set_fields_native_async", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_coefficients",
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
 )
 
@@ -77,6 +77,7 @@ def load(path: str | None = None):
     lib.ahs_set_fields.argtypes = [vp, vp, i64]; lib.ahs_set_fields.restype = i32
     lib.ahs_get_fields_native.argtypes = [vp, vp]; lib.ahs_get_fields_native.restype = i32
     lib.ahs_set_fields_native.argtypes = [vp, vp, i64]; lib.ahs_set_fields_native.restype = i32
+    lib.ahs_set_fields_native_async.argtypes = [vp, vp, i64]; lib.ahs_set_fields_native_async.restype = i32
     lib.ahs_field_device_ptr.argtypes = [vp, i32, C.POINTER(vp)]; lib.ahs_field_device_ptr.restype = i32
     lib.ahs_get_state.argtypes = [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64)]; lib.ahs_get_state.restype = i32
     lib.ahs_kernel_kind.argtypes = [vp]; lib.ahs_kernel_kind.restype = i32
@@ -218,9 +219,12 @@ class Simulation:
         _check(load().ahs_get_fields_native(self._h, ptr))
         return out
 
-    def set_fields_native(self, src, step: int = 0):
+    def set_fields_native(self, src, step: int = 0, wait: bool = True):
+        """Upload a snapshot in the storage type.  wait=False: ahs_set_fields_native_async (the caller keeps `src` alive and
+        unchanged until a synchronising call of this handle has returned)."""
         ptr = src if isinstance(src, int) else src.ctypes.data
-        _check(load().ahs_set_fields_native(self._h, ptr, int(step)))
+        lib = load()
+        _check((lib.ahs_set_fields_native if wait else lib.ahs_set_fields_native_async)(self._h, ptr, int(step)))
 
     def field_device_ptr(self, k: int) -> int:
         p = C.c_void_p()

@@ -395,7 +395,7 @@ int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
     return AHS_OK;
 }
 
-int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
+int32_t ahs_set_fields_native_async(ahs_sim* s, const void* host10, int64_t step)
 {
     AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
@@ -404,8 +404,15 @@ int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
     for (int k = 0; k < 10; ++k)
         AHS_CUDA(cudaMemcpyAsync(s->base + (size_t)live_slot(s, k) * s->array_bytes, (const char*)host10 + (size_t)k * bytes, bytes,
                                  cudaMemcpyHostToDevice, s->stream));
-    AHS_CUDA(cudaStreamSynchronize(s->stream));
     s->step = step;
+    return AHS_OK;
+}
+
+int32_t ahs_set_fields_native(ahs_sim* s, const void* host10, int64_t step)
+{
+    if (int r = ahs_set_fields_native_async(s, host10, step)) return r;
+    AHS_ENTER(s);
+    AHS_CUDA(cudaStreamSynchronize(s->stream));
     return AHS_OK;
 }
 

@@ -374,6 +374,14 @@ def test_native_transfer_and_device_pointers(ahs):
         assert np.array_equal(pinned.numpy(), a)
         sim.set_fields_native(pinned.data_ptr(), step=3)
         assert np.array_equal(sim.get_fields_native(), a)
+        sim.step(1)
+        sim.set_fields_native(pinned.data_ptr(), step=3, wait=False)      # ahs_set_fields_native_async: ordered on the handle's stream
+        sim.step(2)
+        b = sim.get_fields_native()
+        sim.set_fields_native(a, step=3)
+        sim.step(2)
+        assert sim.step_count == 5 and np.array_equal(sim.get_fields_native(), b)
+        sim.set_fields_native(a, step=3)
         ptr = sim.field_device_ptr(0)
         assert ptr != 0 and ptr % 256 == 0
         st, tau, nl = sim.state()
@@ -513,6 +521,27 @@ def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
             out.append((hashlib.md5(sim.get_fields_native().tobytes()).hexdigest(), d["n_pierced"], d["v2_num"], d["gauss_max"]))
             assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"]), d
     assert out[0] == out[1]
+
+
+def test_chunk_starts_under_stress_are_bit_identical(ahs):
+    """The hand-over of the prologue's stages to the copy engine at every z-chunk start (profiles/r2_race.md): 1000 launches at
+    256^3 with 128 chunks per tile -- a chunk start every second plane, 3.4e7 hand-overs per run, 64 x the default shape's -- in both
+    staging modes.  A stage overwritten while a slower warp still reads it corrupts a site; the fields must instead equal the
+    default launch shape's bit for bit (they do not depend on where the chunk boundaries fall) and Gauss's law must hold."""
+    import hashlib
+    N, nsteps = 256, 1000
+    digests = {}
+    for name, opts in (("default", {}), ("128 chunks, tensor maps", {ahs.AHS_OPT_STEP_CHUNKS: 128}),
+                       ("128 chunks, row copies", {ahs.AHS_OPT_STEP_CHUNKS: 128, ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS}),
+                       ("85 chunks (uneven), tensor maps", {ahs.AHS_OPT_STEP_CHUNKS: 85})):
+        with ahs.Simulation(N=N, precision="f32", m=1.0, s=0.0, seed=180900995) as sim:
+            for k, v in opts.items():
+                sim.set_option(k, v)
+            sim.step(nsteps)
+            d = sim.diagnostics()
+            assert d["nonfinite"] == 0 and d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"]), (name, d)
+            digests[name] = (hashlib.md5(sim.get_fields_native().tobytes()).hexdigest(), d["n_pierced"])
+    assert len(set(digests.values())) == 1, digests
 
 
 def test_c_B_parameter_reaches_the_weight(ahs, oracle):
