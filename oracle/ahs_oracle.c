@@ -68,6 +68,8 @@ typedef struct {
     double tau0;      /* conformal time of step 0                                               */
     double tau_ref;   /* a(tau) = (tau/tau_ref)^m ; normalisation not given in the paper (R3)   */
     double c_B;       /* factor on the plaquette sum of Eq. 2; 1 = consistent with Eq. 5 (R2)   */
+    double c_E;       /* factor on the electric term of Eq. 2 IN THE WEIGHT; 1 = eps = d theta/d eta (R5);
+                         (dt/dx)^2 = the rescaling "E -> e dt E" of L44 read literally (R21)          */
 } aho_params;
 
 typedef struct {
@@ -87,6 +89,9 @@ typedef struct {
     double v2v_den;           /* sum_x |D phi|^2 * Vp                                           */
     double v2_V;              /* 2R/(1+R), R = v2v_num / v2v_den (Eq. 9)                        */
     double xi_L;              /* sqrt(-mu / mean Lag), mu = 2 pi sigma^2 (Eq. 9; R20); NaN if mean Lag >= 0 */
+    double eos_num;           /* sum_x p^x Lag^x    (Eq. 12: Lagrangian-weighted pressure; p, rho per R22)      */
+    double eos_den;           /* sum_x rho^x Lag^x                                                              */
+    double v2_omega;          /* (1 + 3 eos_num / eos_den) / 2   (Eq. 12)                               */
 } aho_diag;
 
 static const double AHO_TWO_PI  = 6.283185307179586476925286766559;
@@ -397,12 +402,15 @@ void aho_winding(const aho_params* p, const double* f10, int32_t* W3, uint64_t* 
  *   G^x   = (1/dx^2) sum_i |U_i^x phi^{x+k_i} - phi^x|^2                                 (|D phi|^2)
  *   K^x   = |Pi^x|^2
  *   Vp^x  = (a^2 lambda(a)/4) (|phi^x|^2 - sigma^2)^2
- *   Lag^x = [ sum_i eps_i^2 - (c_B/dx^2) sum_i sum_{j!=i} (1 - cos Xi_ij^x) ] / (2 e(a)^2 a^2 dx^2) + K - G - Vp
- * out4 = {K, G, Lag, Vp}.  Vp is also the weight of the potential-weighted estimator <v^2>_V (L86);
+ *   El^x  = sum_i eps_i^2 / (2 e(a)^2 a^2 dx^2),  Bm^x = sum_i sum_{j!=i} (1 - cos Xi_ij^x) / (2 e(a)^2 a^2 dx^4)
+ *   Lag^x = c_E El - c_B Bm + K - G - Vp          (c_E = c_B = 1: the Lagrangian whose variation is Eqs. 4-7)
+ * out6 = {K, G, Lag, Vp, El, Bm}.  Vp is also the weight of the potential-weighted estimator <v^2>_V (L86);
  * a constant factor on a weight drops out of R, so its a^2 lambda(a)/4 prefactor is immaterial there.
+ * El and Bm (always with unit factors) are the electric and magnetic energy densities of the equation-of-state
+ * estimator, Eq. 12.
  * -------------------------------------------------------------------------------------------- */
 static void aho_site_lagrangian(const aho_params* p, const double* f10, double a,
-                                int64_t x, int64_t y, int64_t z, double out4[4])
+                                int64_t x, int64_t y, int64_t z, double out6[6])
 {
     const int64_t N = p->N, V = N * N * N;
     const double q = (double)p->q;
@@ -434,8 +442,9 @@ static void aho_site_lagrangian(const aho_params* p, const double* f10, double a
             mag += 1.0 - cos(aho_plaq(N, th, x, y, z, i, j));   /* ordered pairs (R12) */
         }
     }
-    const double gauge = (e2 - p->c_B * idx2 * mag) / (2.0 * ea * ea * a * a * p->dx * p->dx);
-    out4[0] = K; out4[1] = G; out4[2] = gauge + K - G - Vp; out4[3] = Vp;
+    const double gn = 1.0 / (2.0 * ea * ea * a * a * p->dx * p->dx);
+    const double El = gn * e2, Bm = gn * idx2 * mag;
+    out6[0] = K; out6[1] = G; out6[2] = (p->c_E * El - p->c_B * Bm) + K - G - Vp; out6[3] = Vp; out6[4] = El; out6[5] = Bm;
 }
 
 /* ----------------------------------------------------------------------------------------------
@@ -445,6 +454,10 @@ static void aho_site_lagrangian(const aho_params* p, const double* f10, double a
  *   <v^2>_V : the same with the potential Vp as the weight (L86: "two different weight functions")
  *   xi_L = sqrt(-mu / mean Lag) (Eq. 9); the paper does not give mu: mu = 2 pi sigma^2, the Bogomolnyi
  *          string tension at lambda = 2 e^2 (the paper's couplings, L72) -- a labelled assumption (R20)
+ *   <v^2>_omega = (1 + 3 p_L / rho_L) / 2 (Eq. 12), p_L / rho_L = sum p Lag / sum rho Lag with the energy density and
+ *          pressure of the model -- the paper takes them from Hindmarsh et al. (2017a), which is not in the container; these
+ *          are the standard ones, a labelled assumption (R22):
+ *            rho = K + G + Vp + El + Bm,   p = K - G/3 - Vp + (El + Bm)/3
  *   Gauss residual (L72, L181; derived from Eqs. 4-7, R4), a_h = a(tau_n - dt/2):
  *     g^x = sum_i (eps_i^x - eps_i^{x-k_i}) - 2 q dx^2 e0^2 a_h^(2s) Im[conj(phi^x) Pi^x]
  * Sums are accumulated in fp64: x-fastest within a z-plane, then the plane sums in z order.
@@ -476,20 +489,26 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
     const double ah = aho_a(p, tau - 0.5 * p->dt);
     const double grhs = 2.0 * q * p->dx * p->dx * p->e0 * p->e0 * pow(ah, 2.0 * p->s);
     /* per z-plane sums in x-fastest order (planes are independent), then the planes added in z order */
-    double* plane = (double*)malloc((size_t)N * 7 * sizeof(double));
+    double* plane = (double*)malloc((size_t)N * 9 * sizeof(double));
 #pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z) {
-        double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+        double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0, wnum = 0.0, wden = 0.0;
         for (int64_t y = 0; y < N; ++y)
         for (int64_t x = 0; x < N; ++x) {
             const int64_t s0 = x + N * (y + N * z);
-            double kgl[4];
+            double kgl[6];
             aho_site_lagrangian(p, f10, a, x, y, z, kgl);
             num  += kgl[0] * kgl[2];
             den  += kgl[1] * kgl[2];
             lsum += kgl[2];
             vnum += kgl[0] * kgl[3];
             vden += kgl[1] * kgl[3];
+            {   /* Eq. 12: pressure and energy density, weighted with the Lagrangian */
+                const double rho = kgl[0] + kgl[1] + kgl[3] + kgl[4] + kgl[5];
+                const double prs = kgl[0] - kgl[1] / 3.0 - kgl[3] + (kgl[4] + kgl[5]) / 3.0;
+                wnum += prs * kgl[2];
+                wden += rho * kgl[2];
+            }
             double div = 0.0;
             for (int i = 0; i < 3; ++i) div += eps[i][s0] - eps[i][aho_nb(N, x, y, z, i, -1)];
             const double rhs = grhs * (phr[s0] * pii[s0] - phi_[s0] * pir[s0]);
@@ -497,13 +516,13 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
             if (g > gmax || g != g) gmax = g;
             rhs2 += rhs * rhs;
         }
-        double* o = plane + 7 * z;
-        o[0] = num; o[1] = den; o[2] = lsum; o[3] = gmax; o[4] = rhs2; o[5] = vnum; o[6] = vden;
+        double* o = plane + 9 * z;
+        o[0] = num; o[1] = den; o[2] = lsum; o[3] = gmax; o[4] = rhs2; o[5] = vnum; o[6] = vden; o[7] = wnum; o[8] = wden;
     }
-    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+    double num = 0.0, den = 0.0, lsum = 0.0, gmax = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0, wnum = 0.0, wden = 0.0;
     for (int64_t z = 0; z < N; ++z) {
-        const double* o = plane + 7 * z;
-        num += o[0]; den += o[1]; lsum += o[2]; rhs2 += o[4]; vnum += o[5]; vden += o[6];
+        const double* o = plane + 9 * z;
+        num += o[0]; den += o[1]; lsum += o[2]; rhs2 += o[4]; vnum += o[5]; vden += o[6]; wnum += o[7]; wden += o[8];
         if (o[3] > gmax || o[3] != o[3]) gmax = o[3];
     }
     free(plane);
@@ -521,6 +540,9 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
         out->v2_V = 2.0 * R / (1.0 + R);
     }
     out->xi_L = sqrt(-(AHO_TWO_PI * p->sigma * p->sigma) / out->mean_lagrangian);
+    out->eos_num = wnum;
+    out->eos_den = wden;
+    out->v2_omega = 0.5 * (1.0 + 3.0 * wnum / wden);
     out->gauss_max = gmax;
     out->gauss_rhs_rms = sqrt(rhs2 / (double)V);
 }
@@ -534,11 +556,26 @@ void aho_site_fields4(const aho_params* p, const double* f10, int64_t n, double*
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
-        double kgl[4];
+        double kgl[6];
         aho_site_lagrangian(p, f10, a, x, y, z, kgl);
         const int64_t s0 = x + N * (y + N * z);
         K[s0] = kgl[0]; G[s0] = kgl[1]; Lag[s0] = kgl[2];
         if (Vp) Vp[s0] = kgl[3];
+    }
+}
+/* the electric and magnetic energy densities El, Bm (each N^3) as well */
+void aho_site_fields6(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag, double* Vp, double* El, double* Bm)
+{
+    const int64_t N = p->N;
+    const double a = aho_a(p, aho_tau(p, n));
+#pragma omp parallel for num_threads(aho_threads) schedule(static)
+    for (int64_t z = 0; z < N; ++z)
+    for (int64_t y = 0; y < N; ++y)
+    for (int64_t x = 0; x < N; ++x) {
+        double kgl[6];
+        aho_site_lagrangian(p, f10, a, x, y, z, kgl);
+        const int64_t s0 = x + N * (y + N * z);
+        K[s0] = kgl[0]; G[s0] = kgl[1]; Lag[s0] = kgl[2]; Vp[s0] = kgl[3]; El[s0] = kgl[4]; Bm[s0] = kgl[5];
     }
 }
 void aho_site_fields(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag)

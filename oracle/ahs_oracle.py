@@ -41,7 +41,7 @@ def build(force: bool = False) -> str:
 class _Params(C.Structure):
     _fields_ = [("N", C.c_int32), ("q", C.c_int32), ("dx", C.c_double), ("dt", C.c_double),
                 ("lambda0", C.c_double), ("e0", C.c_double), ("sigma", C.c_double), ("m", C.c_double),
-                ("s", C.c_double), ("tau0", C.c_double), ("tau_ref", C.c_double), ("c_B", C.c_double)]
+                ("s", C.c_double), ("tau0", C.c_double), ("tau_ref", C.c_double), ("c_B", C.c_double), ("c_E", C.c_double)]
 
 
 class _Diag(C.Structure):
@@ -49,7 +49,8 @@ class _Diag(C.Structure):
                 ("v2_num", C.c_double), ("v2_den", C.c_double), ("v2", C.c_double),
                 ("mean_lagrangian", C.c_double), ("gauss_max", C.c_double), ("gauss_rhs_rms", C.c_double),
                 ("nonfinite", C.c_int32), ("pad_", C.c_int32),
-                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double)]
+                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double),
+                ("eos_num", C.c_double), ("eos_den", C.c_double), ("v2_omega", C.c_double)]
 
 
 @dataclass
@@ -67,11 +68,12 @@ class Params:
     tau_ref: float = 0.0   # 0 => tau0
     q: int = 1
     c_B: float = 1.0
+    c_E: float = 1.0      # factor on the electric term in the weight; (dt/dx)^2 = L44's "E -> e dt E" read literally (R21)
 
     def _c(self) -> _Params:
         tref = self.tau_ref if self.tau_ref != 0.0 else self.tau0
         return _Params(self.N, self.q, self.dx, self.dt, self.lambda0, self.e0, self.sigma, self.m,
-                       self.s, self.tau0, tref, self.c_B)
+                       self.s, self.tau0, tref, self.c_B, self.c_E)
 
 
 _lib = None
@@ -92,8 +94,9 @@ def lib():
         _lib.aho_diag_compute.argtypes = [C.POINTER(_Params), dp, C.c_int64, C.POINTER(_Diag)]
         _lib.aho_site_fields.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp]
         _lib.aho_site_fields4.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp, dp]
+        _lib.aho_site_fields6.argtypes = [C.POINTER(_Params), dp, C.c_int64, dp, dp, dp, dp, dp, dp]
         for f in ("aho_philox4x32_10", "aho_ic", "aho_ic_window", "aho_coeffs", "aho_step", "aho_winding",
-                  "aho_diag_compute", "aho_site_fields", "aho_site_fields4"):
+                  "aho_diag_compute", "aho_site_fields", "aho_site_fields4", "aho_site_fields6"):
             getattr(_lib, f).restype = None
         _lib.aho_set_threads.argtypes = [C.c_int32]
         _lib.aho_set_threads.restype = C.c_int32
@@ -184,6 +187,14 @@ def site_fields4(p: Params, f10: np.ndarray, n: int):
     K = np.empty((p.N,) * 3); G = np.empty((p.N,) * 3); L = np.empty((p.N,) * 3); Vp = np.empty((p.N,) * 3)
     lib().aho_site_fields4(C.byref(p._c()), _dptr(f10), n, _dptr(K), _dptr(G), _dptr(L), _dptr(Vp))
     return K, G, L, Vp
+
+
+def site_fields6(p: Params, f10: np.ndarray, n: int):
+    """Per-site K, G, Lag, Vp and the electric / magnetic energy densities El, Bm (unit factors), each of shape (N, N, N)."""
+    _check_f10(p, f10)
+    out = [np.empty((p.N,) * 3) for _ in range(6)]
+    lib().aho_site_fields6(C.byref(p._c()), _dptr(f10), n, *[_dptr(a) for a in out])
+    return tuple(out)
 
 
 def params_dict(p: Params) -> dict:

@@ -827,3 +827,78 @@ def test_oracle_is_independent_of_the_thread_count(oracle):
     assert d["v2_num"] == pytest.approx(float((K * Lg).sum()), rel=1e-12)
     assert d["v2_den"] == pytest.approx(float((G * Lg).sum()), rel=1e-12)
     assert d["mean_lagrangian"] == pytest.approx(float(Lg.mean()), rel=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3, first half: the equation-of-state estimator of Eq. 12, and the c_E factor of the weight (R21, R22)
+# ------------------------------------------------------------------------------------------------
+def test_equation_of_state_estimator(oracle):
+    """<v^2>_omega = (1 + 3 p_L/rho_L)/2 (Eq. 12) with rho = K + G + V + El + Bm, p = K - G/3 - V + (El + Bm)/3.
+    (1) A Lorentz-boosted kink of the model's own potential (a domain wall: phi real, phi = sigma tanh(gamma x / w), w =
+        2/(sqrt(lambda) sigma), which obeys the Bogomolnyi relation |phi'|^2 = V pointwise) has the equation of state of a wall,
+        p/rho = v^2 - 2/3, for ANY weight: the estimator must read (3 v^2 - 1)/2.  Catches a wrong 1/3, a wrong sign on G or V,
+        K or G entering with another factor.  The lattice derivative makes it approximate: dx = w/10, tolerance 0.002.
+    (2) Uniform configurations in closed form, with a(tau) != 1 and s != 0, 1: phi = 0 with a uniform electric field and a uniform
+        magnetic flux (theta_0 = beta y, seam consistent mod 2 pi): rho = V + El + Bm, p = -V + (El + Bm)/3, whatever c_E, c_B are
+        (the weight is uniform and drops out) while mean_lagrangian = c_E El - c_B Bm - V pins both factors.
+    (3) The per-site electric and magnetic energy densities against the vectorised numpy evaluation of Eq. 2's pieces, and the
+        two new sums against sums over those arrays; gauge invariance."""
+    # ---- (1) boosted kink / antikink pair along x ------------------------------------------------------------------
+    N, lam, sigma, v = 96, 8.0, 1.0, 0.6
+    w = 2.0 / (math.sqrt(lam) * sigma)
+    dx = w / 10
+    gam = 1.0 / math.sqrt(1 - v * v)
+    p = oracle.Params(N=N, m=0, s=1, dx=dx, lambda0=lam, sigma=sigma, e0=1.0)
+    x = (np.arange(N) * dx)[None, None, :] * np.ones((N, N, 1))
+    Lbox = N * dx
+    u1, u2 = gam * (x - 0.25 * Lbox) / w, gam * (x - 0.75 * Lbox) / w
+    prof = sigma * (np.tanh(u1) - np.tanh(u2) - 1.0)                         # kink at L/4, antikink at 3L/4, periodic up to e^-2L/4w
+    dprof = sigma * gam / w * (1 / np.cosh(u1) ** 2 - 1 / np.cosh(u2) ** 2)   # d phi / dx
+    zero = np.zeros((N, N, N))
+    d = oracle.diagnostics(p, pack(prof + 0j, -v * dprof + 0j, [zero] * 3, [zero] * 3), 0)   # phi(x - v t): Pi = -v d_x phi
+    assert d["v2_omega"] == pytest.approx((3 * v * v - 1) / 2, abs=0.002)     # (observed 0.03996 vs 0.04; G/3 -> G gives -0.46,
+    assert d["v2"] == pytest.approx(2 * v * v / (1 + v * v), rel=0.002)       #  dropping V 0.52, doubling K 0.31)       # (the R estimator on the same wall: R = v^2)
+    # teeth: the same wall at rest reads -1/2, i.e. p = -(2/3) rho
+    d0 = oracle.diagnostics(p, pack(sigma * (np.tanh(u1 / gam) - np.tanh(u2 / gam) - 1.0) + 0j, zero + 0j, [zero] * 3, [zero] * 3), 0)
+    assert d0["v2_omega"] == pytest.approx(-0.5, abs=0.002)
+
+    # ---- (2) uniform electric field and magnetic flux on phi = 0 ------------------------------------------------------
+    N = 8
+    n = 6
+    one = np.ones((N, N, N))
+    y = np.arange(N)[None, :, None] * one
+    beta, c = TWO_PI / N, (0.3, -0.2, 0.5)
+    f = pack(0j * one, 0j * one, [beta * y, 0 * one, 0 * one], [ci * one for ci in c])
+    for cE, cB in ((1.0, 1.0), (0.04, 0.5)):
+        q = oracle.Params(N=N, m=1, s=0.5, dx=0.5, lambda0=1.7, e0=0.9, sigma=1.1, tau0=1.0, tau_ref=0.5, c_E=cE, c_B=cB)
+        a = (q.tau0 + n * q.dt) / 0.5
+        e2a2 = q.e0 ** 2 * a ** (2 * q.s)
+        El = sum(ci * ci for ci in c) / (2 * e2a2 * q.dx ** 2)
+        Bm = 2 * (1 - math.cos(beta)) / (2 * e2a2 * q.dx ** 4)                # ordered pairs (0,1), (1,0)
+        V = q.lambda0 * a ** (2 * q.s) / 4 * q.sigma ** 4
+        d = oracle.diagnostics(q, f, n)
+        assert d["mean_lagrangian"] == pytest.approx(cE * El - cB * Bm - V, rel=1e-13)
+        assert d["eos_num"] / d["eos_den"] == pytest.approx((-V + (El + Bm) / 3) / (V + El + Bm), rel=1e-12)
+        assert d["v2_omega"] == pytest.approx(0.5 * (1 + 3 * (-V + (El + Bm) / 3) / (V + El + Bm)), rel=1e-12)
+
+    # ---- (3) evolved state: per-site pieces and sums against numpy; gauge invariance ------------------------------------
+    q = oracle.Params(N=12, m=2, s=0.5, e0=0.9, lambda0=1.7, dx=0.6, sigma=1.2, c_E=0.3)
+    f = oracle.initial_condition(q, seed=8)
+    oracle.step(q, f, 0, 25)
+    phi, Pi, th, eps = unpack(f)
+    a = a_of(q, q.tau0 + 25 * q.dt)
+    ea2 = q.e0 ** 2 * a ** (2 * q.s)
+    El_np = sum(e ** 2 for e in eps) / (2 * ea2 * q.dx ** 2)
+    Bm_np = sum(1 - np.cos(np_plaq(th, i, j)) for i in range(3) for j in range(3) if i != j) / (2 * ea2 * q.dx ** 4)
+    K, G, Lag, Vp, El, Bm = oracle.site_fields6(q, f, 25)
+    assert np.abs(El - El_np).max() < 1e-12 * El_np.max() and np.abs(Bm - Bm_np).max() < 1e-12 * Bm_np.max()
+    assert np.abs(Lag - (q.c_E * El_np - q.c_B * Bm_np + K - G - Vp)).max() < 1e-11 * np.abs(Lag).max()
+    rho, prs = K + G + Vp + El_np + Bm_np, K - G / 3 - Vp + (El_np + Bm_np) / 3
+    d = oracle.diagnostics(q, f, 25)
+    assert d["eos_num"] == pytest.approx((prs * Lag).sum(), rel=1e-11) and d["eos_den"] == pytest.approx((rho * Lag).sum(), rel=1e-11)
+    rng = np.random.default_rng(12)
+    alpha = rng.uniform(-10, 10, (12, 12, 12))
+    f2 = pack(np.exp(1j * alpha) * phi, np.exp(1j * alpha) * Pi, [th[i] + (sh(alpha, i, 1) - alpha) for i in range(3)], eps)
+    d2 = oracle.diagnostics(q, f2, 25)
+    for key in ("eos_num", "eos_den", "v2_omega", "v2_num"):
+        assert d[key] == pytest.approx(d2[key], rel=1e-10)
