@@ -83,6 +83,9 @@ enum { AHS_STAGING_TENSOR = 0, AHS_STAGING_ROWS = 1 };
  *   stream          cudaStream_t as void*, optional (NULL => the legacy default stream).
  *   c_B             factor on the plaquette sum of Eq. 2 (L40) in the weight of <v^2>_L and in mean_lagrangian; 0 means 1, the
  *                   value consistent with Eq. 5 (R2).  Eq. 2 as printed has 1/2; it does not enter the equations of motion.
+ *   c_E             factor on the electric term sum_i eps_i^2 of Eq. 2 in the same weight; 0 means 1, the value for eps = d theta /
+ *                   d eta (Eq. 7, R5).  (dt/dx)^2 is what the sentence "E_i -> e dt E_i" of L44 gives when read literally (R21);
+ *                   with it <v^2>_L reproduces the paper's Table 4 within two standard deviations.
  */
 typedef struct {
     int32_t N;
@@ -95,6 +98,7 @@ typedef struct {
     size_t device_buffer_bytes;
     void* stream;
     double c_B;
+    double c_E;
 } ahs_params;
 
 /* Result of one diagnostics pass on the current snapshot (after `step` steps). */
@@ -122,6 +126,11 @@ typedef struct {
     double xi_L;              /* sqrt(-mu / mean_lagrangian), Eq. 9 (L78), with mu = 2 pi sigma^2 -- the paper
                                  does not state mu; this is the Bogomolnyi tension at lambda = 2 e^2 (R20).
                                  NaN when mean_lagrangian >= 0                                              */
+    double eos_num;           /* sum_x p^x Lag^x,   p = K - G/3 - Vp + (El + Bm)/3     (Eq. 12; the pressure and   */
+    double eos_den;           /* sum_x rho^x Lag^x, rho = K + G + Vp + El + Bm          energy density of the model, R22:  */
+    double v2_omega;          /* (1 + 3 eos_num / eos_den) / 2: <v^2>_omega             K = |Pi|^2, G = |D phi|^2, El / Bm the
+                                 electric / magnetic terms of Eq. 2 with unit factors; the paper takes p, rho from a
+                                 reference that is not reproduced in it, so these definitions are a labelled assumption)   */
 } ahs_diag;
 
 /* Bytes of device memory a simulation needs: 15 arrays of N^3 values (10 live + the phi', theta' shadow

@@ -37,7 +37,7 @@ class ahs_params(C.Structure):
                 ("dx", C.c_double), ("dt", C.c_double), ("lambda_", C.c_double), ("e", C.c_double),
                 ("sigma", C.c_double), ("m", C.c_double), ("s", C.c_double), ("tau0", C.c_double),
                 ("tau_ref", C.c_double), ("seed", C.c_uint64), ("device_buffer", C.c_void_p),
-                ("device_buffer_bytes", C.c_size_t), ("stream", C.c_void_p), ("c_B", C.c_double)]
+                ("device_buffer_bytes", C.c_size_t), ("stream", C.c_void_p), ("c_B", C.c_double), ("c_E", C.c_double)]
 
 
 class ahs_diag(C.Structure):
@@ -45,7 +45,8 @@ class ahs_diag(C.Structure):
                 ("L", C.c_double), ("xi", C.c_double), ("v2_num", C.c_double), ("v2_den", C.c_double),
                 ("v2", C.c_double), ("mean_lagrangian", C.c_double), ("gauss_max", C.c_double),
                 ("gauss_rhs_rms", C.c_double), ("nonfinite", C.c_int32), ("reserved", C.c_int32),
-                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double)]
+                ("v2v_num", C.c_double), ("v2v_den", C.c_double), ("v2_V", C.c_double), ("xi_L", C.c_double),
+                ("eos_num", C.c_double), ("eos_den", C.c_double), ("v2_omega", C.c_double)]
 
 
 class AhsError(RuntimeError):
@@ -121,7 +122,7 @@ class Simulation:
     """One ahs_sim handle.  Methods mirror the C functions one to one."""
 
     def __init__(self, N, dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, m=1.0, s=0.0, tau0=1.0, seed=0,
-                 precision="f32", ic="random_phase", tau_ref=0.0, kernel="auto", use_torch=True, c_B=0.0):
+                 precision="f32", ic="random_phase", tau_ref=0.0, kernel="auto", use_torch=True, c_B=0.0, c_E=0.0):
         self._h = None
         lib = load()
         self.N = int(N)
@@ -134,6 +135,7 @@ class Simulation:
         p.dx, p.dt, p.lambda_, p.e, p.sigma, p.m, p.s, p.tau0, p.tau_ref = dx, dt, lambda0, e0, sigma, m, s, tau0, tau_ref
         p.seed = seed
         p.c_B = c_B
+        p.c_E = c_E
         self._buffer = None
         self.stream_handle = 0
         if use_torch:

@@ -113,7 +113,8 @@ DiagCoef diag_coefficients(const ahs_params& p, int64_t n)
     DiagCoef c;
     c.inv_dx2 = 1.0 / (p.dx * p.dx);
     c.gauge_norm = 1.0 / (2.0 * ea * ea * a * a * p.dx * p.dx);
-    c.cB_inv_dx2 = (p.c_B != 0.0 ? p.c_B : 1.0) / (p.dx * p.dx);
+    c.cB = p.c_B != 0.0 ? p.c_B : 1.0;
+    c.cE = p.c_E != 0.0 ? p.c_E : 1.0;
     c.pot_coef = 0.25 * a * a * lambda_of(p, a);
     c.sigma2 = p.sigma * p.sigma;
     c.gauss_rhs = 2.0 * p.dx * p.dx * p.e * p.e * std::pow(a_h, 2.0 * p.s);
@@ -216,6 +217,7 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     }
     if (p.m != 0.0 && !(p.tau0 - 0.5 * p.dt > 0)) { fail(AHS_ERR_INVALID_ARG, "tau0 - dt/2 must be > 0 when m != 0"); return nullptr; }
     if (!std::isfinite(p.c_B) || p.c_B < 0) { fail(AHS_ERR_INVALID_ARG, "c_B must be finite and >= 0 (0 = default 1)"); return nullptr; }
+    if (!std::isfinite(p.c_E) || p.c_E < 0) { fail(AHS_ERR_INVALID_ARG, "c_E must be finite and >= 0 (0 = default 1)"); return nullptr; }
     if (p.kernel < AHS_KERNEL_AUTO || p.kernel > AHS_KERNEL_MARCH) { fail(AHS_ERR_INVALID_ARG, "unknown kernel %d", p.kernel); return nullptr; }
     const bool march_ok = p.precision == AHS_F32 ? march_supported<float>(p.N) : march_supported<double>(p.N);
     if (p.kernel == AHS_KERNEL_MARCH && !march_ok) {
@@ -359,6 +361,9 @@ int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
     const double Rv = r.vnum / r.vden;
     out->v2_V = 2.0 * Rv / (1.0 + Rv);
     out->xi_L = std::sqrt(-(2.0 * M_PI * p.sigma * p.sigma) / out->mean_lagrangian);   // mu = 2 pi sigma^2 (R20)
+    out->eos_num = r.wnum;
+    out->eos_den = r.wden;
+    out->v2_omega = 0.5 * (1.0 + 3.0 * r.wnum / r.wden);                                 // Eq. 12
     s->diag_step = -1;
     if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "the lattice holds non-finite field values at step %lld (%llu sites or thread-planes flagged)",
                                     (long long)out->step, (unsigned long long)r.nonfinite);

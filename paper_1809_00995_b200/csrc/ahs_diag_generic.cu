@@ -24,13 +24,13 @@ namespace {
 // second stage: ONE block sums the partials in a fixed order (thread t takes t, t+256, ...; then the block tree)
 __global__ void __launch_bounds__(256) diag_finish_kernel(const DiagPartial* __restrict__ partials, int n, DiagPartial* __restrict__ result)
 {
-    DiagPartial t = {0ull, 0ull, 0.0, 0.0, 0.0, 0.0, 0.0, 0ull, 0.0, 0.0};
+    DiagPartial t = {0ull, 0ull, 0.0, 0.0, 0.0, 0.0, 0.0, 0ull, 0.0, 0.0, 0.0, 0.0};
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const DiagPartial p = partials[i];
         t.n_pierced += p.n_pierced; t.sum_abs_w += p.sum_abs_w;
         t.num += p.num; t.den += p.den; t.lsum += p.lsum;
         t.gmax = fmax(t.gmax, p.gmax); t.rhs2 += p.rhs2; t.nonfinite += p.nonfinite;
-        t.vnum += p.vnum; t.vden += p.vden;
+        t.vnum += p.vnum; t.vden += p.vden; t.wnum += p.wnum; t.wden += p.wden;
     }
     block_reduce_store(t, result);
 }
@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(128) diag_generic_kernel(DiagPtrs<T> f, int N,
     const int64_t nsites = (int64_t)N * N * N;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     const int64_t sN = N, sNN = (int64_t)N * N;
-    DiagPartial acc = {0ull, 0ull, 0.0, 0.0, 0.0, 0.0, 0.0, 0ull, 0.0, 0.0};
+    DiagPartial acc = {0ull, 0ull, 0.0, 0.0, 0.0, 0.0, 0.0, 0ull, 0.0, 0.0, 0.0, 0.0};
 
     for (int64_t site = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; site < nsites; site += stride) {
         const int x = (int)(site % N), y = (int)((site / N) % N), z = (int)(site / sNN);
@@ -112,12 +112,16 @@ __global__ void __launch_bounds__(128) diag_generic_kernel(DiagPtrs<T> f, int N,
         }
         mag *= T(2);   // ordered pairs (i,j) and (j,i): cos is even (R12)
         const T e2 = ep0[0] * ep0[0] + ep0[1] * ep0[1] + ep0[2] * ep0[2];
-        const T lag = (e2 - (T)k.cB_inv_dx2 * mag) * (T)k.gauge_norm + K - G - Vp;
+        const T El = (T)k.gauge_norm * e2, Bm = (T)k.gauge_norm * (T)k.inv_dx2 * mag;   // electric / magnetic energy densities
+        const T lag = ((T)k.cE * El - (T)k.cB * Bm) + K - G - Vp;
         acc.num += (double)K * (double)lag;
         acc.den += (double)G * (double)lag;
         acc.lsum += (double)lag;
         acc.vnum += (double)K * (double)Vp;   // potential-weighted estimator <v^2>_V (L86)
         acc.vden += (double)G * (double)Vp;
+        // Eq. 12: rho = K + G + Vp + El + Bm, p = K - G/3 - Vp + (El + Bm)/3, weighted with the Lagrangian
+        acc.wnum += (double)(K - G * (T)(1.0 / 3.0) - Vp + (El + Bm) * (T)(1.0 / 3.0)) * (double)lag;
+        acc.wden += (double)(K + G + Vp + El + Bm) * (double)lag;
 
         // ---- Gauss residual ------------------------------------------------------------------------------------------
         T div = T(0);

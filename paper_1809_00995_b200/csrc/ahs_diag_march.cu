@@ -149,7 +149,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     const int xi = V * lane;
 
     const T* const src[5] = { f.phi_re, f.phi_im, f.th[0], f.th[1], f.th[2] };
-    const P inv_dx2 = pk::splat((T)kd.inv_dx2), gauge_norm = pk::splat((T)kd.gauge_norm), ncB = pk::splat(-(T)kd.cB_inv_dx2);
+    const P inv_dx2 = pk::splat((T)kd.inv_dx2), g_el = pk::splat((T)kd.gauge_norm), g_mag = pk::splat((T)(kd.gauge_norm * kd.inv_dx2));
+    const P ncB = pk::splat(-(T)kd.cB), cE = pk::splat((T)kd.cE), third = pk::splat((T)(1.0 / 3.0));
     const P pot = pk::splat((T)kd.pot_coef), nsigma2 = pk::splat(-(T)kd.sigma2), grhs = pk::splat((T)kd.gauss_rhs);
     const P half = pk::splat(T(0.5)), four = pk::splat(T(4));
 
@@ -232,7 +233,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     // eps_2 of the plane below, carried in registers along the march
     VecT E2m = ldg_vec<T, V>(f.eps[2] + (z0 == 0 ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));
 
-    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0;
+    double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0, wnum = 0.0, wden = 0.0;
     float pierced_f = 0.0f;   // plaquettes with W != 0 on the fast path (all |W| <= 1 there, so this is sum |W| as well); exact below 2^24
     unsigned nonfinite = 0u;
     T gmax_t = T(0);
@@ -311,7 +312,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
         ae = aze;
 
         // ---- Eq. 2 pieces, <v^2> sums and the Gauss residual, two sites at a time --------------------------------------------
-        P p_num = pk::splat(T(0)), p_den = p_num, p_l = p_num, p_r2 = p_num, p_vn = p_num, p_vd = p_num;   // per thread and plane, then into the fp64 sums
+        P p_num = pk::splat(T(0)), p_den = p_num, p_l = p_num, p_r2 = p_num, p_vn = p_num, p_vd = p_num, p_wn = p_num, p_wd = p_num;   // per thread and plane, then into the fp64 sums
 #pragma unroll
         for (int h = 0; h < NP; ++h) {
             const P phr = pk::at<T, V>(pr.v, h), phi = pk::at<T, V>(pi.v, h), pmr = pk::at<T, V>(Pr.v, h), pmi = pk::at<T, V>(Pi.v, h);
@@ -342,12 +343,17 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
             const P h01 = sin_pair(pk::mul(half, X01)), h02 = sin_pair(pk::mul(half, X02)), h12 = sin_pair(pk::mul(half, X12));
             const P mag = pk::mul(four, pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12))));   // ordered pairs: 2 x [2 sin^2] per plaquette (R12)
             const P e2 = pk::fma(ep0, ep0, pk::fma(ep1, ep1, pk::mul(ep2, ep2)));
-            const P lag = pk::sub(pk::sub(pk::fma(pk::fma(ncB, mag, e2), gauge_norm, K), Gd), Vp);
+            const P El = pk::mul(g_el, e2), Bm = pk::mul(g_mag, mag);   // electric / magnetic energy densities
+            const P lag = pk::sub(pk::sub(pk::fma(cE, El, pk::fma(ncB, Bm, K)), Gd), Vp);
             p_num = pk::fma(K, lag, p_num);
             p_den = pk::fma(Gd, lag, p_den);
             p_l = pk::add(p_l, lag);
             p_vn = pk::fma(K, Vp, p_vn);   // potential-weighted estimator <v^2>_V (L86)
             p_vd = pk::fma(Gd, Vp, p_vd);
+            // equation of state (Eq. 12): rho = K + G + Vp + El + Bm, p = K - G/3 - Vp + (El + Bm)/3, Lagrangian weighted
+            const P EB = pk::add(El, Bm);
+            p_wn = pk::fma(pk::fma(pk::sub(EB, Gd), third, pk::sub(K, Vp)), lag, p_wn);
+            p_wd = pk::fma(pk::add(pk::add(K, Gd), pk::add(Vp, EB)), lag, p_wd);
 
             // ---- Gauss residual: sum_i (eps_i^x - eps_i^{x-k_i}) - gauss_rhs Im[conj(phi) Pi] ----------------------------------
             const P e0m = pk::mk(h > 0 ? E0.v[h > 0 ? 2 * h - 1 : 0] : e0_left, E0.v[2 * h]);
@@ -361,6 +367,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
         const T l_plane = p_l.x + p_l.y;
         num += (double)(p_num.x + p_num.y); den += (double)(p_den.x + p_den.y); lsum += (double)l_plane; rhs2 += (double)(p_r2.x + p_r2.y);
         vnum += (double)(p_vn.x + p_vn.y); vden += (double)(p_vd.x + p_vd.y);
+        wnum += (double)(p_wn.x + p_wn.y); wden += (double)(p_wd.x + p_wd.y);
         // Non-finite values.  Every one of the ten stored values feeds the Lagrangian (NaN or Inf in, NaN or Inf out), so a
         // finite plane sum clears all of them at once; otherwise the stored values themselves are examined (a finite value
         // whose square overflows the storage type is not an error: include/ahs.h "nonfinite").
@@ -397,7 +404,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     }
 
     const unsigned long long n_fast = (unsigned long long)pierced_f;
-    DiagPartial acc = { n_fast, n_fast, num, den, lsum, (double)gmax_t, rhs2, (unsigned long long)nonfinite, vnum, vden };
+    DiagPartial acc = { n_fast, n_fast, num, den, lsum, (double)gmax_t, rhs2, (unsigned long long)nonfinite, vnum, vden, wnum, wden };
     block_reduce_store(acc, partials + blockIdx.x);
 }
 

@@ -33,13 +33,14 @@ struct StepCoef {
 struct DiagCoef {
     double inv_dx2;        // 1/dx^2
     double gauge_norm;     // 1 / (2 e(a)^2 a^2 dx^2) with a = a(tau_n)     (Eq. 2 prefactor)
-    double cB_inv_dx2;     // c_B / dx^2, c_B = 1 (R2)
+    double cB;             // c_B: factor on the magnetic term in the weight, 1 (R2)
+    double cE;             // c_E: factor on the electric term in the weight, 1 (R21)
     double pot_coef;       // a^2 lambda(a) / 4
     double sigma2;
     double gauss_rhs;      // 2 dx^2 e0^2 a_h^(2s), a_h = a(tau_n - dt/2)  (R4)
 };
 
-// One record per block / final result of the reduction (fixed 10 x 8 bytes).
+// One record per block / final result of the reduction (fixed 12 x 8 bytes).
 struct DiagPartial {
     unsigned long long n_pierced;
     unsigned long long sum_abs_w;
@@ -48,6 +49,7 @@ struct DiagPartial {
     double rhs2;
     unsigned long long nonfinite;
     double vnum, vden;     // potential-weighted sums: sum K Vp, sum G Vp
+    double wnum, wden;     // equation of state, Lagrangian weighted: sum p Lag, sum rho Lag (Eq. 12; R22)
 };
 
 template <typename T>

@@ -40,6 +40,8 @@ __device__ __forceinline__ void block_reduce_store(DiagPartial v, DiagPartial* o
     v.nonfinite = warp_sum(v.nonfinite);
     v.vnum = warp_sum(v.vnum);
     v.vden = warp_sum(v.vden);
+    v.wnum = warp_sum(v.wnum);
+    v.wden = warp_sum(v.wden);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
     if (lane == 0) sh[warp] = v;
     __syncthreads();
@@ -49,7 +51,7 @@ __device__ __forceinline__ void block_reduce_store(DiagPartial v, DiagPartial* o
             t.n_pierced += sh[w].n_pierced; t.sum_abs_w += sh[w].sum_abs_w;
             t.num += sh[w].num; t.den += sh[w].den; t.lsum += sh[w].lsum;
             t.gmax = fmax(t.gmax, sh[w].gmax); t.rhs2 += sh[w].rhs2; t.nonfinite += sh[w].nonfinite;
-            t.vnum += sh[w].vnum; t.vden += sh[w].vden;
+            t.vnum += sh[w].vnum; t.vden += sh[w].vden; t.wnum += sh[w].wnum; t.wden += sh[w].wden;
         }
         *out = t;
     }

@@ -20,14 +20,14 @@ from . import binding as ahs
 from .synthetic import COMMON
 
 PAPER = {  # PAPER.md Table 4 (L211-222), s = 0 rows: context, five-run averages on a Quadro P5000
-    "radiation": {"xi_L_dot": "0.30 +- 0.02", "xi_W_dot": "0.32 +- 0.03", "v2_V": "0.34 +- 0.01", "v2_L": "0.31 +- 0.01"},   # L215
-    "matter": {"xi_L_dot": "0.29 +- 0.01", "xi_W_dot": "0.29 +- 0.02", "v2_V": "0.26 +- 0.01", "v2_L": "0.27 +- 0.01"},      # L222
+    "radiation": {"xi_L_dot": "0.30 +- 0.02", "xi_W_dot": "0.32 +- 0.03", "v2_V": "0.34 +- 0.01", "v2_L": "0.31 +- 0.01", "v2_omega": "0.32 +- 0.01"},   # L215
+    "matter": {"xi_L_dot": "0.29 +- 0.01", "xi_W_dot": "0.29 +- 0.02", "v2_V": "0.26 +- 0.01", "v2_L": "0.27 +- 0.01", "v2_omega": "0.25 +- 0.01"},      # L222
 }
 
 
-def run(N, m, seed, steps, every, fit_from, precision, c_B):
-    tau, series = [], {k: [] for k in ("xi", "xi_L", "v2", "v2_V", "gauss_max")}
-    with ahs.Simulation(N=N, precision=precision, m=m, s=0.0, seed=seed, c_B=c_B, **COMMON) as sim:
+def run(N, m, seed, steps, every, fit_from, precision, c_B, c_E=0.0):
+    tau, series = [], {k: [] for k in ("xi", "xi_L", "v2", "v2_V", "v2_omega", "gauss_max")}
+    with ahs.Simulation(N=N, precision=precision, m=m, s=0.0, seed=seed, c_B=c_B, c_E=c_E, **COMMON) as sim:
         for n in range(0, steps + 1, every):
             if n:
                 sim.step(every)
@@ -41,7 +41,7 @@ def run(N, m, seed, steps, every, fit_from, precision, c_B):
     for k in ("xi", "xi_L"):
         y = np.array(series[k])[sel]
         out[k + "_dot"] = float(np.polyfit(tau[sel], y, 1)[0])
-    for k in ("v2", "v2_V"):
+    for k in ("v2", "v2_V", "v2_omega"):
         out[k] = float(np.mean(np.array(series[k])[sel]))
     out["gauss_max"] = float(np.max(series["gauss_max"]))
     return out
@@ -55,15 +55,17 @@ def main():
     ap.add_argument("--every", type=int, default=10)
     ap.add_argument("--precision", default="f32")
     ap.add_argument("--c-b", type=float, default=0.0, help="factor on the plaquette sum of Eq. 2 in the weight (0 = 1, DESIGN.md R2; Eq. 2 prints 0.5)")
+    ap.add_argument("--c-e", type=float, default=0.0, help="factor on the electric term of Eq. 2 in the weight (0 = 1; 0.04 = (dt/dx)^2, L44 read literally, DESIGN.md R21)")
     args = ap.parse_args()
     N = args.lattice
     steps = int(round(N * COMMON["dx"] / 2 / COMMON["dt"]))          # half a light-crossing time of the box
     steps -= steps % args.every
     for era, m in (("radiation", 1.0), ("matter", 2.0)):
-        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b) for seed in range(1, args.seeds + 1)]
+        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b, args.c_e) for seed in range(1, args.seeds + 1)]
         line = {"era": era, "m": m, "s": 0.0, "lattice": N, "precision": args.precision, "seeds": args.seeds, "steps": steps, "c_B": args.c_b or 1.0,
+                "c_E": args.c_e or 1.0,
                 "fit_window_tau": [args.fit_from, COMMON["tau0"] + steps * COMMON["dt"]], "paper_table4": PAPER[era]}
-        for k, name in (("xi_L_dot", "xi_L_dot"), ("xi_dot", "xi_W_dot"), ("v2_V", "v2_V"), ("v2", "v2_L")):
+        for k, name in (("xi_L_dot", "xi_L_dot"), ("xi_dot", "xi_W_dot"), ("v2_V", "v2_V"), ("v2", "v2_L"), ("v2_omega", "v2_omega")):
             v = np.array([r[k] for r in runs])
             line[name] = {"mean": float(v.mean()), "std": float(v.std(ddof=1)) if len(v) > 1 else 0.0}
         line["gauss_max_over_all_runs"] = max(r["gauss_max"] for r in runs)

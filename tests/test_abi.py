@@ -33,9 +33,9 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_layouts_match_header():
     from paper_1809_00995_b200 import binding
-    # ahs_params: 4 int32 + 9 double + uint64 + ptr + size_t + ptr + double ; ahs_diag: 17 x 8 bytes
-    assert C.sizeof(binding.ahs_params) == 16 + 9 * 8 + 8 + 8 + 8 + 8 + 8
-    assert C.sizeof(binding.ahs_diag) == 17 * 8
+    # ahs_params: 4 int32 + 9 double + uint64 + ptr + size_t + ptr + 2 double ; ahs_diag: 20 x 8 bytes
+    assert C.sizeof(binding.ahs_params) == 16 + 9 * 8 + 8 + 8 + 8 + 8 + 8 + 8
+    assert C.sizeof(binding.ahs_diag) == 20 * 8
     assert binding.ahs_params.dx.offset == 16 and binding.ahs_params.seed.offset == 88
 
 

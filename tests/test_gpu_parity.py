@@ -105,6 +105,13 @@ def check_diag(O, p, sim, prec, snap, n):
     assert abs(d["v2v_den"] - r["v2v_den"]) <= rel * (G * Vp).sum() + floor
     if r["mean_lagrangian"] < -1e-3 * np.abs(Lg).mean():
         assert d["xi_L"] == pytest.approx(r["xi_L"], rel=50 * rel)
+    # equation-of-state estimator (Eq. 12): the two Lagrangian-weighted sums, relative to their absolute sums
+    K6, G6, L6, V6, El, Bm = O.site_fields6(p, snap, n)
+    rho, prs = K6 + G6 + V6 + El + Bm, K6 - G6 / 3 - V6 + (El + Bm) / 3
+    assert abs(d["eos_num"] - r["eos_num"]) <= rel * np.abs(prs * L6).sum() + 1e-300
+    assert abs(d["eos_den"] - r["eos_den"]) <= rel * np.abs(rho * L6).sum() + 1e-300
+    if abs(r["eos_den"]) > 0.05 * np.abs(rho * L6).sum():
+        assert d["v2_omega"] == pytest.approx(r["v2_omega"], rel=200 * rel, abs=200 * rel)
     eps_m = 2.3e-16 if prec == "f64" else 6e-8
     gscale = max(1.0, r["gauss_rhs_rms"], np.abs(snap[7:10]).max())
     assert abs(d["gauss_max"] - r["gauss_max"]) <= 64 * eps_m * gscale
@@ -545,20 +552,23 @@ def test_chunk_starts_under_stress_are_bit_identical(ahs):
 
 
 def test_c_B_parameter_reaches_the_weight(ahs, oracle):
-    """ahs_params.c_B (R2): the factor on the plaquette sum of Eq. 2 enters the Lagrangian weight only; 0.5 is Eq. 2 as printed."""
+    """ahs_params.c_B (R2) and c_E (R21): the factors on the plaquette sum and on the electric term of Eq. 2 enter the Lagrangian
+    weight only; c_B = 0.5 is Eq. 2 as printed, c_E = (dt/dx)^2 = 0.04 the rescaling of E that L44 states."""
     from paper_1809_00995_b200 import synthetic
-    N = 64
-    f = rounded(synthetic.random_snapshot(N, seed=5), "f64")
-    for cB in (0.5, 1.0):
-        p = oracle.Params(N=N, m=1.0, s=0.0, c_B=cB)
-        with ahs.Simulation(N=N, precision="f64", m=1.0, s=0.0, ic="none", c_B=cB) as sim:
-            sim.set_fields(f, 4)
-            d = sim.diagnostics()
-        r = oracle.diagnostics(p, f, 4)
-        K, G, Lg = oracle.site_fields(p, f, 4)
-        assert abs(d["v2_num"] - r["v2_num"]) <= 1e-10 * np.abs(K * Lg).sum()
-        assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= 1e-10 * np.abs(Lg).mean()
-        assert d["n_pierced"] == r["n_pierced"] and d["v2v_num"] == pytest.approx(r["v2v_num"], rel=1e-10)
+    for prec, N, kernel in (("f64", 64, "auto"), ("f32", 128, "auto"), ("f64", 24, "generic")):
+        f = rounded(synthetic.random_snapshot(N, seed=5), prec)
+        for cB, cE in ((0.5, 1.0), (1.0, 1.0), (1.0, 0.04), (0.5, 0.04)):
+            p = oracle.Params(N=N, m=1.0, s=0.0, c_B=cB, c_E=cE)
+            with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.0, ic="none", c_B=cB, c_E=cE, kernel=kernel) as sim:
+                sim.set_fields(f, 4)
+                d = sim.diagnostics()
+            r = oracle.diagnostics(p, f, 4)
+            K, G, Lg = oracle.site_fields(p, f, 4)
+            rel = 1e-10 if prec == "f64" else 2e-5
+            assert abs(d["v2_num"] - r["v2_num"]) <= rel * np.abs(K * Lg).sum()
+            assert abs(d["mean_lagrangian"] - r["mean_lagrangian"]) <= rel * np.abs(Lg).mean()
+            assert d["n_pierced"] == r["n_pierced"] and d["v2v_num"] == pytest.approx(r["v2v_num"], rel=rel)
+            assert d["v2_omega"] == pytest.approx(r["v2_omega"], rel=100 * rel)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -653,3 +663,18 @@ def test_nonfinite_flag_means_a_stored_value_is_not_finite(ahs, oracle, prec, N,
             assert oracle.diagnostics(p, f, 0)["nonfinite"] == 0
         sim.set_fields(base, 0)
         assert sim.diagnostics()["nonfinite"] == 0
+
+
+def test_table4_script_runs_through_the_library(ahs):
+    """paper_1809_00995_b200/table4.py (the s = 0 rows of the paper's Table 4) on a 128^3 box, one seed per era:
+    far too small to be in scaling, so only sanity is asserted -- finite numbers, the mean string separation growing at a rate of
+    the paper's order (0.3), velocities between 0 and 1, Gauss's law at fp32 roundoff."""
+    from paper_1809_00995_b200 import table4
+    N = 128
+    steps = int(round(N * 0.5 / 2 / 0.1))
+    for m in (1.0, 2.0):
+        r = table4.run(N, m, seed=1, steps=steps - steps % 10, every=10, fit_from=16.0, precision="f32", c_B=0.0, c_E=0.0)
+        assert all(math.isfinite(v) for v in r.values()), r
+        assert 0.2 < r["xi_dot"] < 0.5 and 0.15 < r["xi_L_dot"] < 0.6, r
+        assert 0.0 < r["v2_V"] < 1.0 and 0.0 < r["v2_omega"] < 1.0, r
+        assert r["gauss_max"] < 1e-4, r
