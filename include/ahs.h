@@ -207,6 +207,34 @@ AHS_API int32_t ahs_synchronize(ahs_sim* sim);
 /* Free the handle and the device memory the library allocated. NULL is allowed. */
 AHS_API int32_t ahs_destroy(ahs_sim* sim);
 
+/*
+ * ---- z-slab decomposition: one lattice on several handles / GPUs of this process -------------------------------------------
+ * The paper's stated next step (L252-258: "extending to multiple GPUs").  The N^3 lattice is cut into nslabs slabs of N / nslabs
+ * z-planes; each slab is a handle with one ghost plane below and above (15 arrays of N x N x (N/nslabs + 2) values) on
+ * devices[r] (HOST array of nslabs CUDA device ordinals; NULL = the current device for all; ordinals may repeat, so the path can
+ * be exercised on one GPU).  The halo exchange is part of the fused step kernel: besides its own arrays it stores the new phi,
+ * theta (Eqs. 6-7) of its bottom / top plane -- and eps_2 of the top plane, which the Gauss residual of the slab above needs --
+ * into the neighbouring slabs' ghost planes, through peer memory (NVLink) when they live on another GPU: 5 N^2 values per face and
+ * step.  CUDA events order step n+1 of a slab behind step n of its two neighbours; nothing waits on the device.  Results are those
+ * of a single handle: fields bit for bit, counts exactly, sums to the rounding order of the final reduction.
+ * params: as for ahs_create_ex with device_buffer = stream = NULL and N % 128 == 0 (fp32) / N % 64 == 0 (fp64); nslabs in 1..64
+ * must divide N.  Slabs on different devices need peer access between neighbours.  One host thread drives a group.
+ */
+typedef struct ahs_group ahs_group;
+AHS_API ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int32_t* devices /* HOST, may be NULL */);
+AHS_API int32_t ahs_group_step(ahs_group* group, int32_t n);                         /* asynchronous, like ahs_step */
+AHS_API int32_t ahs_group_diagnostics(ahs_group* group, ahs_diag* out /* HOST */);   /* every slab's pass, combined; synchronises */
+/* The whole lattice in the storage type, 10 N^3 values in the field order above, gathered from / scattered to the slabs (HOST
+ * pointers; ahs_group_set_fields_native also sets the step counter and fills the ghost planes).  Synchronise. */
+AHS_API int32_t ahs_group_get_fields_native(ahs_group* group, void* host10);
+AHS_API int32_t ahs_group_set_fields_native(ahs_group* group, const void* host10, int64_t step);
+AHS_API int32_t ahs_group_synchronize(ahs_group* group);
+AHS_API int32_t ahs_group_slab_count(ahs_group* group);
+/* The handle of slab r (owned by the group: for ahs_set_option, ahs_get_state, ahs_kernel_kind; its fields are read and written
+ * through the group).  NULL if r is out of range. */
+AHS_API ahs_sim* ahs_group_slab(ahs_group* group, int32_t r);
+AHS_API int32_t ahs_group_destroy(ahs_group* group);                                 /* NULL is allowed */
+
 /* Message of the last failure on this thread ("" if none). Never NULL. */
 AHS_API const char* ahs_last_error(void);
 

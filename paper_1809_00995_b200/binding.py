@@ -29,6 +29,8 @@ SYMBOLS = (
     "ahs_diagnostics_launch", "ahs_diagnostics_fetch", "ahs_get_fields", "ahs_set_fields", "ahs_get_fields_native",
     "ahs_set_fields_native", "ahs_set_fields_native_async", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_coefficients",
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
+    "ahs_group_create", "ahs_group_step", "ahs_group_diagnostics", "ahs_group_get_fields_native", "ahs_group_set_fields_native",
+    "ahs_group_synchronize", "ahs_group_slab_count", "ahs_group_slab", "ahs_group_destroy",
 )
 
 
@@ -88,6 +90,15 @@ def load(path: str | None = None):
     lib.ahs_destroy.argtypes = [vp]; lib.ahs_destroy.restype = i32
     lib.ahs_last_error.argtypes = []; lib.ahs_last_error.restype = C.c_char_p
     lib.ahs_version.argtypes = []; lib.ahs_version.restype = C.c_char_p
+    lib.ahs_group_create.argtypes = [C.POINTER(ahs_params), i32, C.POINTER(i32)]; lib.ahs_group_create.restype = vp
+    lib.ahs_group_step.argtypes = [vp, i32]; lib.ahs_group_step.restype = i32
+    lib.ahs_group_diagnostics.argtypes = [vp, C.POINTER(ahs_diag)]; lib.ahs_group_diagnostics.restype = i32
+    lib.ahs_group_get_fields_native.argtypes = [vp, vp]; lib.ahs_group_get_fields_native.restype = i32
+    lib.ahs_group_set_fields_native.argtypes = [vp, vp, i64]; lib.ahs_group_set_fields_native.restype = i32
+    lib.ahs_group_synchronize.argtypes = [vp]; lib.ahs_group_synchronize.restype = i32
+    lib.ahs_group_slab_count.argtypes = [vp]; lib.ahs_group_slab_count.restype = i32
+    lib.ahs_group_slab.argtypes = [vp, i32]; lib.ahs_group_slab.restype = vp
+    lib.ahs_group_destroy.argtypes = [vp]; lib.ahs_group_destroy.restype = i32
     _lib = lib
     return lib
 
@@ -265,6 +276,81 @@ class Simulation:
 
     def synchronize(self):
         _check(load().ahs_synchronize(self._h))
+
+
+class Group:
+    """One lattice cut into z-slabs (ahs_group): one handle per slab on `devices` (CUDA ordinals, may repeat; None = the current
+    device for all).  Methods mirror the C functions one to one."""
+
+    def __init__(self, N, nslabs, devices=None, dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, m=1.0, s=0.0, tau0=1.0, seed=0,
+                 precision="f32", ic="random_phase", tau_ref=0.0, c_B=0.0, c_E=0.0):
+        self._g = None
+        lib = load()
+        self.N, self.nslabs = int(N), int(nslabs)
+        self.precision = _prec(precision)
+        self.dtype = np.float32 if self.precision == AHS_F32 else np.float64
+        p = ahs_params()
+        p.N, p.precision, p.ic_kind, p.kernel = self.N, self.precision, _ICS[ic], AHS_KERNEL_AUTO
+        p.dx, p.dt, p.lambda_, p.e, p.sigma, p.m, p.s, p.tau0, p.tau_ref = dx, dt, lambda0, e0, sigma, m, s, tau0, tau_ref
+        p.seed, p.c_B, p.c_E = seed, c_B, c_E
+        dev = (C.c_int32 * self.nslabs)(*[int(d) for d in devices]) if devices is not None else None
+        g = lib.ahs_group_create(C.byref(p), self.nslabs, dev)
+        if not g:
+            msg = last_error()
+            raise AhsError(AHS_ERR_CUDA if "CUDA" in msg or "device" in msg else AHS_ERR_INVALID_ARG, msg)
+        self._g = C.c_void_p(g)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def destroy(self):
+        if self._g is not None:
+            load().ahs_group_destroy(self._g)
+            self._g = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def step(self, n=1):
+        _check(load().ahs_group_step(self._g, int(n)))
+
+    def diagnostics(self, allow_nonfinite=True) -> dict:
+        d = ahs_diag()
+        _check(load().ahs_group_diagnostics(self._g, C.byref(d)), allow=(AHS_ERR_NONFINITE,) if allow_nonfinite else ())
+        return {k: getattr(d, k) for k, _ in ahs_diag._fields_ if k != "reserved"}
+
+    def get_fields_native(self, out=None):
+        if out is None:
+            out = np.empty((10, self.N, self.N, self.N), dtype=self.dtype)
+        _check(load().ahs_group_get_fields_native(self._g, out if isinstance(out, int) else out.ctypes.data))
+        return out
+
+    def set_fields_native(self, src, step: int = 0):
+        _check(load().ahs_group_set_fields_native(self._g, src if isinstance(src, int) else src.ctypes.data, int(step)))
+
+    def synchronize(self):
+        _check(load().ahs_group_synchronize(self._g))
+
+    def set_option(self, option: int, value: int):
+        """ahs_set_option on every slab."""
+        lib = load()
+        for r in range(lib.ahs_group_slab_count(self._g)):
+            _check(lib.ahs_set_option(C.c_void_p(lib.ahs_group_slab(self._g, r)), int(option), int(value)))
+
+    @property
+    def kernel_launches(self):
+        lib, tot = load(), 0
+        for r in range(lib.ahs_group_slab_count(self._g)):
+            nl = C.c_int64()
+            _check(lib.ahs_get_state(C.c_void_p(lib.ahs_group_slab(self._g, r)), None, None, C.byref(nl)))
+            tot += nl.value
+        return tot
 
 
 def create(N, dx, dt, lambda0, e0, sigma, m, s, tau0, seed):

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "ahs_internal.cuh"
 
@@ -33,7 +34,18 @@ struct ahs_sim {
     StepMaps step_maps[2];     // the same for the step march (buffer 0 / 1 as the level-n input)
     bool step_maps_ok;
     MarchOptions opt;          // ahs_set_option
+    // z-slab of an ahs_group; a whole lattice has zr = { N, 0, periodic, N } and no ghost targets
+    ZRange zr;
+    int z_offset;              // global plane of the first own plane
+    int64_t nsites_alloc;      // N * N * zr.nz_alloc
+    bool owns_stream;
+    // where the step kernel also stores its bottom / top plane, per OUTPUT buffer (0 / 1): the neighbours' ghost planes
+    void* ghost_lo[2][5];
+    void* ghost_hi[2][5];
+    void* ghost_eps2_hi;
 };
+
+struct SlabSpec { int nz; int z_offset; };
 
 namespace {
 
@@ -135,7 +147,11 @@ int do_step(ahs_sim* s)
     }
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
     const StepCoef c = step_coefficients(s->p, s->step);
-    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, c, s->step_maps_ok ? &s->step_maps[s->cur] : nullptr, s->opt, s->stream)
+    GhostPtrs<T> gh;
+    const int ob = s->cur ^ 1;
+    for (int i = 0; i < 5; ++i) { gh.lo[i] = (T*)s->ghost_lo[ob][i]; gh.hi[i] = (T*)s->ghost_hi[ob][i]; }
+    gh.eps2_hi = (T*)s->ghost_eps2_hi;
+    return s->kernel == AHS_KERNEL_MARCH ? launch_step_march<T>(f, s->p.N, s->zr, &gh, c, s->step_maps_ok ? &s->step_maps[s->cur] : nullptr, s->opt, s->stream)
                                          : launch_step_generic<T>(f, s->p.N, c, s->stream);
 }
 
@@ -149,10 +165,42 @@ int do_diag(ahs_sim* s)
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
     const DiagCoef c = diag_coefficients(s->p, s->step);
     return s->kernel == AHS_KERNEL_MARCH
-               ? launch_diag_march<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result,
-                                      slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1), 5 * s->array_bytes,
+               ? launch_diag_march<T>(f, s->p.N, s->zr, c, s->partials, kMaxDiagPartials, s->result,
+                                      // the doubt list: the shadow buffer, from its first OWN plane on (a slab's ghost planes there
+                                      // belong to the neighbours' next step)
+                                      slot<T>(s, s->cur ? PHI_RE0 : PHI_RE1) + (size_t)s->zr.zbase * s->p.N * s->p.N,
+                                      5 * s->array_bytes - (size_t)s->zr.zbase * s->p.N * s->p.N * sizeof(T),
                                       s->diag_map_ok ? &s->diag_map[s->cur] : nullptr, s->opt, s->stream)   // shadow buffer: dead between steps
                : launch_diag_generic<T>(f, s->p.N, c, s->partials, kMaxDiagPartials, s->result, s->stream);
+}
+
+// The record of a diagnostics pass (raw sums of the reduction) -> the quantities of include/ahs.h
+void fill_diag(ahs_diag* out, const ahs_params& p, int64_t diag_step, double nsites, const DiagPartial& r)
+{
+    std::memset(out, 0, sizeof(*out));
+    out->step = diag_step;
+    out->tau = tau_of(p, diag_step);
+    out->n_pierced = r.n_pierced;
+    out->sum_abs_w = r.sum_abs_w;
+    out->L = (M_PI / 6.0) * p.dx * (double)r.n_pierced;                     // L93
+    const double box = (double)p.N * p.dx;
+    out->xi = r.n_pierced ? std::sqrt(box * box * box / out->L) : INFINITY; // L88
+    out->v2_num = r.num;
+    out->v2_den = r.den;
+    const double R = r.num / r.den;                                          // Eq. 10
+    out->v2 = 2.0 * R / (1.0 + R);                                           // Eq. 9
+    out->mean_lagrangian = r.lsum / nsites;
+    out->gauss_max = r.gmax;
+    out->gauss_rhs_rms = std::sqrt(r.rhs2 / nsites);
+    out->nonfinite = r.nonfinite ? 1 : 0;
+    out->v2v_num = r.vnum;
+    out->v2v_den = r.vden;
+    const double Rv = r.vnum / r.vden;
+    out->v2_V = 2.0 * Rv / (1.0 + Rv);
+    out->xi_L = std::sqrt(-(2.0 * M_PI * p.sigma * p.sigma) / out->mean_lagrangian);   // mu = 2 pi sigma^2 (DESIGN.md R20)
+    out->eos_num = r.wnum;
+    out->eos_den = r.wden;
+    out->v2_omega = 0.5 * (1.0 + 3.0 * r.wnum / r.wden);                                 // Eq. 12
 }
 
 int check_sim(const ahs_sim* s)
@@ -201,7 +249,7 @@ size_t ahs_required_bytes(int32_t N, int32_t precision)
     return (size_t)NUM_SLOTS * round256(nsites * elem) + scratch_bytes();
 }
 
-ahs_sim* ahs_create_ex(const ahs_params* params)
+ahs_sim* create_sim(const ahs_params* params, const SlabSpec* slab)
 {
     g_err[0] = 0;
     if (!params) { fail(AHS_ERR_INVALID_ARG, "params is NULL"); return nullptr; }
@@ -234,14 +282,26 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     s->p = p;
     s->nsites = (int64_t)p.N * p.N * p.N;
     s->elem = p.precision == AHS_F32 ? 4 : 8;
-    s->array_bytes = round256((size_t)s->nsites * s->elem);
+    s->zr = slab ? ZRange{ slab->nz, 1, 0, slab->nz + 2 } : ZRange{ p.N, 0, 1, p.N };
+    s->z_offset = slab ? slab->z_offset : 0;
+    s->nsites_alloc = (int64_t)p.N * p.N * s->zr.nz_alloc;
+    s->array_bytes = round256((size_t)s->nsites_alloc * s->elem);
     s->stream = (cudaStream_t)p.stream;
+    s->owns_stream = false;
+    std::memset(s->ghost_lo, 0, sizeof(s->ghost_lo));
+    std::memset(s->ghost_hi, 0, sizeof(s->ghost_hi));
+    s->ghost_eps2_hi = nullptr;
+    if (slab) {
+        if (!march_ok || p.device_buffer) { fail(AHS_ERR_INVALID_ARG, "a z-slab needs the z-marching kernels (N %% %d == 0) and library-owned memory", p.precision == AHS_F32 ? 128 : 64); delete s; return nullptr; }
+        if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaStreamCreate: %s", cudaGetErrorString(cudaGetLastError())); delete s; return nullptr; }
+        s->owns_stream = true;
+    }
     s->cur = 0; s->step = 0; s->launches = 0; s->diag_step = -1; s->device = dev;
     s->kernel = (p.kernel == AHS_KERNEL_AUTO) ? (march_ok ? AHS_KERNEL_MARCH : AHS_KERNEL_GENERIC) : p.kernel;
     s->result_host = nullptr;
     s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0 };
 
-    const size_t need = ahs_required_bytes(p.N, p.precision);
+    const size_t need = (size_t)NUM_SLOTS * s->array_bytes + scratch_bytes();
     if (p.device_buffer) {
         if (p.device_buffer_bytes < need || ((uintptr_t)p.device_buffer & 255)) {
             fail(AHS_ERR_INVALID_ARG, "device_buffer must hold %zu bytes and be 256-byte aligned", need);
@@ -273,15 +333,15 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     s->step_maps_ok = false;
     if (s->kernel == AHS_KERNEL_MARCH) {
         s->step_maps_ok = p.precision == AHS_F32
-            ? make_step_march_maps<float>(&s->step_maps[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
-              make_step_march_maps<float>(&s->step_maps[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)
-            : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), p.N, s->array_bytes) &&
-              make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), p.N, s->array_bytes);
+            ? make_step_march_maps<float>(&s->step_maps[0], slot<float>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_step_march_maps<float>(&s->step_maps[1], slot<float>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes)
+            : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes);
         s->diag_map_ok = p.precision == AHS_F32
-            ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->array_bytes) &&
-              make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->array_bytes)
-            : make_diag_march_map<double>(&s->diag_map[0], slot<double>(s, PHI_RE0), p.N, s->array_bytes) &&
-              make_diag_march_map<double>(&s->diag_map[1], slot<double>(s, PHI_RE1), p.N, s->array_bytes);
+            ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes)
+            : make_diag_march_map<double>(&s->diag_map[0], slot<double>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_diag_march_map<double>(&s->diag_map[1], slot<double>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes);
     }
 
     // initial condition (L72): everything zero, then phi from Philox
@@ -289,13 +349,15 @@ ahs_sim* ahs_create_ex(const ahs_params* params)
     if (ce != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(ce)); ahs_destroy(s); return nullptr; }
     if (p.ic_kind != AHS_IC_NONE) {
         const int r = p.precision == AHS_F32
-                          ? launch_ic<float>(slot<float>(s, PHI_RE0), slot<float>(s, PHI_IM0), p.N, p.sigma, p.seed, p.ic_kind, s->stream)
-                          : launch_ic<double>(slot<double>(s, PHI_RE0), slot<double>(s, PHI_IM0), p.N, p.sigma, p.seed, p.ic_kind, s->stream);
+                          ? launch_ic<float>(slot<float>(s, PHI_RE0), slot<float>(s, PHI_IM0), p.N, s->zr.nz_alloc, s->z_offset - s->zr.zbase, p.sigma, p.seed, p.ic_kind, s->stream)
+                          : launch_ic<double>(slot<double>(s, PHI_RE0), slot<double>(s, PHI_IM0), p.N, s->zr.nz_alloc, s->z_offset - s->zr.zbase, p.sigma, p.seed, p.ic_kind, s->stream);
         if (r < 0) { fail(AHS_ERR_CUDA, "IC kernel launch: %s", cudaGetErrorString(cudaGetLastError())); ahs_destroy(s); return nullptr; }
         s->launches += r;
     }
     return s;
 }
+
+ahs_sim* ahs_create_ex(const ahs_params* params) { return create_sim(params, nullptr); }
 
 ahs_sim* ahs_create(int32_t N, double dx, double dt, double lambda, double e, double sigma, double m, double s, double tau0, uint64_t seed)
 {
@@ -339,31 +401,7 @@ int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
     AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
     AHS_CUDA(cudaStreamSynchronize(s->stream));
     const DiagPartial& r = *s->result_host;
-    const ahs_params& p = s->p;
-    std::memset(out, 0, sizeof(*out));
-    out->step = s->diag_step;
-    out->tau = tau_of(p, s->diag_step);
-    out->n_pierced = r.n_pierced;
-    out->sum_abs_w = r.sum_abs_w;
-    out->L = (M_PI / 6.0) * p.dx * (double)r.n_pierced;                     // L93
-    const double box = (double)p.N * p.dx;
-    out->xi = r.n_pierced ? std::sqrt(box * box * box / out->L) : INFINITY; // L88
-    out->v2_num = r.num;
-    out->v2_den = r.den;
-    const double R = r.num / r.den;                                          // Eq. 10
-    out->v2 = 2.0 * R / (1.0 + R);                                           // Eq. 9
-    out->mean_lagrangian = r.lsum / (double)s->nsites;
-    out->gauss_max = r.gmax;
-    out->gauss_rhs_rms = std::sqrt(r.rhs2 / (double)s->nsites);
-    out->nonfinite = r.nonfinite ? 1 : 0;
-    out->v2v_num = r.vnum;
-    out->v2v_den = r.vden;
-    const double Rv = r.vnum / r.vden;
-    out->v2_V = 2.0 * Rv / (1.0 + Rv);
-    out->xi_L = std::sqrt(-(2.0 * M_PI * p.sigma * p.sigma) / out->mean_lagrangian);   // mu = 2 pi sigma^2 (DESIGN.md R20)
-    out->eos_num = r.wnum;
-    out->eos_den = r.wden;
-    out->v2_omega = 0.5 * (1.0 + 3.0 * r.wnum / r.wden);                                 // Eq. 12
+    fill_diag(out, s->p, s->diag_step, (double)s->nsites, r);
     s->diag_step = -1;
     if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "the lattice holds non-finite field values at step %lld (%llu sites or thread-planes flagged)",
                                     (long long)out->step, (unsigned long long)r.nonfinite);
@@ -391,6 +429,7 @@ int32_t ahs_diagnostics(ahs_sim* s, double* L, double* v2, double* gauss)
 int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
 {
     AHS_ENTER(s);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's fields are read and written through its ahs_group");
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     const size_t bytes = (size_t)s->nsites * s->elem;
     for (int k = 0; k < 10; ++k)
@@ -403,6 +442,7 @@ int32_t ahs_get_fields_native(ahs_sim* s, void* host10)
 int32_t ahs_set_fields_native_async(ahs_sim* s, const void* host10, int64_t step)
 {
     AHS_ENTER(s);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's fields are read and written through its ahs_group");
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
     const size_t bytes = (size_t)s->nsites * s->elem;
@@ -428,6 +468,7 @@ int32_t ahs_get_fields(ahs_sim* s, double* host10)
     AHS_ENTER(s);
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (s->p.precision == AHS_F64) return ahs_get_fields_native(s, host10);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's fields are read and written through its ahs_group");
     const int shadow = s->cur ? PHI_RE0 : PHI_RE1;   // 5 dead float arrays = room for 2 double arrays
     double* stage = reinterpret_cast<double*>(s->base + (size_t)shadow * s->array_bytes);
     const size_t bytes = (size_t)s->nsites * sizeof(double);
@@ -447,6 +488,7 @@ int32_t ahs_set_fields(ahs_sim* s, const double* host10, int64_t step)
     if (!host10) return fail(AHS_ERR_INVALID_ARG, "host10 is NULL");
     if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
     if (s->p.precision == AHS_F64) return ahs_set_fields_native(s, host10, step);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's fields are read and written through its ahs_group");
     const int shadow = s->cur ? PHI_RE0 : PHI_RE1;
     double* stage = reinterpret_cast<double*>(s->base + (size_t)shadow * s->array_bytes);
     const size_t bytes = (size_t)s->nsites * sizeof(double);
@@ -526,8 +568,254 @@ int32_t ahs_destroy(ahs_sim* s)
     cudaStreamSynchronize(s->stream);
     if (s->result_host) cudaFreeHost(s->result_host);
     if (s->owns_buffer && s->base) cudaFree(s->base);
+    if (s->owns_stream) cudaStreamDestroy(s->stream);
     delete s;
     return AHS_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// ahs_group: one lattice cut into z-slabs, one slab per handle, handles on one or several GPUs of this process (
+// the paper's stated next step).  The exchange is part of the step kernel: it stores the new (phi, theta) of
+// its boundary planes into the neighbouring slabs' ghost planes (peer memory over NVLink when they live on another GPU), and
+// CUDA events order step n+1 of a slab behind step n of its two neighbours.  Nothing spins on the device.
+// ---------------------------------------------------------------------------------------------------------------------------
+struct ahs_group {
+    ahs_params p;
+    int P;
+    std::vector<ahs_sim*> slab;
+    std::vector<cudaEvent_t> done[2];   // done[k][r]: slab r has finished its most recent step of parity k (or later work)
+    int parity;                         // parity of the NEXT step's events
+    bool have_prev;
+    int64_t step;
+};
+
+namespace {
+
+int lo_of(const ahs_group* g, int r) { return (r + g->P - 1) % g->P; }
+int hi_of(const ahs_group* g, int r) { return (r + 1) % g->P; }
+
+char* plane_ptr(const ahs_sim* s, int slot_index, int local_plane)
+{
+    return s->base + (size_t)slot_index * s->array_bytes + (size_t)local_plane * s->p.N * s->p.N * s->elem;
+}
+
+// slab r's next launch runs behind the last step (and anything enqueued after it) of its two neighbours
+int wait_for_neighbours(ahs_group* g, int r)
+{
+    if (!g->have_prev) return AHS_OK;
+    const int k = g->parity ^ 1;
+    for (int nb : { lo_of(g, r), hi_of(g, r) })
+        if (nb != r && cudaStreamWaitEvent(g->slab[r]->stream, g->done[k][nb], 0) != cudaSuccess)
+            return fail(AHS_ERR_CUDA, "cudaStreamWaitEvent: %s", cudaGetErrorString(cudaGetLastError()));
+    return AHS_OK;
+}
+
+int group_sync(ahs_group* g)
+{
+    for (ahs_sim* s : g->slab) {
+        DeviceGuard guard(s->device);
+        if (cudaStreamSynchronize(s->stream) != cudaSuccess) return fail(AHS_ERR_CUDA, "cudaStreamSynchronize: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    return AHS_OK;
+}
+
+// ghost planes of the CURRENT (phi, theta) buffer and of eps_2 from the neighbours' boundary planes (after the fields were set from the host)
+int refresh_ghosts(ahs_group* g)
+{
+    if (int r = group_sync(g)) return r;
+    for (int r = 0; r < g->P; ++r) {
+        ahs_sim* s = g->slab[r];
+        const ahs_sim* lo = g->slab[lo_of(g, r)];
+        const ahs_sim* hi = g->slab[hi_of(g, r)];
+        const size_t plane = (size_t)s->p.N * s->p.N * s->elem;
+        DeviceGuard guard(s->device);
+        const int b = s->cur ? PHI_RE1 : PHI_RE0;
+        for (int i = 0; i < 5; ++i) {
+            AHS_CUDA(cudaMemcpyPeerAsync(plane_ptr(s, b + i, 0), s->device, plane_ptr(lo, b + i, lo->zr.nz), lo->device, plane, s->stream));
+            AHS_CUDA(cudaMemcpyPeerAsync(plane_ptr(s, b + i, s->zr.nz + 1), s->device, plane_ptr(hi, b + i, 1), hi->device, plane, s->stream));
+        }
+        AHS_CUDA(cudaMemcpyPeerAsync(plane_ptr(s, EPS2, 0), s->device, plane_ptr(lo, EPS2, lo->zr.nz), lo->device, plane, s->stream));
+    }
+    return group_sync(g);
+}
+
+}  // namespace
+
+int32_t ahs_group_destroy(ahs_group* g)
+{
+    if (!g) return AHS_OK;
+    for (ahs_sim* s : g->slab)
+        if (s) { DeviceGuard guard(s->device); cudaStreamSynchronize(s->stream); }
+    for (int k = 0; k < 2; ++k)
+        for (size_t r = 0; r < g->done[k].size(); ++r)
+            if (g->done[k][r]) { DeviceGuard guard(g->slab[r]->device); cudaEventDestroy(g->done[k][r]); }
+    for (ahs_sim* s : g->slab) ahs_destroy(s);
+    delete g;
+    return AHS_OK;
+}
+
+ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int32_t* devices)
+{
+    g_err[0] = 0;
+    if (!params) { fail(AHS_ERR_INVALID_ARG, "params is NULL"); return nullptr; }
+    if (nslabs < 1 || nslabs > 64 || !valid_N(params->N) || params->N % nslabs != 0) {
+        fail(AHS_ERR_INVALID_ARG, "nslabs must be in 1..64 and divide N"); return nullptr;
+    }
+    if (params->device_buffer || params->stream) { fail(AHS_ERR_INVALID_ARG, "a group owns its memory and streams: device_buffer and stream must be NULL"); return nullptr; }
+    int ndev = 0, home = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || cudaGetDevice(&home) != cudaSuccess) {
+        cudaGetLastError();
+        fail(AHS_ERR_CUDA, "no CUDA device (libahs has no CPU fallback)"); return nullptr;
+    }
+    ahs_group* g = new (std::nothrow) ahs_group();
+    if (!g) { fail(AHS_ERR_OOM, "host allocation failed"); return nullptr; }
+    g->p = *params; g->P = nslabs; g->parity = 0; g->have_prev = false; g->step = 0;
+    g->slab.assign(nslabs, nullptr);
+    g->done[0].assign(nslabs, nullptr); g->done[1].assign(nslabs, nullptr);
+    const int nz = params->N / nslabs;
+    for (int r = 0; r < nslabs; ++r) {
+        const int dev = devices ? devices[r] : home;
+        if (dev < 0 || dev >= ndev) { fail(AHS_ERR_INVALID_ARG, "device %d of slab %d does not exist (%d devices)", dev, r, ndev); ahs_group_destroy(g); return nullptr; }
+        DeviceGuard guard(dev);
+        ahs_params p = *params;
+        p.kernel = AHS_KERNEL_MARCH;
+        SlabSpec spec = { nz, r * nz };
+        g->slab[r] = create_sim(&p, &spec);
+        if (!g->slab[r]) { ahs_group_destroy(g); return nullptr; }
+        for (int k = 0; k < 2; ++k)
+            if (cudaEventCreateWithFlags(&g->done[k][r], cudaEventDisableTiming) != cudaSuccess) {
+                fail(AHS_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(cudaGetLastError())); ahs_group_destroy(g); return nullptr;
+            }
+    }
+    // peer access between neighbouring slabs on different devices, then the ghost targets of every slab
+    for (int r = 0; r < nslabs; ++r)
+        for (int nb : { lo_of(g, r), hi_of(g, r) }) {
+            const int a = g->slab[r]->device, b = g->slab[nb]->device;
+            if (a == b) continue;
+            int can = 0;
+            DeviceGuard guard(a);
+            if (cudaDeviceCanAccessPeer(&can, a, b) != cudaSuccess || !can) {
+                cudaGetLastError();
+                fail(AHS_ERR_CUDA, "device %d cannot access device %d: slabs on different GPUs need peer access (NVLink / NVSwitch)", a, b);
+                ahs_group_destroy(g); return nullptr;
+            }
+            const cudaError_t e = cudaDeviceEnablePeerAccess(b, 0);
+            if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) { fail(AHS_ERR_CUDA, "cudaDeviceEnablePeerAccess: %s", cudaGetErrorString(e)); ahs_group_destroy(g); return nullptr; }
+            cudaGetLastError();
+        }
+    for (int r = 0; r < nslabs; ++r) {
+        ahs_sim* s = g->slab[r];
+        const ahs_sim* lo = g->slab[lo_of(g, r)];
+        const ahs_sim* hi = g->slab[hi_of(g, r)];
+        for (int ob = 0; ob < 2; ++ob) {
+            const int b = ob ? PHI_RE1 : PHI_RE0;
+            for (int i = 0; i < 5; ++i) {
+                s->ghost_lo[ob][i] = plane_ptr(lo, b + i, lo->zr.nz + 1);   // my bottom plane is the lower neighbour's ghost above
+                s->ghost_hi[ob][i] = plane_ptr(hi, b + i, 0);               // my top plane is the upper neighbour's ghost below
+            }
+        }
+        s->ghost_eps2_hi = plane_ptr(hi, EPS2, 0);
+    }
+    if (group_sync(g) != AHS_OK) { ahs_group_destroy(g); return nullptr; }
+    return g;
+}
+
+int32_t ahs_group_step(ahs_group* g, int32_t n)
+{
+    if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
+    if (n < 0) return fail(AHS_ERR_INVALID_ARG, "n must be >= 0");
+    for (int32_t k = 0; k < n; ++k) {
+        for (int r = 0; r < g->P; ++r) {
+            ahs_sim* s = g->slab[r];
+            DeviceGuard guard(s->device);
+            if (!guard.ok()) return fail(AHS_ERR_CUDA, "cannot make device %d current", s->device);
+            if (int e = wait_for_neighbours(g, r)) return e;
+            const int rc = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
+            if (rc < 0) return fail(rc, "step kernel launch failed on slab %d at step %lld: %s", r, (long long)s->step, cudaGetErrorString(cudaGetLastError()));
+            s->launches += rc;
+            AHS_CUDA(cudaEventRecord(g->done[g->parity][r], s->stream));
+        }
+        for (ahs_sim* s : g->slab) { s->cur ^= 1; s->step += 1; }
+        g->parity ^= 1;
+        g->have_prev = true;
+        g->step += 1;
+    }
+    return AHS_OK;
+}
+
+int32_t ahs_group_diagnostics(ahs_group* g, ahs_diag* out)
+{
+    if (!g || !out) return fail(AHS_ERR_INVALID_ARG, "null group or out");
+    for (int r = 0; r < g->P; ++r) {
+        ahs_sim* s = g->slab[r];
+        DeviceGuard guard(s->device);
+        if (int e = wait_for_neighbours(g, r)) return e;     // the ghosts it reads are the neighbours' last step
+        const int rc = s->p.precision == AHS_F32 ? do_diag<float>(s) : do_diag<double>(s);
+        if (rc < 0) return fail(rc, "diagnostics kernel launch failed on slab %d: %s", r, cudaGetErrorString(cudaGetLastError()));
+        s->launches += rc;
+        AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
+    }
+    DiagPartial t;
+    std::memset(&t, 0, sizeof(t));
+    for (int r = 0; r < g->P; ++r) {   // fixed order: the result does not depend on which slab finishes first
+        ahs_sim* s = g->slab[r];
+        DeviceGuard guard(s->device);
+        AHS_CUDA(cudaStreamSynchronize(s->stream));
+        const DiagPartial& q = *s->result_host;
+        t.n_pierced += q.n_pierced; t.sum_abs_w += q.sum_abs_w; t.num += q.num; t.den += q.den; t.lsum += q.lsum;
+        t.gmax = q.gmax > t.gmax || q.gmax != q.gmax ? q.gmax : t.gmax;
+        t.rhs2 += q.rhs2; t.nonfinite += q.nonfinite; t.vnum += q.vnum; t.vden += q.vden; t.wnum += q.wnum; t.wden += q.wden;
+    }
+    fill_diag(out, g->p, g->step, (double)g->p.N * g->p.N * g->p.N, t);
+    if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "the lattice holds non-finite field values at step %lld", (long long)out->step);
+    return AHS_OK;
+}
+
+// the whole lattice, 10 N^3 values of the storage type in the field order of include/ahs.h, gathered from / scattered to the slabs
+int32_t ahs_group_get_fields_native(ahs_group* g, void* host10)
+{
+    if (!g || !host10) return fail(AHS_ERR_INVALID_ARG, "null group or host10");
+    const size_t field = (size_t)g->p.N * g->p.N * g->p.N * g->slab[0]->elem;
+    for (ahs_sim* s : g->slab) {
+        DeviceGuard guard(s->device);
+        const size_t plane = (size_t)s->p.N * s->p.N * s->elem;
+        for (int k = 0; k < 10; ++k)
+            AHS_CUDA(cudaMemcpyAsync((char*)host10 + (size_t)k * field + (size_t)s->z_offset * plane, plane_ptr(s, live_slot(s, k), 1),
+                                     plane * s->zr.nz, cudaMemcpyDeviceToHost, s->stream));
+    }
+    return group_sync(g);
+}
+
+int32_t ahs_group_set_fields_native(ahs_group* g, const void* host10, int64_t step)
+{
+    if (!g || !host10 || step < 0) return fail(AHS_ERR_INVALID_ARG, "null group or host10, or step < 0");
+    if (int r = group_sync(g)) return r;
+    const size_t field = (size_t)g->p.N * g->p.N * g->p.N * g->slab[0]->elem;
+    for (ahs_sim* s : g->slab) {
+        DeviceGuard guard(s->device);
+        const size_t plane = (size_t)s->p.N * s->p.N * s->elem;
+        for (int k = 0; k < 10; ++k)
+            AHS_CUDA(cudaMemcpyAsync(plane_ptr(s, live_slot(s, k), 1), (const char*)host10 + (size_t)k * field + (size_t)s->z_offset * plane,
+                                     plane * s->zr.nz, cudaMemcpyHostToDevice, s->stream));
+        s->step = step;
+    }
+    g->step = step;
+    return refresh_ghosts(g);
+}
+
+int32_t ahs_group_synchronize(ahs_group* g)
+{
+    if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
+    return group_sync(g);
+}
+
+int32_t ahs_group_slab_count(ahs_group* g) { return g ? g->P : fail(AHS_ERR_INVALID_ARG, "null group"); }
+
+ahs_sim* ahs_group_slab(ahs_group* g, int32_t r)
+{
+    if (!g || r < 0 || r >= g->P) { fail(AHS_ERR_INVALID_ARG, "null group or slab index out of range"); return nullptr; }
+    return g->slab[r];
 }
 
 }  // extern "C"

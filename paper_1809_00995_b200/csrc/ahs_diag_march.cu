@@ -85,7 +85,7 @@ __device__ __forceinline__ float2 to_float2(double2 v) { return make_float2((flo
 // fields; resolving them in-line (an out-of-line call inside the march) made every warp of the CTA wait for the one
 // that took the slow path (profiles/r2: 30 % of the issue slots), a separate pass costs ~0.1 ms at 1024^3.
 template <typename T>
-__global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N, const unsigned* __restrict__ list,
+__global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N, int periodic_z, const unsigned* __restrict__ list,
                                                            const unsigned long long* __restrict__ count, DiagPartial* __restrict__ extra)
 {
     constexpr int V = 16 / sizeof(T);
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
     for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (unsigned long long)gridDim.x * blockDim.x) {
         const unsigned u = list[e];
         const int xv = (int)(u & 1023u), y = (int)((u >> 10) & 2047u), z = (int)(u >> 21);
-        const int yp = y + 1 == N ? 0 : y + 1, zp = z + 1 == N ? 0 : z + 1;
+        const int yp = y + 1 == N ? 0 : y + 1, zp = (periodic_z && z + 1 == N) ? 0 : z + 1;   // (z is the LOCAL plane index: a slab has its ghost above)
         auto at = [&](int x, int yy, int zz) { return ((size_t)zz * N + (size_t)yy) * N + (size_t)x; };
         auto arg = [&](size_t i) { return atan2((double)f.phi_im[i], (double)f.phi_re[i]); };
         auto ln = [](double as, double a_t, T th) { return (int)rint((a_t - as - (double)th) * kInv2Pi); };
@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
 
 template <typename T>
 __global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, DiagCfg<T>::MINB)
-diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
+diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
                   unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
                   const __grid_constant__ CUtensorMap wmap, int use_tma)
 {
@@ -143,9 +143,9 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     const int tx = bid % tiles_x;
     bid /= tiles_x;
     const int ty = bid % tiles_y, zc = bid / tiles_y;
-    // z-chunk zc of nchunks: planes [zc N / nchunks, (zc + 1) N / nchunks)
-    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * N / nchunks);
-    const int zlen = (int)((long long)(zc + 1) * N / nchunks) - z0;
+    // z-chunk zc of nchunks: own planes [zc nz / nchunks, (zc + 1) nz / nchunks)
+    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * zr.nz / nchunks);
+    const int zlen = (int)((long long)(zc + 1) * zr.nz / nchunks) - z0;
     const int xi = V * lane;
 
     const T* const src[5] = { f.phi_re, f.phi_im, f.th[0], f.th[1], f.th[2] };
@@ -161,8 +161,8 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     }
     __syncthreads();
 
-    // plane index p of this CTA's march = lattice plane z0 + p (periodic); planes 0 .. zlen are needed
-    auto plane_of = [&](int p) { const int z = z0 + p; return z >= N ? z - N : z; };
+    // plane index p of this CTA's march = own plane z0 + p (periodic in a whole lattice, the ghost above in a slab); planes 0 .. zlen are needed
+    auto plane_of = [&](int p) { const int z = z0 + p; return ((zr.periodic && z >= N) ? z - N : z) + zr.zbase; };
     // One tensor copy per plane for tiles away from the periodic boundary.  Tiles on the right edge get the main box
     // (zero-filled out of bounds) plus a V-wide tensor copy of the wrapped column x = 0 .. V-1 into a side buffer, which the
     // readers of column TX use instead; tiles on the top edge in y (1 of N/TY tile rows) keep the row copies.
@@ -227,11 +227,11 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
     // The momenta (no halo) come straight from global memory: g = element offset of this thread's vector in plane z0 + it, a
     // running offset; the row below (eps_1^{x-k_1}) and the site left of the tile (eps_0^{x-k_0}, lane 0) sit at fixed distances.
     const size_t plane_stride = (size_t)N * N;
-    size_t g = ((size_t)z0 * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+    size_t g = ((size_t)(zr.zbase + z0) * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
     const ptrdiff_t d_row_below = (y0 + w == 0) ? (ptrdiff_t)(N - 1) * N : -(ptrdiff_t)N;
     const ptrdiff_t d_site_left = (x0 + xi == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;
     // eps_2 of the plane below, carried in registers along the march
-    VecT E2m = ldg_vec<T, V>(f.eps[2] + (z0 == 0 ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));
+    VecT E2m = ldg_vec<T, V>(f.eps[2] + ((zr.periodic && z0 == 0) ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));   // (slab: the ghost below)
 
     double num = 0.0, den = 0.0, lsum = 0.0, rhs2 = 0.0, vnum = 0.0, vden = 0.0, wnum = 0.0, wden = 0.0;
     float pierced_f = 0.0f;   // plaquettes with W != 0 on the fast path (all |W| <= 1 there, so this is sum |W| as well); exact below 2^24
@@ -302,7 +302,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
             const bool sure = (fmaxf(rmax, rmax_c) < 0.5f - kTieMargin * (1.0f + fmaxf(tmax, tmax_c))) && (ssq.x + ssq.y == cnt);
             if (!sure) {   // fp64 decides (diag_resolve_kernel)
                 const unsigned long long e = atomicAdd(doubt_count, 1ull);
-                doubt_list[e] = (unsigned)((x0 + xi) / V) | ((unsigned)(y0 + w) << 10) | ((unsigned)(z0 + it) << 21);   // N <= 2048
+                doubt_list[e] = (unsigned)((x0 + xi) / V) | ((unsigned)(y0 + w) << 10) | ((unsigned)(zr.zbase + z0 + it) << 21);   // N <= 2048, local plane index
             }
             pierced_f += sure ? cnt : 0.0f;
         }
@@ -411,30 +411,31 @@ diag_march_kernel(DiagPtrs<T> f, int N, int nchunks, DiagCoef kd, DiagPartial* _
 // z-chunks per tile, measured (profiles/r4_chunks.md; see pick_chunks of the step march): 32 up to 512^3, 16 beyond and for
 // fp64 lattices; halved until the partial records fit and the count divides N.
 template <typename T>
-int pick_chunks(int N, long tiles, int max_partials)
+int pick_chunks(int N, int nz, long tiles, int max_partials)
 {
     int c = (sizeof(T) == 4 && N <= 512) ? 32 : 16;
     while (c > 1 && (N % c != 0 || N / c < 4 || tiles * c + 2 > max_partials)) c /= 2;
-    return c;
+    const int zlen = N / c;                 // planes per chunk, read off the whole lattice; a slab of nz planes gets nz / zlen chunks
+    return nz >= zlen ? nz / zlen : 1;
 }
 
 }  // namespace
 
 template <typename T>
-int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
+int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagCoef& c, DiagPartial* partials, int max_partials, DiagPartial* result,
                       void* list, size_t list_bytes, const DiagMaps* tmap, const MarchOptions& opt, cudaStream_t st)
 {
     using C = DiagCfg<T>;
-    if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
+    if (!march_supported<T>(N) || zr.nz < 1) return AHS_ERR_INVALID_ARG;
     auto kern = diag_march_kernel<T>;
     static SmemAttribute attr;   // per device
     if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
     const long tiles = (long)(N / C::TX) * (N / C::TY);
-    int nchunks = pick_chunks<T>(N, tiles, max_partials);
-    if (opt.diag_chunks > 0 && opt.diag_chunks <= N && tiles * opt.diag_chunks + 2 <= max_partials) nchunks = opt.diag_chunks;
+    int nchunks = pick_chunks<T>(N, zr.nz, tiles, max_partials);
+    if (opt.diag_chunks > 0 && opt.diag_chunks <= zr.nz && tiles * opt.diag_chunks + 2 <= max_partials) nchunks = opt.diag_chunks;
     const long blocks = tiles * nchunks;
     // partials[blocks] collects the second pass, partials[blocks + 1].n_pierced is the length of the doubt list
-    if (blocks + 2 > max_partials || list_bytes < sizeof(unsigned) * ((size_t)N * N * N / C::V)) return AHS_ERR_INVALID_ARG;
+    if (blocks + 2 > max_partials || list_bytes < sizeof(unsigned) * ((size_t)N * N * zr.nz / C::V)) return AHS_ERR_INVALID_ARG;
     DiagPartial* extra = partials + blocks;
     unsigned long long* count = &partials[blocks + 1].n_pierced;
     if (cudaMemsetAsync(extra, 0, 2 * sizeof(DiagPartial), st) != cudaSuccess) return AHS_ERR_CUDA;
@@ -442,9 +443,9 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartia
     memset(&none, 0, sizeof(none));
     const bool use_tma = tmap && opt.staging == AHS_STAGING_TENSOR;
     const DiagMaps& mp = use_tma ? *tmap : none;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0);
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zr, nchunks, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
-    diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, (const unsigned*)list, count, extra);
+    diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, zr.periodic, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     const int r = launch_diag_finish(partials, (int)blocks + 1, result, st);
     return r < 0 ? r : 3;
@@ -452,17 +453,17 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartia
 
 // the tensor map of one (phi, theta) buffer for the tile shape above: box (TX + V, TY + 1, 1, 5)
 template <typename T>
-bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t array_bytes)
+bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes)
 {
     using G = typename DiagCfg<T>::G;
     if (!march_supported<T>(N)) return false;
-    return make_tile_map<T>(&out->tile, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 5) &&
-           make_tile_map<T>(&out->wrap, phi_re_base, N, array_bytes, 5, G::V, G::ROWS, 5);
+    return make_tile_map<T>(&out->tile, phi_re_base, N, nz_alloc, array_bytes, 5, G::PITCH, G::ROWS, 5) &&
+           make_tile_map<T>(&out->wrap, phi_re_base, N, nz_alloc, array_bytes, 5, G::V, G::ROWS, 5);
 }
-template bool make_diag_march_map<float>(DiagMaps*, const void*, int, size_t);
-template bool make_diag_march_map<double>(DiagMaps*, const void*, int, size_t);
+template bool make_diag_march_map<float>(DiagMaps*, const void*, int, int, size_t);
+template bool make_diag_march_map<double>(DiagMaps*, const void*, int, int, size_t);
 
-template int launch_diag_march<float>(const DiagPtrs<float>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
-template int launch_diag_march<double>(const DiagPtrs<double>&, int, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
+template int launch_diag_march<float>(const DiagPtrs<float>&, int, const ZRange&, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
+template int launch_diag_march<double>(const DiagPtrs<double>&, int, const ZRange&, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
 
 }  // namespace ahs

@@ -38,12 +38,16 @@ __device__ __forceinline__ double unit53(uint32_t hi, uint32_t lo)
 
 template <typename T>
 __global__ void __launch_bounds__(256) ic_kernel(T* __restrict__ phi_re, T* __restrict__ phi_im, int64_t nsites,
+                                                 int64_t plane_sites, int64_t lattice_sites, int64_t first_site,
                                                  double sigma, uint64_t seed, int kind)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t site = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; site < nsites; site += stride) {
+        // site index of the full lattice (the Philox counter, R9): local planes map to global planes periodically
+        int64_t gsite = first_site + site;
+        while (gsite >= lattice_sites) gsite -= lattice_sites;
         uint32_t r[4];
-        philox4x32_10((uint64_t)site, seed, r);
+        philox4x32_10((uint64_t)gsite, seed, r);
         double amp, ang;
         if (kind == AHS_IC_RANDOM_PHASE) {
             amp = sigma;
@@ -77,10 +81,12 @@ inline int grid_for(int64_t n)
 }  // namespace
 
 template <typename T>
-int launch_ic(T* phi_re, T* phi_im, int N, double sigma, uint64_t seed, int kind, cudaStream_t st)
+int launch_ic(T* phi_re, T* phi_im, int N, int nz_alloc, int z_first, double sigma, uint64_t seed, int kind, cudaStream_t st)
 {
-    const int64_t nsites = (int64_t)N * N * N;
-    ic_kernel<T><<<grid_for(nsites), 256, 0, st>>>(phi_re, phi_im, nsites, sigma, seed, kind);
+    const int64_t plane = (int64_t)N * N, nsites = plane * nz_alloc, lattice = plane * N;
+    const int64_t first = plane * (((int64_t)z_first % N + N) % N);
+    if (nz_alloc > N + 2) return AHS_ERR_INVALID_ARG;
+    ic_kernel<T><<<grid_for(nsites), 256, 0, st>>>(phi_re, phi_im, nsites, plane, lattice, first, sigma, seed, kind);
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
 
@@ -98,8 +104,8 @@ int launch_convert_to_double(const T* src, double* dst, int64_t n, cudaStream_t 
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
 
-template int launch_ic<float>(float*, float*, int, double, uint64_t, int, cudaStream_t);
-template int launch_ic<double>(double*, double*, int, double, uint64_t, int, cudaStream_t);
+template int launch_ic<float>(float*, float*, int, int, int, double, uint64_t, int, cudaStream_t);
+template int launch_ic<double>(double*, double*, int, int, int, double, uint64_t, int, cudaStream_t);
 template int launch_convert_from_double<float>(const double*, float*, int64_t, cudaStream_t);
 template int launch_convert_from_double<double>(const double*, double*, int64_t, cudaStream_t);
 template int launch_convert_to_double<float>(const float*, double*, int64_t, cudaStream_t);

@@ -52,6 +52,26 @@ struct DiagPartial {
     double wnum, wden;     // equation of state, Lagrangian weighted: sum p Lag, sum rho Lag (Eq. 12; R22)
 };
 
+// Which z-planes of the allocated arrays a handle owns.  A whole lattice: nz = nz_alloc = N, zbase = 0, periodic in z.  A z-slab
+// (ahs_group): nz own planes at local indices zbase = 1 .. nz, a ghost plane below (local 0, the lower neighbour's top
+// plane) and above (local nz + 1), no wrap: the neighbours keep the ghosts current (peer stores of the step kernel).
+struct ZRange {
+    int nz;         // own planes
+    int zbase;      // local index of the first own plane
+    int periodic;   // wrap z inside the array (whole lattice) or not (slab with ghost planes)
+    int nz_alloc;   // planes allocated per array
+};
+
+// Where the step kernel also stores the new (phi, theta) of its bottom / top own plane: the neighbouring slabs' ghost planes, in
+// THEIR output buffer (device pointers to the first element of the plane; peer memory over NVLink when the slab lives on another
+// GPU).  eps2_hi: the upper neighbour's ghost-below plane of eps_2 (the Gauss residual needs eps_2^{x-k_2}).  NULL = none.
+template <typename T>
+struct GhostPtrs {
+    T* lo[5];
+    T* hi[5];
+    T* eps2_hi;
+};
+
 template <typename T>
 struct FieldPtrs {
     const T* phi_re; const T* phi_im; const T* th[3];   // level n (read only)
@@ -89,25 +109,26 @@ struct SmemAttribute {
 };
 
 // ---- kernel launchers (each returns the number of kernels it launched, or a negative ahs error) -------------
-template <typename T> int launch_ic(T* phi_re, T* phi_im, int N, double sigma, uint64_t seed, int kind, cudaStream_t st);
+// IC on nz_alloc planes starting at global plane z_first (periodic): the Philox counter is the site index of the FULL N^3 lattice
+template <typename T> int launch_ic(T* phi_re, T* phi_im, int N, int nz_alloc, int z_first, double sigma, uint64_t seed, int kind, cudaStream_t st);
 template <typename T> int launch_step_generic(const FieldPtrs<T>& f, int N, const StepCoef& c, cudaStream_t st);
 // TMA descriptors of the step march: the four-array stage and theta_2 of one (phi, theta) buffer
 struct StepMaps { CUtensorMap stage, th2, wstage, wth2; };   // w*: the V-wide wrapped halo column of x-edge tiles
-template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps /* HOST, may be NULL */,
-                                            const MarchOptions& opt, cudaStream_t st);
-template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, size_t array_bytes);
+template <typename T> int launch_step_march(const FieldPtrs<T>& f, int N, const ZRange& zr, const GhostPtrs<T>* ghosts /* may be NULL */, const StepCoef& c,
+                                            const StepMaps* maps /* HOST, may be NULL */, const MarchOptions& opt, cudaStream_t st);
+template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes);
 template <typename T> bool march_supported(int N);
 template <typename T> int launch_diag_generic(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
                                               int max_partials, DiagPartial* result, cudaStream_t st);
 // TMA descriptors of the diagnostics march: the five-array forward-halo tile and the V-wide wrapped column of right-edge tiles
 struct DiagMaps { CUtensorMap tile, wrap; };
 // `list`: DEVICE scratch of >= 4 N^3 / (16 / sizeof(T)) bytes for the winding doubt list (the dead phi', theta' shadow buffer)
-template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
+template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagCoef& c, DiagPartial* partials,
                                             int max_partials, DiagPartial* result, void* list, size_t list_bytes,
                                             const DiagMaps* tmap /* HOST, may be NULL: row copies only */, const MarchOptions& opt,
                                             cudaStream_t st);
 // tensor map (TMA descriptor) of the five level-n arrays of one (phi, theta) buffer for the diagnostics march; false if unavailable
-template <typename T> bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, size_t array_bytes);
+template <typename T> bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes);
 int launch_diag_finish(const DiagPartial* partials, int n, DiagPartial* result, cudaStream_t st);
 template <typename T> int launch_convert_from_double(const double* src, T* dst, int64_t n, cudaStream_t st);
 template <typename T> int launch_convert_to_double(const T* src, double* dst, int64_t n, cudaStream_t st);

@@ -74,7 +74,7 @@ struct MarchCfg {
 
 template <typename T, int TY, int MINB, int NSTG>
 __global__ void __launch_bounds__(MarchCfg<T, TY, NSTG>::NTHREADS, MINB)
-step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
+step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks, StepCoefT<T> k, const __grid_constant__ CUtensorMap map_stage,
                   const __grid_constant__ CUtensorMap map_th2, const __grid_constant__ CUtensorMap map_wstage,
                   const __grid_constant__ CUtensorMap map_wth2, int use_tma)
 {
@@ -102,9 +102,9 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     const int tx = bid % tiles_x;
     bid /= tiles_x;
     const int ty = bid % tiles_y, zc = bid / tiles_y;
-    // z-chunk zc of nchunks: planes [zc N / nchunks, (zc + 1) N / nchunks) -- the chunks need not be of equal length
-    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * N / nchunks);
-    const int zlen = (int)((long long)(zc + 1) * N / nchunks) - z0;
+    // z-chunk zc of nchunks: own planes [zc nz / nchunks, (zc + 1) nz / nchunks) -- the chunks need not be of equal length
+    const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * zr.nz / nchunks);
+    const int zlen = (int)((long long)(zc + 1) * zr.nz / nchunks) - z0;
     const int xi = V * lane;
 
     const T* const src[4] = { f.phi_re, f.phi_im, f.th[0], f.th[1] };
@@ -118,8 +118,12 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     }
     __syncthreads();
 
-    // plane index i of this CTA's march = lattice plane z0 - 1 + i (periodic)
-    auto plane_of = [&](int i) { const int z = z0 - 1 + i; return z < 0 ? z + N : (z >= N ? z - N : z); };
+    // plane index i of this CTA's march = own plane z0 - 1 + i: periodic inside a whole lattice, running into the ghost planes of a slab
+    auto plane_of = [&](int i) {
+        int z = z0 - 1 + i;
+        if (zr.periodic) z = z < 0 ? z + N : (z >= N ? z - N : z);
+        return z + zr.zbase;
+    };
     // Tiles that do not touch the periodic boundary fetch a plane with two tensor copies (UTMALDG: the four-array stage
     // and theta_2) instead of 30 row copies; the others keep the row copies (TMA zero-fills out of bounds, it does not wrap).
     // x-edge tiles: the main box runs out of bounds on one side (zero-filled) and the wrapped halo column (x = N-V.. for the
@@ -207,7 +211,8 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
     // requested right after the barrier of plane it, where register pressure is lowest, and consumed at the end of phase 1
     // of plane it+1 (profiles/r1: requested at the top of their own plane they cost 15 % of the issue slots in stalls).
     const size_t plane_stride = (size_t)N * N;
-    size_t gnext = ((size_t)z0 * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+    size_t gnext = ((size_t)(zr.zbase + z0) * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
+    const size_t in_plane = (size_t)(y0 + w) * N + (size_t)(x0 + xi);   // offset inside a plane: for the neighbours' ghost planes
     VecT nPr = ldg_vec<T, V>(f.pi_re + gnext), nPi = ldg_vec<T, V>(f.pi_im + gnext);
     VecT nE0 = ldg_vec<T, V>(f.eps[0] + gnext), nE1 = ldg_vec<T, V>(f.eps[1] + gnext), nE2 = ldg_vec<T, V>(f.eps[2] + gnext);
 
@@ -392,6 +397,18 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
             stg_vec<T, V>(f.eps[0] + g, oE0); stg_vec<T, V>(f.eps[1] + g, oE1); stg_vec<T, V>(f.eps[2] + g, oE2);
             stg_vec<T, V>(f.phi_re_out + g, oFr); stg_vec<T, V>(f.phi_im_out + g, oFi);
             stg_vec<T, V>(f.th_out[0] + g, oT0); stg_vec<T, V>(f.th_out[1] + g, oT1); stg_vec<T, V>(f.th_out[2] + g, oT2);
+            // z-slabs: the new (phi, theta) of the bottom / top own plane also go into the neighbouring slabs' ghost planes (peer
+            // memory when they live on another GPU: the exchange of DESIGN.md 10 is these stores), eps_2 of the top plane as well
+            const int zown = z0 + it - 1;
+            if (zown == 0 && gh.lo[0] != nullptr) {
+                stg_vec<T, V>(gh.lo[0] + in_plane, oFr); stg_vec<T, V>(gh.lo[1] + in_plane, oFi);
+                stg_vec<T, V>(gh.lo[2] + in_plane, oT0); stg_vec<T, V>(gh.lo[3] + in_plane, oT1); stg_vec<T, V>(gh.lo[4] + in_plane, oT2);
+            }
+            if (zown == zr.nz - 1 && gh.hi[0] != nullptr) {
+                stg_vec<T, V>(gh.hi[0] + in_plane, oFr); stg_vec<T, V>(gh.hi[1] + in_plane, oFi);
+                stg_vec<T, V>(gh.hi[2] + in_plane, oT0); stg_vec<T, V>(gh.hi[3] + in_plane, oT1); stg_vec<T, V>(gh.hi[4] + in_plane, oT2);
+                stg_vec<T, V>(gh.eps2_hi + in_plane, oE2);
+            }
         }
     }
 }
@@ -401,29 +418,34 @@ step_march_kernel(FieldPtrs<T> f, int N, int nchunks, StepCoefT<T> k, const __gr
 // along z, their halo rows then miss L2, and every chunk boundary re-aligns them.  32 chunks (fp32) / 16 (fp64, twice the
 // tiles per plane) were fastest at 256^3, 512^3 and 1024^3 alike; chunk counts that do not divide N lose 3-6 % at small N.
 template <typename T>
-int pick_chunks(int N)
+int pick_chunks(int N, int nz)
 {
     int c = sizeof(T) == 4 ? 32 : 16;
     while (c > 1 && (N % c != 0 || N / c < 4)) c /= 2;
-    return c;
+    const int zlen = N / c;                 // planes per chunk, read off the whole lattice; a slab of nz planes gets nz / zlen chunks
+    return nz >= zlen ? nz / zlen : 1;
 }
 
 template <typename T, int TY, int MINB, int NSTG>
-int launch_cfg(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
+int launch_cfg(const FieldPtrs<T>& f, int N, const ZRange& zr, const GhostPtrs<T>* ghosts, const StepCoef& c, const StepMaps* maps,
+               const MarchOptions& opt, cudaStream_t st)
 {
     using C = MarchCfg<T, TY, NSTG>;
     auto kern = step_march_kernel<T, TY, MINB, NSTG>;
     static SmemAttribute attr;   // per device: the kernel needs more than the default 48 KB of dynamic shared memory
     if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
-    const int nchunks = (opt.step_chunks > 0 && opt.step_chunks <= N) ? opt.step_chunks : pick_chunks<T>(N);
+    const int nchunks = (opt.step_chunks > 0 && opt.step_chunks <= zr.nz) ? opt.step_chunks : pick_chunks<T>(N, zr.nz);
     const long blocks = (long)(N / C::TX) * (N / TY) * nchunks;
+    GhostPtrs<T> gh;
+    memset(&gh, 0, sizeof(gh));
+    if (ghosts) gh = *ghosts;
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
     if (maps && opt.staging == AHS_STAGING_TENSOR) {
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, k, maps->stage, maps->th2, maps->wstage, maps->wth2, 1);
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, gh, N, zr, nchunks, k, maps->stage, maps->th2, maps->wstage, maps->wth2, 1);
     } else {
         StepMaps none;
         memset(&none, 0, sizeof(none));
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, nchunks, k, none.stage, none.th2, none.wstage, none.wth2, 0);
+        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, gh, N, zr, nchunks, k, none.stage, none.th2, none.wstage, none.wth2, 0);
     }
     return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
 }
@@ -438,31 +460,32 @@ bool march_supported(int N)
 }
 
 template <typename T>
-int launch_step_march(const FieldPtrs<T>& f, int N, const StepCoef& c, const StepMaps* maps, const MarchOptions& opt, cudaStream_t st)
+int launch_step_march(const FieldPtrs<T>& f, int N, const ZRange& zr, const GhostPtrs<T>* ghosts, const StepCoef& c, const StepMaps* maps,
+                      const MarchOptions& opt, cudaStream_t st)
 {
-    if (!march_supported<T>(N)) return AHS_ERR_INVALID_ARG;
-    return launch_cfg<T, StepShape<T>::TY, StepShape<T>::MINB, StepShape<T>::NS>(f, N, c, maps, opt, st);
+    if (!march_supported<T>(N) || zr.nz < 1) return AHS_ERR_INVALID_ARG;
+    return launch_cfg<T, StepShape<T>::TY, StepShape<T>::MINB, StepShape<T>::NS>(f, N, zr, ghosts, c, maps, opt, st);
 }
 
 // the marching diagnostics kernel lives in ahs_diag_march.cu
 template bool march_supported<float>(int);
 template bool march_supported<double>(int);
-template int launch_step_march<float>(const FieldPtrs<float>&, int, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
-template int launch_step_march<double>(const FieldPtrs<double>&, int, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
+template int launch_step_march<float>(const FieldPtrs<float>&, int, const ZRange&, const GhostPtrs<float>*, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
+template int launch_step_march<double>(const FieldPtrs<double>&, int, const ZRange&, const GhostPtrs<double>*, const StepCoef&, const StepMaps*, const MarchOptions&, cudaStream_t);
 
 // tensor maps of one (phi, theta) buffer for the tile shape above
 template <typename T>
-bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, size_t array_bytes)
+bool make_step_march_maps(StepMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes)
 {
     using C = MarchCfg<T, StepShape<T>::TY, StepShape<T>::NS>;
     using G = typename C::G;
     if (!march_supported<T>(N)) return false;
-    return make_tile_map<T>(&out->stage, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
-           make_tile_map<T>(&out->th2, phi_re_base, N, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
-           make_tile_map<T>(&out->wstage, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 4) &&
-           make_tile_map<T>(&out->wth2, phi_re_base, N, array_bytes, 5, C::V, G::ROWS, 1);
+    return make_tile_map<T>(&out->stage, phi_re_base, N, nz_alloc, array_bytes, 5, G::PITCH, G::ROWS, 4) &&
+           make_tile_map<T>(&out->th2, phi_re_base, N, nz_alloc, array_bytes, 5, G::PITCH, G::ROWS, 1) &&
+           make_tile_map<T>(&out->wstage, phi_re_base, N, nz_alloc, array_bytes, 5, C::V, G::ROWS, 4) &&
+           make_tile_map<T>(&out->wth2, phi_re_base, N, nz_alloc, array_bytes, 5, C::V, G::ROWS, 1);
 }
-template bool make_step_march_maps<float>(StepMaps*, const void*, int, size_t);
-template bool make_step_march_maps<double>(StepMaps*, const void*, int, size_t);
+template bool make_step_march_maps<float>(StepMaps*, const void*, int, int, size_t);
+template bool make_step_march_maps<double>(StepMaps*, const void*, int, int, size_t);
 
 }  // namespace ahs

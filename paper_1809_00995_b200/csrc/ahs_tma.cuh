@@ -35,7 +35,7 @@ __device__ __forceinline__ void tma_prefetch_descriptor(const CUtensorMap* map)
 // spaced by array_bytes, with a box of (box_x, box_y, 1, box_a) elements.  Returns false if the driver entry point is
 // missing or the encode fails (the callers then keep the row-copy path).
 template <typename T>
-inline bool make_tile_map(CUtensorMap* out, const void* base, int N, size_t array_bytes, int narrays, int box_x, int box_y, int box_a)
+inline bool make_tile_map(CUtensorMap* out, const void* base, int N, int nz_alloc, size_t array_bytes, int narrays, int box_x, int box_y, int box_a)
 {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -46,7 +46,7 @@ inline bool make_tile_map(CUtensorMap* out, const void* base, int N, size_t arra
         return reinterpret_cast<EncodeFn>(fn);
     }();
     if (!encode) { cudaGetLastError(); return false; }
-    const cuuint64_t gdim[4] = { (cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)narrays };
+    const cuuint64_t gdim[4] = { (cuuint64_t)N, (cuuint64_t)N, (cuuint64_t)nz_alloc, (cuuint64_t)narrays };
     const cuuint64_t gstride[3] = { (cuuint64_t)N * sizeof(T), (cuuint64_t)N * N * sizeof(T), (cuuint64_t)array_bytes };
     const cuuint32_t box[4] = { (cuuint32_t)box_x, (cuuint32_t)box_y, 1u, (cuuint32_t)box_a };
     const cuuint32_t estr[4] = { 1u, 1u, 1u, 1u };

@@ -678,3 +678,61 @@ def test_table4_script_runs_through_the_library(ahs):
         assert 0.2 < r["xi_dot"] < 0.5 and 0.15 < r["xi_L_dot"] < 0.6, r
         assert 0.0 < r["v2_V"] < 1.0 and 0.0 < r["v2_omega"] < 1.0, r
         assert r["gauss_max"] < 1e-4, r
+
+
+# ---------------------------------------------------------------------------------------------------------
+# z-slab decomposition (ahs_group): every slab on THIS GPU -- the same kernels, peer stores and event
+# ordering as across GPUs, launched one after another (nothing waits on the device)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,N,slabs", [("f32", 256, (1, 2, 4, 8)), ("f64", 128, (2, 4)), ("f32", 128, (2, 32))])
+def test_slab_group_reproduces_the_single_lattice_bit_for_bit(ahs, prec, N, slabs):
+    """A lattice cut into P z-slabs with ghost planes kept current by the step kernel's stores into the neighbours' memory must
+    evolve exactly like the whole lattice on one handle: fields bit for bit (every site's arithmetic is the same), winding counts
+    exactly, fp64 sums to the order of the final reduction, Gauss's law at roundoff across the slab faces."""
+    nsteps = 12
+    with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.0, seed=77) as ref:
+        ic = ref.get_fields_native()
+        ref.step(nsteps)
+        want, dref = ref.get_fields_native(), ref.diagnostics()
+    for P in slabs:
+        with ahs.Group(N=N, nslabs=P, precision=prec, m=1.0, s=0.0, seed=77) as g:
+            assert np.array_equal(g.get_fields_native(), ic), P                       # the same Philox initial condition, slab by slab
+            g.step(5)
+            d5 = g.diagnostics()
+            g.step(nsteps - 5)
+            got, d = g.get_fields_native(), g.diagnostics()
+            assert np.array_equal(got, want), (P, [int((got[k] != want[k]).sum()) for k in range(10)])
+            assert d["step"] == nsteps and d5["step"] == 5
+            assert (d["n_pierced"], d["sum_abs_w"], d["nonfinite"]) == (dref["n_pierced"], dref["sum_abs_w"], 0), P
+            for key in ("v2_num", "v2_den", "v2v_num", "v2v_den", "eos_num", "eos_den", "mean_lagrangian", "gauss_rhs_rms"):
+                assert d[key] == pytest.approx(dref[key], rel=1e-11, abs=1e-11 * abs(dref["v2_den"])), (P, key)
+            assert d["gauss_max"] == dref["gauss_max"], P
+
+
+def test_slab_group_from_uploaded_fields_and_options(ahs, oracle):
+    """ahs_group_set_fields_native fills the ghost planes from the neighbours; then 20 steps against the ORACLE (all ten fields
+    non-zero from the start), with a chunk count that does not divide the slab and row-copy staging on one of the runs."""
+    from paper_1809_00995_b200 import synthetic
+    N, nsteps = 128, 20
+    f0 = synthetic.random_snapshot(N, seed=31).astype(np.float32)
+    p = oracle.Params(N=N, m=2.0, s=0.0, tau0=2.0)
+    ref = oracle.step(p, f0.astype(np.float64), 3, nsteps)
+    for P, opts in ((4, {}), (2, {ahs.AHS_OPT_STEP_CHUNKS: 7, ahs.AHS_OPT_DIAG_CHUNKS: 3}), (8, {ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS})):
+        with ahs.Group(N=N, nslabs=P, precision="f32", m=2.0, s=0.0, tau0=2.0, ic="none") as g:
+            for k, v in opts.items():
+                g.set_option(k, v)
+            g.set_fields_native(f0, step=3)
+            assert np.array_equal(g.get_fields_native(), f0)
+            g.step(nsteps)
+            got = g.get_fields_native().astype(np.float64)
+            assert_fields("slab_group_vs_oracle", got, ref, "f32", oracle.FIELD_NAMES, N=N, slabs=P, nsteps=nsteps)
+            d = g.diagnostics()
+            r = oracle.diagnostics(p, got, 3 + nsteps)                                   # the oracle on the group's own snapshot
+            assert (d["n_pierced"], d["sum_abs_w"]) == (r["n_pierced"], r["sum_abs_w"])
+            K, G, Lg = oracle.site_fields(p, got, 3 + nsteps)
+            assert abs(d["v2_num"] - r["v2_num"]) <= 2e-5 * np.abs(K * Lg).sum()
+            assert abs(d["gauss_max"] - r["gauss_max"]) <= 64 * 6e-8 * max(1.0, r["gauss_rhs_rms"], np.abs(got[7:10]).max())
+    with pytest.raises(ahs.AhsError):
+        ahs.Group(N=N, nslabs=3)                                                          # must divide N
+    with pytest.raises(ahs.AhsError):
+        ahs.Group(N=N, nslabs=2, devices=[0, 99])
