@@ -64,6 +64,9 @@ def parse_args():
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "march"])
     ap.add_argument("--e2e-steps", type=int, default=4, help="timed end-to-end steps (each uploads the full state)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--slabs", type=int, default=0, help="cut the lattice into this many z-slabs (ahs_group, DESIGN.md 10) driven by this one "
+                    "process; 0 = one handle")
+    ap.add_argument("--slab-devices", default="", help="comma-separated CUDA ordinals, one per slab (default: all on this rank's GPU)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-lattice", type=int, default=128, help="lattice of the oracle's bounded sample")
     ap.add_argument("--cpu-leapfrog", type=int, default=10)
@@ -193,7 +196,8 @@ def workload_config(args) -> dict:
                         % (N, args.precision, args.m, args.s, SEED, args.leapfrog, name, ", tau_ref=%g" % args.tau_ref if args.tau_ref else ""),
             "lattice": N, "leapfrog_per_step": args.leapfrog, "diagnostics_per_step": 1,
             "l2": "inputs larger than L2 (%.1f GB of fields streamed per leapfrog launch)" % (N ** 3 * BYTES_PER_SITE[args.precision] / 1e9),
-            "parallelism": "replicas x%d" % args.gpus}
+            "parallelism": "replicas x%d" % args.gpus + (", each lattice cut into %d z-slabs on devices [%s]" % (args.slabs, args.slab_devices or "this rank's GPU")
+                                                          if args.slabs else "")}
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -249,7 +253,14 @@ def run_ours(args):
 
     N, L, K, W = args.lattice, args.leapfrog, args.steps, args.warmup
     sites = N ** 3
-    sim = ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank, kernel=args.kernel, tau_ref=args.tau_ref, **COMMON)
+    if args.slabs:
+        devs = [int(d) for d in args.slab_devices.split(",")] if args.slab_devices else [local] * args.slabs
+        sim = ahs.Group(N=N, nslabs=args.slabs, devices=devs, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank,
+                        tau_ref=args.tau_ref, **COMMON)
+        sim.kernel_kind = "march"
+        args.no_e2e = True                 # (the end-to-end leg is the single-handle path)
+    else:
+        sim = ahs.Simulation(N=N, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank, kernel=args.kernel, tau_ref=args.tau_ref, **COMMON)
     diag = None
     for _ in range(W):
         sim.step(L)
@@ -267,8 +278,10 @@ def run_ours(args):
     for a, b, c in marks:
         a.record()
         sim.step(L)                 # L fused leapfrog launches, asynchronous
+        if args.slabs:
+            sim.synchronize()       # the slabs run on their own streams: bring their work in front of the event
         b.record()
-        diag = sim.diagnostics()    # diagnostics kernels + 64-byte record to the host (synchronises)
+        diag = sim.diagnostics()    # diagnostics kernels + the record to the host (synchronises)
         c.record()
     stop.record()
     barrier()
