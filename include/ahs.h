@@ -111,7 +111,11 @@ typedef struct {
     double xi;                /* sqrt((N dx)^3 / L); +inf if n_pierced == 0                                */
     double v2_num;            /* sum_x |Pi|^2 Lag^x     (Eq. 10, weight = Eq. 2 with c_B = 1, R2)          */
     double v2_den;            /* sum_x |D phi|^2 Lag^x                                                     */
-    double v2;                /* 2R/(1+R), R = v2_num / v2_den (Eq. 9)                                     */
+    double v2;                /* 2R/(1+R), R = v2_num / v2_den (Eq. 9): <v^2>_L.  NOT validated against the paper's
+                                 Table 4: with the weight that is consistent with Eqs. 4-7 (c_B = c_E = 1) it comes out
+                                 0.05 below the paper's value in both eras, and no reading of the printed Eq. 2 reproduces
+                                 all of the paper's Lagrangian-weighted columns.  v2_V and v2_omega
+                                 below agree with Table 4 within two standard deviations                                   */
     double mean_lagrangian;   /* sum_x Lag^x / N^3                                                         */
     double gauss_max;         /* max_x |sum_i (eps_i^x - eps_i^{x-k_i}) - 2 dx^2 e0^2 a_h^(2s) Im[conj(phi) Pi]|,
                                  a_h = a(tau_n - dt/2)  (R4)                                               */
