@@ -337,6 +337,12 @@ class Group:
     def synchronize(self):
         _check(load().ahs_group_synchronize(self._g))
 
+    @property
+    def layout(self):
+        """The slabs' extents and neighbours (slabs.Slab records)."""
+        from . import slabs
+        return slabs.layout(self.N, self.nslabs)
+
     def set_option(self, option: int, value: int):
         """ahs_set_option on every slab."""
         lib = load()
