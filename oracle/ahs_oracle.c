@@ -70,6 +70,10 @@ typedef struct {
     double c_B;       /* factor on the plaquette sum of Eq. 2; 1 = consistent with Eq. 5 (R2)   */
     double c_E;       /* factor on the electric term of Eq. 2 IN THE WEIGHT; 1 = eps = d theta/d eta (R5);
                          (dt/dx)^2 = the rescaling "E -> e dt E" of L44 read literally (R21)          */
+    int32_t ns;       /* knots of a time-dependent s(tau) (L66-70: core growth, then s = 1); 0 = constant s     */
+    int32_t pad_;
+    const double* sched_tau;   /* ns increasing conformal times                                      (R23)      */
+    const double* sched_s;     /* s at the knots; linear in between, constant outside                           */
 } aho_params;
 
 typedef struct {
@@ -194,8 +198,21 @@ void aho_ic_window(const aho_params* p, uint64_t seed, int32_t kind, int64_t Nfu
  * Scale factor and running couplings (a ~ eta^m ; Eq. 8).
  * -------------------------------------------------------------------------------------------- */
 static double aho_a(const aho_params* p, double tau) { return pow(tau / p->tau_ref, p->m); }
-static double aho_e(const aho_params* p, double a) { return p->e0 * pow(a, p->s - 1.0); }
-static double aho_lambda(const aho_params* p, double a) { return p->lambda0 * pow(a, 2.0 * (p->s - 1.0)); }
+/* s of Eq. 8 at conformal time tau: the constant p->s, or the piecewise-linear schedule (R23: the paper's runs "with core
+ * growth" change s during the run, L66-70, but do not give the schedule) */
+static double aho_s(const aho_params* p, double tau)
+{
+    if (p->ns <= 0) return p->s;
+    if (tau <= p->sched_tau[0]) return p->sched_s[0];
+    for (int32_t k = 1; k < p->ns; ++k)
+        if (tau <= p->sched_tau[k]) {
+            const double w = (tau - p->sched_tau[k - 1]) / (p->sched_tau[k] - p->sched_tau[k - 1]);
+            return p->sched_s[k - 1] + w * (p->sched_s[k] - p->sched_s[k - 1]);
+        }
+    return p->sched_s[p->ns - 1];
+}
+static double aho_e(const aho_params* p, double a, double tau) { return p->e0 * pow(a, aho_s(p, tau) - 1.0); }
+static double aho_lambda(const aho_params* p, double a, double tau) { return p->lambda0 * pow(a, 2.0 * (aho_s(p, tau) - 1.0)); }
 static double aho_tau(const aho_params* p, int64_t n) { return p->tau0 + (double)n * p->dt; }
 
 /* ----------------------------------------------------------------------------------------------
@@ -216,8 +233,8 @@ void aho_coeffs(const aho_params* p, int64_t n, double c[6])
     const double am = aho_a(p, tau - 0.5 * p->dt);
     const double a0 = aho_a(p, tau);
     const double ap = aho_a(p, tau + 0.5 * p->dt);
-    const double em = aho_e(p, am), e0 = aho_e(p, a0), ep = aho_e(p, ap);
-    const double lam0 = aho_lambda(p, a0);
+    const double em = aho_e(p, am, tau - 0.5 * p->dt), e0 = aho_e(p, a0, tau), ep = aho_e(p, ap, tau + 0.5 * p->dt);
+    const double lam0 = aho_lambda(p, a0, tau);
     const double idx2 = 1.0 / (p->dx * p->dx);
     c[0] = (am / ap) * (am / ap);
     c[1] = p->dt * idx2 * (a0 / ap) * (a0 / ap);
@@ -409,7 +426,7 @@ void aho_winding(const aho_params* p, const double* f10, int32_t* W3, uint64_t* 
  * El and Bm (always with unit factors) are the electric and magnetic energy densities of the equation-of-state
  * estimator, Eq. 12.
  * -------------------------------------------------------------------------------------------- */
-static void aho_site_lagrangian(const aho_params* p, const double* f10, double a,
+static void aho_site_lagrangian(const aho_params* p, const double* f10, double a, double tau,
                                 int64_t x, int64_t y, int64_t z, double out6[6])
 {
     const int64_t N = p->N, V = N * N * N;
@@ -420,7 +437,7 @@ static void aho_site_lagrangian(const aho_params* p, const double* f10, double a
     const double* const eps[3] = { f10 + 7 * V, f10 + 8 * V, f10 + 9 * V };
     const int64_t s0 = x + N * (y + N * z);
     const double idx2 = 1.0 / (p->dx * p->dx);
-    const double ea = aho_e(p, a), la = aho_lambda(p, a);
+    const double ea = aho_e(p, a, tau), la = aho_lambda(p, a, tau);
     const double fr = phr[s0], fi = phi_[s0];
     double G = 0.0;
     for (int i = 0; i < 3; ++i) {
@@ -487,7 +504,8 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
     const double tau = aho_tau(p, n);
     const double a = aho_a(p, tau);
     const double ah = aho_a(p, tau - 0.5 * p->dt);
-    const double grhs = 2.0 * q * p->dx * p->dx * p->e0 * p->e0 * pow(ah, 2.0 * p->s);
+    const double eh = aho_e(p, ah, tau - 0.5 * p->dt);   /* e(a_h)^2 a_h^2 = e0^2 a_h^(2s) for a constant s */
+    const double grhs = 2.0 * q * p->dx * p->dx * eh * eh * ah * ah;
     /* per z-plane sums in x-fastest order (planes are independent), then the planes added in z order */
     double* plane = (double*)malloc((size_t)N * 9 * sizeof(double));
 #pragma omp parallel for num_threads(aho_threads) schedule(static)
@@ -497,7 +515,7 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
         for (int64_t x = 0; x < N; ++x) {
             const int64_t s0 = x + N * (y + N * z);
             double kgl[6];
-            aho_site_lagrangian(p, f10, a, x, y, z, kgl);
+            aho_site_lagrangian(p, f10, a, tau, x, y, z, kgl);
             num  += kgl[0] * kgl[2];
             den  += kgl[1] * kgl[2];
             lsum += kgl[2];
@@ -551,13 +569,14 @@ void aho_diag_compute(const aho_params* p, const double* f10, int64_t n, aho_dia
 void aho_site_fields4(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag, double* Vp)
 {
     const int64_t N = p->N;
-    const double a = aho_a(p, aho_tau(p, n));
+    const double tau = aho_tau(p, n);
+    const double a = aho_a(p, tau);
 #pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
         double kgl[6];
-        aho_site_lagrangian(p, f10, a, x, y, z, kgl);
+        aho_site_lagrangian(p, f10, a, tau, x, y, z, kgl);
         const int64_t s0 = x + N * (y + N * z);
         K[s0] = kgl[0]; G[s0] = kgl[1]; Lag[s0] = kgl[2];
         if (Vp) Vp[s0] = kgl[3];
@@ -567,13 +586,14 @@ void aho_site_fields4(const aho_params* p, const double* f10, int64_t n, double*
 void aho_site_fields6(const aho_params* p, const double* f10, int64_t n, double* K, double* G, double* Lag, double* Vp, double* El, double* Bm)
 {
     const int64_t N = p->N;
-    const double a = aho_a(p, aho_tau(p, n));
+    const double tau = aho_tau(p, n);
+    const double a = aho_a(p, tau);
 #pragma omp parallel for num_threads(aho_threads) schedule(static)
     for (int64_t z = 0; z < N; ++z)
     for (int64_t y = 0; y < N; ++y)
     for (int64_t x = 0; x < N; ++x) {
         double kgl[6];
-        aho_site_lagrangian(p, f10, a, x, y, z, kgl);
+        aho_site_lagrangian(p, f10, a, tau, x, y, z, kgl);
         const int64_t s0 = x + N * (y + N * z);
         K[s0] = kgl[0]; G[s0] = kgl[1]; Lag[s0] = kgl[2]; Vp[s0] = kgl[3]; El[s0] = kgl[4]; Bm[s0] = kgl[5];
     }

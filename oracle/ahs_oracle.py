@@ -41,7 +41,8 @@ def build(force: bool = False) -> str:
 class _Params(C.Structure):
     _fields_ = [("N", C.c_int32), ("q", C.c_int32), ("dx", C.c_double), ("dt", C.c_double),
                 ("lambda0", C.c_double), ("e0", C.c_double), ("sigma", C.c_double), ("m", C.c_double),
-                ("s", C.c_double), ("tau0", C.c_double), ("tau_ref", C.c_double), ("c_B", C.c_double), ("c_E", C.c_double)]
+                ("s", C.c_double), ("tau0", C.c_double), ("tau_ref", C.c_double), ("c_B", C.c_double), ("c_E", C.c_double),
+                ("ns", C.c_int32), ("pad_", C.c_int32), ("sched_tau", C.POINTER(C.c_double)), ("sched_s", C.POINTER(C.c_double))]
 
 
 class _Diag(C.Structure):
@@ -69,11 +70,19 @@ class Params:
     q: int = 1
     c_B: float = 1.0
     c_E: float = 1.0      # factor on the electric term in the weight; (dt/dx)^2 = L44's "E -> e dt E" read literally (R21)
+    s_schedule: tuple = ()   # ((tau_0, s_0), (tau_1, s_1), ...): piecewise-linear s(tau) (R23); empty = the constant s
 
     def _c(self) -> _Params:
         tref = self.tau_ref if self.tau_ref != 0.0 else self.tau0
-        return _Params(self.N, self.q, self.dx, self.dt, self.lambda0, self.e0, self.sigma, self.m,
-                       self.s, self.tau0, tref, self.c_B, self.c_E)
+        c = _Params(self.N, self.q, self.dx, self.dt, self.lambda0, self.e0, self.sigma, self.m,
+                    self.s, self.tau0, tref, self.c_B, self.c_E)
+        if self.s_schedule:
+            k = len(self.s_schedule)
+            c._keep = ((C.c_double * k)(*[float(t) for t, _ in self.s_schedule]), (C.c_double * k)(*[float(v) for _, v in self.s_schedule]))
+            c.ns = k
+            c.sched_tau = C.cast(c._keep[0], C.POINTER(C.c_double))
+            c.sched_s = C.cast(c._keep[1], C.POINTER(C.c_double))
+        return c
 
 
 _lib = None

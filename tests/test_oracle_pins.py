@@ -902,3 +902,54 @@ def test_equation_of_state_estimator(oracle):
     d2 = oracle.diagnostics(q, f2, 25)
     for key in ("eos_num", "eos_den", "v2_omega", "v2_num"):
         assert d[key] == pytest.approx(d2[key], rel=1e-10)
+
+
+# ------------------------------------------------------------------------------------------------
+# NEXT-3, second half: a time-dependent s(tau) (core growth, then s = 1; R23)
+# ------------------------------------------------------------------------------------------------
+def test_s_schedule(oracle):
+    """The paper changes s during a run ("controlled throughout the simulation", L70) but gives no schedule: ours is piecewise
+    linear in tau (a labelled assumption).  (1) A constant schedule is the constant s, bit for bit.  (2) The six coefficients of a
+    step that straddles a ramp, written out by hand: each coupling takes s at ITS OWN time level (e_{n+-1/2}, e_n, lambda_n).
+    (3) Gauss's law stays at roundoff across growth, ramp and s = 1 -- it holds for any e(tau) only if d1, d2 and the residual use
+    e at tau_{n+-1/2} consistently (using e_n in d2, or s(tau_n) in the residual, breaks it at O(1); shown).  (4) The homogeneous mode
+    follows the scalar recurrence with the scheduled lambda."""
+    N = 8
+    sched = ((1.0, -1.0), (2.0, -1.0), (3.0, 1.0))                       # growth (s = -1) to tau = 2, ramp to s = 1 at tau = 3
+    s_of = lambda t: -1.0 if t <= 2 else (1.0 if t >= 3 else -1.0 + 2.0 * (t - 2.0))
+    p = oracle.Params(N=N, m=1, s=0.25, tau0=1.0, dt=0.1, dx=0.5, lambda0=2.0, e0=1.0)
+    # (1)
+    f = oracle.initial_condition(p, 4)
+    g = f.copy()
+    oracle.step(p, f, 0, 25)
+    oracle.step(oracle.Params(**{**oracle.params_dict(p), "s_schedule": ((0.0, 0.25), (50.0, 0.25))}), g, 0, 25)
+    assert np.array_equal(f, g)
+    # (2) step n = 14: tau_n = 2.4, tau_{n-1/2} = 2.35, tau_{n+1/2} = 2.45 -- all inside the ramp, all different s
+    ps = oracle.Params(**{**oracle.params_dict(p), "s_schedule": sched})
+    n = 14
+    tm, t0, tp = 2.35, 2.4, 2.45
+    am, a0, ap = tm, t0, tp                                                # a = tau / tau_ref, tau_ref = tau0 = 1, m = 1
+    e = lambda a, t: a ** (s_of(t) - 1.0)
+    lam0 = 2.0 * a0 ** (2.0 * (s_of(t0) - 1.0))
+    want = [(am / ap) ** 2, 0.1 / 0.25 * (a0 / ap) ** 2, 0.1 * (a0 * a0 / ap) ** 2 * lam0 / 2,
+            (e(ap, tp) / e(am, tm)) ** 2, 2 * 0.1 * a0 ** 2 * e(ap, tp) ** 2, 0.1 / 0.25 * (e(ap, tp) / e(a0, t0)) ** 2]
+    np.testing.assert_allclose(oracle.coeffs(ps, n), want, rtol=1e-13)
+    # (3)
+    f = oracle.initial_condition(ps, 4)
+    for k in range(0, 30, 5):                                              # tau 1 -> 4: growth, ramp, s = 1
+        oracle.step(ps, f, k, 5)
+        d = oracle.diagnostics(ps, f, k + 5)
+        assert d["gauss_max"] <= 1e-12 * max(1.0, d["gauss_rhs_rms"]), (k, d["gauss_max"], d["gauss_rhs_rms"])
+    #     teeth: the residual evaluated with the constant s of the snapshot's level instead of the schedule at tau_{n-1/2}
+    bad = oracle.diagnostics(oracle.Params(**{**oracle.params_dict(p), "s": s_of(2.4)}), oracle.step(ps, oracle.initial_condition(ps, 4), 0, 14), 14)
+    assert bad["gauss_max"] > 1e-3 * bad["gauss_rhs_rms"]
+    # (4) homogeneous real phi = f(tau), theta = 0:  pi <- c1 pi - c3 (f^2 - sigma^2) f ;  f <- f + dt pi
+    one = np.ones((N, N, N))
+    f = pack(0.3 * one + 0j, 0j * one, [0 * one] * 3, [0 * one] * 3)
+    fv, pv = 0.3, 0.0
+    for k in range(30):
+        c = oracle.coeffs(ps, k)
+        oracle.step(ps, f, k, 1)
+        pv = c[0] * pv - c[2] * (fv * fv - 1.0) * fv
+        fv = fv + 0.1 * pv
+    assert np.abs(f[0] - fv).max() < 1e-13 and np.abs(f[2] - pv).max() < 1e-13
