@@ -205,6 +205,13 @@ AHS_API int32_t ahs_set_option(ahs_sim* sim, int32_t option, int32_t value);
  * them. out6: HOST. */
 AHS_API int32_t ahs_coefficients(ahs_sim* sim, int64_t n, double* out6);
 
+/* A time-dependent s of Eq. 8 (L66-70: "this parameter can be controlled throughout the simulation", e.g. core growth with s < 0 and the
+ * true equations, s = 1, thereafter).  The paper does not give its schedule; this one is piecewise linear in conformal time: nknots
+ * strictly increasing times tau[] with values s_values[] (HOST arrays, copied), linear in between, constant outside (R23).  Every coupling
+ * of Eqs. 4-5 takes s at its own time level (e at tau_n -+ dt/2 and tau_n, lambda at tau_n), and so do the weights and the Gauss residual
+ * of the diagnostics.  nknots = 0 restores the constant ahs_params.s.  Takes effect at the next step / diagnostics call. */
+AHS_API int32_t ahs_set_s_schedule(ahs_sim* sim, int32_t nknots, const double* tau, const double* s_values);
+
 /* Block until all work of the handle has finished. */
 AHS_API int32_t ahs_synchronize(ahs_sim* sim);
 

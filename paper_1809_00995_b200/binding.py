@@ -27,7 +27,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "theta_0", "theta_1", "thet
 SYMBOLS = (
     "ahs_required_bytes", "ahs_create", "ahs_create_ex", "ahs_step", "ahs_diagnostics", "ahs_diagnostics_ex",
     "ahs_diagnostics_launch", "ahs_diagnostics_fetch", "ahs_get_fields", "ahs_set_fields", "ahs_get_fields_native",
-    "ahs_set_fields_native", "ahs_set_fields_native_async", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_coefficients",
+    "ahs_set_fields_native", "ahs_set_fields_native_async", "ahs_field_device_ptr", "ahs_get_state", "ahs_kernel_kind", "ahs_set_option", "ahs_set_s_schedule", "ahs_coefficients",
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
     "ahs_group_create", "ahs_group_step", "ahs_group_diagnostics", "ahs_group_get_fields_native", "ahs_group_set_fields_native",
     "ahs_group_synchronize", "ahs_group_slab_count", "ahs_group_slab", "ahs_group_destroy",
@@ -85,6 +85,7 @@ def load(path: str | None = None):
     lib.ahs_get_state.argtypes = [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(i64)]; lib.ahs_get_state.restype = i32
     lib.ahs_kernel_kind.argtypes = [vp]; lib.ahs_kernel_kind.restype = i32
     lib.ahs_set_option.argtypes = [vp, i32, i32]; lib.ahs_set_option.restype = i32
+    lib.ahs_set_s_schedule.argtypes = [vp, i32, C.POINTER(dbl), C.POINTER(dbl)]; lib.ahs_set_s_schedule.restype = i32
     lib.ahs_coefficients.argtypes = [vp, i64, C.POINTER(dbl)]; lib.ahs_coefficients.restype = i32
     lib.ahs_synchronize.argtypes = [vp]; lib.ahs_synchronize.restype = i32
     lib.ahs_destroy.argtypes = [vp]; lib.ahs_destroy.restype = i32
@@ -269,6 +270,10 @@ class Simulation:
     def set_option(self, option: int, value: int):
         _check(load().ahs_set_option(self._h, int(option), int(value)))
 
+    def set_s_schedule(self, knots):
+        """ahs_set_s_schedule: knots = ((tau_0, s_0), (tau_1, s_1), ...); () restores the constant s."""
+        _check(_set_s_schedule(self._h, knots))
+
     def coefficients(self, n: int) -> np.ndarray:
         out = (C.c_double * 6)()
         _check(load().ahs_coefficients(self._h, int(n), out))
@@ -276,6 +281,13 @@ class Simulation:
 
     def synchronize(self):
         _check(load().ahs_synchronize(self._h))
+
+
+def _set_s_schedule(handle, knots):
+    k = len(knots)
+    t = (C.c_double * max(k, 1))(*[float(a) for a, _ in knots])
+    v = (C.c_double * max(k, 1))(*[float(b) for _, b in knots])
+    return load().ahs_set_s_schedule(handle, k, t, v)
 
 
 class Group:
@@ -342,6 +354,12 @@ class Group:
         """The slabs' extents and neighbours (slabs.Slab records)."""
         from . import slabs
         return slabs.layout(self.N, self.nslabs)
+
+    def set_s_schedule(self, knots):
+        """ahs_set_s_schedule on every slab."""
+        lib = load()
+        for r in range(lib.ahs_group_slab_count(self._g)):
+            _check(_set_s_schedule(C.c_void_p(lib.ahs_group_slab(self._g, r)), knots))
 
     def set_option(self, option: int, value: int):
         """ahs_set_option on every slab."""

@@ -43,6 +43,8 @@ struct ahs_sim {
     void* ghost_lo[2][5];
     void* ghost_hi[2][5];
     void* ghost_eps2_hi;
+    // time-dependent s(tau) of Eq. 8 (ahs_set_s_schedule; R23): knots, empty = the constant p.s
+    std::vector<double> sched_tau, sched_s;
 };
 
 struct SlabSpec { int nz; int z_offset; };
@@ -95,20 +97,32 @@ double scale_factor(const ahs_params& p, double tau)
     const double tref = (p.tau_ref != 0.0) ? p.tau_ref : p.tau0;
     return std::pow(tau / tref, p.m);
 }
-double e_of(const ahs_params& p, double a) { return p.e * std::pow(a, p.s - 1.0); }
-double lambda_of(const ahs_params& p, double a) { return p.lambda * std::pow(a, 2.0 * (p.s - 1.0)); }
+// s of Eq. 8 at conformal time tau: constant, or piecewise linear between the knots of ahs_set_s_schedule (constant outside)
+double s_of(const ahs_sim* sim, double tau)
+{
+    const std::vector<double>& t = sim->sched_tau;
+    const std::vector<double>& v = sim->sched_s;
+    if (t.empty()) return sim->p.s;
+    if (tau <= t.front()) return v.front();
+    for (size_t k = 1; k < t.size(); ++k)
+        if (tau <= t[k]) return v[k - 1] + (tau - t[k - 1]) / (t[k] - t[k - 1]) * (v[k] - v[k - 1]);
+    return v.back();
+}
+double e_of(const ahs_sim* sim, double a, double tau) { return sim->p.e * std::pow(a, s_of(sim, tau) - 1.0); }
+double lambda_of(const ahs_sim* sim, double a, double tau) { return sim->p.lambda * std::pow(a, 2.0 * (s_of(sim, tau) - 1.0)); }
 
 // Coefficients of Eqs. 4-5 for the step n -> n+1 (L55-57): scale factors at tau_n -+ dt/2 and tau_n.
-StepCoef step_coefficients(const ahs_params& p, int64_t n)
+StepCoef step_coefficients(const ahs_sim* sim, int64_t n)
 {
+    const ahs_params& p = sim->p;
     const double tau = tau_of(p, n);
     const double a_m = scale_factor(p, tau - 0.5 * p.dt), a_0 = scale_factor(p, tau), a_p = scale_factor(p, tau + 0.5 * p.dt);
-    const double e_m = e_of(p, a_m), e_0 = e_of(p, a_0), e_p = e_of(p, a_p);
+    const double e_m = e_of(sim, a_m, tau - 0.5 * p.dt), e_0 = e_of(sim, a_0, tau), e_p = e_of(sim, a_p, tau + 0.5 * p.dt);   // each at its own level
     StepCoef c;
     const double r_mp = a_m / a_p, r_0p = a_0 / a_p, q_0p = a_0 * a_0 / a_p;
     c.c1 = r_mp * r_mp;                                       // (a_{n-1/2}/a_{n+1/2})^2
     c.c2 = p.dt / (p.dx * p.dx) * r_0p * r_0p;                // dt/dx^2 (a_n/a_{n+1/2})^2
-    c.c3 = p.dt * q_0p * q_0p * lambda_of(p, a_0) * 0.5;      // dt (a_n^2/a_{n+1/2})^2 lambda_n/2
+    c.c3 = p.dt * q_0p * q_0p * lambda_of(sim, a_0, tau) * 0.5;   // dt (a_n^2/a_{n+1/2})^2 lambda_n/2
     c.d1 = (e_p / e_m) * (e_p / e_m);                         // (e_{n+1/2}/e_{n-1/2})^2
     c.d2 = 2.0 * p.dt * a_0 * a_0 * e_p * e_p;                // 2 dt a_n^2 e_{n+1/2}^2
     c.d3 = p.dt / (p.dx * p.dx) * (e_p / e_0) * (e_p / e_0);  // dt/dx^2 (e_{n+1/2}/e_n)^2
@@ -117,19 +131,20 @@ StepCoef step_coefficients(const ahs_params& p, int64_t n)
     return c;
 }
 
-DiagCoef diag_coefficients(const ahs_params& p, int64_t n)
+DiagCoef diag_coefficients(const ahs_sim* sim, int64_t n)
 {
+    const ahs_params& p = sim->p;
     const double tau = tau_of(p, n);
     const double a = scale_factor(p, tau), a_h = scale_factor(p, tau - 0.5 * p.dt);
-    const double ea = e_of(p, a);
+    const double ea = e_of(sim, a, tau), e_h = e_of(sim, a_h, tau - 0.5 * p.dt);
     DiagCoef c;
     c.inv_dx2 = 1.0 / (p.dx * p.dx);
     c.gauge_norm = 1.0 / (2.0 * ea * ea * a * a * p.dx * p.dx);
     c.cB = p.c_B != 0.0 ? p.c_B : 1.0;
     c.cE = p.c_E != 0.0 ? p.c_E : 1.0;
-    c.pot_coef = 0.25 * a * a * lambda_of(p, a);
+    c.pot_coef = 0.25 * a * a * lambda_of(sim, a, tau);
     c.sigma2 = p.sigma * p.sigma;
-    c.gauss_rhs = 2.0 * p.dx * p.dx * p.e * p.e * std::pow(a_h, 2.0 * p.s);
+    c.gauss_rhs = 2.0 * p.dx * p.dx * e_h * e_h * a_h * a_h;   // = 2 dx^2 e0^2 a_h^(2s) for a constant s
     return c;
 }
 
@@ -146,7 +161,7 @@ int do_step(ahs_sim* s)
         f.eps[i] = slot<T>(s, EPS0 + i);
     }
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
-    const StepCoef c = step_coefficients(s->p, s->step);
+    const StepCoef c = step_coefficients(s, s->step);
     GhostPtrs<T> gh;
     const int ob = s->cur ^ 1;
     for (int i = 0; i < 5; ++i) { gh.lo[i] = (T*)s->ghost_lo[ob][i]; gh.hi[i] = (T*)s->ghost_hi[ob][i]; }
@@ -163,7 +178,7 @@ int do_diag(ahs_sim* s)
     f.phi_re = slot<T>(s, in); f.phi_im = slot<T>(s, in + 1);
     for (int i = 0; i < 3; ++i) { f.th[i] = slot<T>(s, in + 2 + i); f.eps[i] = slot<T>(s, EPS0 + i); }
     f.pi_re = slot<T>(s, PI_RE); f.pi_im = slot<T>(s, PI_IM);
-    const DiagCoef c = diag_coefficients(s->p, s->step);
+    const DiagCoef c = diag_coefficients(s, s->step);
     return s->kernel == AHS_KERNEL_MARCH
                ? launch_diag_march<T>(f, s->p.N, s->zr, c, s->partials, kMaxDiagPartials, s->result,
                                       // the doubt list: the shadow buffer, from its first OWN plane on (a slab's ghost planes there
@@ -530,7 +545,7 @@ int32_t ahs_coefficients(ahs_sim* s, int64_t n, double* out6)
 {
     AHS_ENTER(s);
     if (!out6 || n < 0) return fail(AHS_ERR_INVALID_ARG, "out6 is NULL or n < 0");
-    const StepCoef c = step_coefficients(s->p, n);
+    const StepCoef c = step_coefficients(s, n);
     out6[0] = c.c1; out6[1] = c.c2; out6[2] = c.c3; out6[3] = c.d1; out6[4] = c.d2; out6[5] = c.d3;
     return AHS_OK;
 }
@@ -559,6 +574,19 @@ int32_t ahs_set_option(ahs_sim* s, int32_t option, int32_t value)
         default:
             return fail(AHS_ERR_INVALID_ARG, "unknown option %d", option);
     }
+}
+
+int32_t ahs_set_s_schedule(ahs_sim* s, int32_t nknots, const double* tau, const double* s_values)
+{
+    AHS_ENTER(s);
+    if (nknots < 0 || nknots > 4096 || (nknots > 0 && (!tau || !s_values))) return fail(AHS_ERR_INVALID_ARG, "nknots must be 0..4096 with non-NULL arrays");
+    for (int32_t k = 0; k < nknots; ++k) {
+        if (!std::isfinite(tau[k]) || !std::isfinite(s_values[k])) return fail(AHS_ERR_INVALID_ARG, "knots must be finite");
+        if (k > 0 && !(tau[k] > tau[k - 1])) return fail(AHS_ERR_INVALID_ARG, "knot times must increase strictly");
+    }
+    s->sched_tau.assign(tau, tau + nknots);
+    s->sched_s.assign(s_values, s_values + nknots);
+    return AHS_OK;
 }
 
 int32_t ahs_destroy(ahs_sim* s)

@@ -736,3 +736,29 @@ def test_slab_group_from_uploaded_fields_and_options(ahs, oracle):
         ahs.Group(N=N, nslabs=3)                                                          # must divide N
     with pytest.raises(ahs.AhsError):
         ahs.Group(N=N, nslabs=2, devices=[0, 99])
+
+
+@pytest.mark.parametrize("prec,N,kernel", [("f64", 64, "auto"), ("f32", 128, "auto"), ("f64", 20, "generic")])
+def test_s_schedule_matches_oracle(ahs, oracle, prec, N, kernel):
+    """ahs_set_s_schedule: core growth (s = -1), a linear ramp, then the true equations (s = 1), 30 steps
+    across all three against the oracle; coefficients on the ramp to 1e-14; Gauss's law at roundoff on the device trajectory (it
+    only holds if every coupling takes s at its own time level); diagnostics on the oracle's snapshot."""
+    sched = ((1.0, -1.0), (2.0, -1.0), (3.0, 1.0))
+    with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.25, ic="none", kernel=kernel) as sim:
+        sim.set_s_schedule(sched)
+        p = oracle.Params(N=N, m=1.0, s=0.25, s_schedule=sched)
+        for n in (3, 14, 17, 25):
+            np.testing.assert_allclose(sim.coefficients(n), oracle.coeffs(p, n), rtol=1e-14)
+        ref = rounded(oracle.initial_condition(p, 9), prec)
+        sim.set_fields(ref, 0)
+        sim.step(30)
+        got = sim.get_fields()
+        oracle.step(p, ref, 0, 30)
+        assert_fields("s_schedule", got, ref, prec, oracle.FIELD_NAMES, tol=1e-12 if prec == "f64" else 2e-4, N=N, kernel=sim.kernel_kind, nsteps=30)
+        d = sim.diagnostics()
+        assert d["gauss_max"] <= (1e-12 if prec == "f64" else 2e-5) * max(1.0, d["gauss_rhs_rms"])
+        check_diag(oracle, p, sim, prec, ref, 30)
+        sim.set_s_schedule(())                                                       # back to the constant s
+        np.testing.assert_allclose(sim.coefficients(14), oracle.coeffs(oracle.Params(N=N, m=1.0, s=0.25), 14), rtol=1e-14)
+        with pytest.raises(ahs.AhsError):
+            sim.set_s_schedule(((2.0, 0.0), (1.0, 1.0)))
