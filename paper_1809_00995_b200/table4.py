@@ -25,9 +25,11 @@ PAPER = {  # PAPER.md Table 4 (L211-222), s = 0 rows: context, five-run averages
 }
 
 
-def run(N, m, seed, steps, every, fit_from, precision, c_B, c_E=0.0):
+def run(N, m, seed, steps, every, fit_from, precision, c_B, c_E=0.0, s_schedule=(), tau_ref=0.0):
     tau, series = [], {k: [] for k in ("xi", "xi_L", "v2", "v2_V", "v2_omega", "gauss_max")}
-    with ahs.Simulation(N=N, precision=precision, m=m, s=0.0, seed=seed, c_B=c_B, c_E=c_E, **COMMON) as sim:
+    with ahs.Simulation(N=N, precision=precision, m=m, s=0.0, seed=seed, c_B=c_B, c_E=c_E, tau_ref=tau_ref, **COMMON) as sim:
+        if s_schedule:
+            sim.set_s_schedule(s_schedule)
         for n in range(0, steps + 1, every):
             if n:
                 sim.step(every)
@@ -56,14 +58,21 @@ def main():
     ap.add_argument("--precision", default="f32")
     ap.add_argument("--c-b", type=float, default=0.0, help="factor on the plaquette sum of Eq. 2 in the weight (0 = 1, DESIGN.md R2; Eq. 2 prints 0.5)")
     ap.add_argument("--c-e", type=float, default=0.0, help="factor on the electric term of Eq. 2 in the weight (0 = 1; 0.04 = (dt/dx)^2, L44 read literally, DESIGN.md R21)")
+    ap.add_argument("--s-schedule", default="", help="'tau:s,tau:s,...' piecewise-linear s(tau) instead of s = 0 (ahs_set_s_schedule, DESIGN.md R23), "
+                    "e.g. core growth then the true equations: '1:-1,40:-1,48:1'")
+    ap.add_argument("--tau-ref", type=float, default=0.0, help="a = (tau/tau_ref)^m; 0 = tau0.  With s = 1 at the end use the end time (R3)")
+    ap.add_argument("--eras", default="radiation,matter")
     args = ap.parse_args()
+    sched = tuple(tuple(float(v) for v in kv.split(":")) for kv in args.s_schedule.split(",") if kv)
     N = args.lattice
     steps = int(round(N * COMMON["dx"] / 2 / COMMON["dt"]))          # half a light-crossing time of the box
     steps -= steps % args.every
     for era, m in (("radiation", 1.0), ("matter", 2.0)):
-        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b, args.c_e) for seed in range(1, args.seeds + 1)]
+        if era not in args.eras.split(","):
+            continue
+        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b, args.c_e, sched, args.tau_ref) for seed in range(1, args.seeds + 1)]
         line = {"era": era, "m": m, "s": 0.0, "lattice": N, "precision": args.precision, "seeds": args.seeds, "steps": steps, "c_B": args.c_b or 1.0,
-                "c_E": args.c_e or 1.0,
+                "c_E": args.c_e or 1.0, "s_schedule": sched or "s = 0", "tau_ref": args.tau_ref or COMMON["tau0"],
                 "fit_window_tau": [args.fit_from, COMMON["tau0"] + steps * COMMON["dt"]], "paper_table4": PAPER[era]}
         for k, name in (("xi_L_dot", "xi_L_dot"), ("xi_dot", "xi_W_dot"), ("v2_V", "v2_V"), ("v2", "v2_L"), ("v2_omega", "v2_omega")):
             v = np.array([r[k] for r in runs])
