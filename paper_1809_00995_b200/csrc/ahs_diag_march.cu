@@ -57,7 +57,13 @@ struct DiagCfg {
     static constexpr int STAGE_STRIDE = (int)(((G::STAGE_BYTES + 127u) & ~127u) / sizeof(T));   // tensor copies land 128-byte aligned
     // right-edge tiles under TMA: the wrapped forward halo column (x = 0 .. V-1) of a plane lands in a side buffer
     static constexpr int WRAP_STRIDE = (int)(((5 * G::ROWS * V * sizeof(T) + 127) & ~(size_t)127) / sizeof(T));
-    static constexpr int SLOT_STRIDE = STAGE_STRIDE + WRAP_STRIDE;   // a ring slot = a stage followed by its side buffer
+    // eps_1 (rows y0-1 .. y0+TY-1, no halo in x) of the same plane rides in the slot too: the divergence needs the row below, and a
+    // register-held global load of it was consumed right at the top of the plane by the compiler (profiles/r5_diag1024_f32_full.md)
+    static constexpr int E1_OFF = STAGE_STRIDE + WRAP_STRIDE;
+    static constexpr int E1_ELEMS = (TY + 1) * TX;
+    static constexpr uint32_t E1_BYTES = E1_ELEMS * sizeof(T);
+    static_assert(E1_BYTES % 128 == 0, "slots stay 128-byte aligned");
+    static constexpr int SLOT_STRIDE = E1_OFF + E1_ELEMS;   // a ring slot = a stage, its side buffer, the eps_1 rows
     static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * SLOT_STRIDE);
 };
 
@@ -152,7 +158,6 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     const P inv_dx2 = pk::splat((T)kd.inv_dx2), g_el = pk::splat((T)kd.gauge_norm), g_mag = pk::splat((T)(kd.gauge_norm * kd.inv_dx2));
     const P ncB = pk::splat(-(T)kd.cB), cE = pk::splat((T)kd.cE), third = pk::splat((T)(1.0 / 3.0));
     const P pot = pk::splat((T)kd.pot_coef), nsigma2 = pk::splat(-(T)kd.sigma2), grhs = pk::splat((T)kd.gauss_rhs);
-    const P half = pk::splat(T(0.5)), four = pk::splat(T(4));
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -169,8 +174,18 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     const bool right_edge = x0 + TX == N;
     const bool tma_tile = use_tma && (y0 + TY < N);
     const bool wrapR = tma_tile && right_edge;
+    const T* const e1_rows = f.eps[1] + (size_t)(zr.zbase + z0) * N * N + (size_t)x0;   // eps_1 of own plane z0 + p: + p N^2 + y N
     auto issue_plane = [&](int s, int p) {
-        mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + (wrapR ? (uint32_t)(5 * G::ROWS * V * sizeof(T)) : 0u));
+        const bool own = p < zlen;   // (plane zlen is only read as the +z neighbour: no momenta)
+        mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + (wrapR ? (uint32_t)(5 * G::ROWS * V * sizeof(T)) : 0u) + (own ? C::E1_BYTES : 0u));
+        if (own) {
+            const T* pl = e1_rows + (size_t)p * N * N;
+#pragma unroll
+            for (int r = 0; r <= TY; ++r) {
+                const int y = (y0 + r == 0) ? N - 1 : y0 + r - 1;
+                bulk_g2s(stages + s * SE + C::E1_OFF + r * TX, pl + (size_t)y * N, TX * sizeof(T), &full[s]);
+            }
+        }
         if (tma_tile) {
             tma_load_4d(stages + s * SE, &tmap, x0, y0, plane_of(p), 0, &full[s]);
             if (wrapR) tma_load_4d(stages + s * SE + C::STAGE_STRIDE, &wmap, 0, y0, plane_of(p), 0, &full[s]);
@@ -228,7 +243,6 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     // running offset; the row below (eps_1^{x-k_1}) and the site left of the tile (eps_0^{x-k_0}, lane 0) sit at fixed distances.
     const size_t plane_stride = (size_t)N * N;
     size_t g = ((size_t)(zr.zbase + z0) * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
-    const ptrdiff_t d_row_below = (y0 + w == 0) ? (ptrdiff_t)(N - 1) * N : -(ptrdiff_t)N;
     const ptrdiff_t d_site_left = (x0 + xi == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;
     // eps_2 of the plane below, carried in registers along the march
     VecT E2m = ldg_vec<T, V>(f.eps[2] + ((zr.periodic && z0 == 0) ? g + (size_t)(N - 1) * plane_stride : g - plane_stride));   // (slab: the ghost below)
@@ -245,8 +259,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
         const T* sn = ring_n ? sc + SE : stages;
 
         const VecT Pr = ldg_vec<T, V>(f.pi_re + g), Pi = ldg_vec<T, V>(f.pi_im + g);
-        const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E1 = ldg_vec<T, V>(f.eps[1] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
-        const VecT E1m = ldg_vec<T, V>(f.eps[1] + (g + d_row_below));
+        const VecT E0 = ldg_vec<T, V>(f.eps[0] + g), E2 = ldg_vec<T, V>(f.eps[2] + g);
         // eps_0 of the site left of the vector: its own scalar load (the line is in flight for the neighbouring lane's vector anyway);
         // a shuffle of E0 would tie the first use of the streamed loads to the top of the plane
         const T e0_left = __ldg(f.eps[0] + (g + d_site_left));
@@ -263,6 +276,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
         const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
         const T prx_e = sc[eo_re], pix_e = sc[eo_im];
         const T t1x_e = sc[eo_t1], t2x_e = sc[eo_t2];
+        const VecT E1 = lds_vec<T, V>(sc + C::E1_OFF + (w + 1) * TX + xi), E1m = lds_vec<T, V>(sc + C::E1_OFF + w * TX + xi);   // eps_1 here and one row below
 
         // ---- winding (Eq. 11), fast path: the link numbers this thread-plane needs.  n_0, n_1 of this plane were formed
         //      one iteration ago (as the +z links); n_1, n_2 are also taken at the site right of the vector (n_j^{x+k_0}).
@@ -336,12 +350,13 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
             const P K = pk::fma(pmr, pmr, pk::mul(pmi, pmi));
             const P dm = pk::fma(phr, phr, pk::fma(phi, phi, nsigma2));
             const P Vp = pk::mul(pot, pk::mul(dm, dm));
-            // 1 - cos Xi = 2 sin^2(Xi/2), without the cancellation of the literal form at small Xi
+            // sum over the ordered pairs (R12) of 1 - cos Xi = sum over the three plaquettes of |exp(i Xi) - 1|^2 = 4 sin^2(Xi/2): no
+            // cancellation at small Xi
             const P X01 = pk::sub(pk::add(th0, pk::next<T, V>(t1.v, h, t1x_e)), pk::add(pk::at<T, V>(t0y.v, h), th1));
             const P X02 = pk::sub(pk::add(th0, pk::next<T, V>(t2.v, h, t2x_e)), pk::add(pk::at<T, V>(t0z.v, h), th2));
             const P X12 = pk::sub(pk::add(th1, pk::at<T, V>(t2y.v, h)), pk::add(pk::at<T, V>(t1z.v, h), th2));
-            const P h01 = sin_pair(pk::mul(half, X01)), h02 = sin_pair(pk::mul(half, X02)), h12 = sin_pair(pk::mul(half, X12));
-            const P mag = pk::mul(four, pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12))));   // ordered pairs: 2 x [2 sin^2] per plaquette (R12)
+            const P h01 = chord_pair(X01), h02 = chord_pair(X02), h12 = chord_pair(X12);   // +- 2 sin(Xi/2)
+            const P mag = pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12)));
             const P e2 = pk::fma(ep0, ep0, pk::fma(ep1, ep1, pk::mul(ep2, ep2)));
             const P El = pk::mul(g_el, e2), Bm = pk::mul(g_mag, mag);   // electric / magnetic energy densities
             const P lag = pk::sub(pk::sub(pk::fma(cE, El, pk::fma(ncB, Bm, K)), Gd), Vp);

@@ -82,20 +82,28 @@ __device__ __forceinline__ void sincos_fast(float2 x, float2& s, float2& c)
     sincos_quadrant(t.y, sr.y, cr.y, s.y, c.y);
 }
 
-// t = x / pi + 1.5 * 2^23; sr = sin(r), r = x - k pi in [-pi/2, pi/2]; sin x = (-1)^k sr
-template <typename W>
+// t = x / pi + 1.5 * 2^23; sr = sin(r), r = x - k pi in [-pi/2, pi/2]; sin x = (-1)^k sr.
+// HALF = 1 evaluates the same polynomial at x/2 without ever forming x/2: every constant is scaled by an exact power of
+// two (HalfAngle), k = rint(x / 2 pi), r = x - 2 pi k in [-pi, pi] and sr = 2 sin(r/2) -- bit for bit twice what HALF = 0
+// returns for x/2; 2 sin(x/2) = (-1)^k sr.
+template <int HALF> struct HalfAngle {
+    static constexpr float inv = HALF ? 0.5f : 1.0f, pi = HALF ? 2.0f : 1.0f;
+    static constexpr float q1 = HALF ? 0.25f : 1.0f, q2 = q1 * q1, q3 = q2 * q1, q4 = q3 * q1, q5 = q4 * q1;   // c_i -> c_i / 4^i
+};
+template <typename W, int HALF = 0>
 __device__ __forceinline__ void sin_core(W x, W& t, W& sr)
 {
     using namespace lanes;
-    t = fma_(x, all<W>(0.31830987334251404f), all<W>(12582912.0f));
+    using H = HalfAngle<HALF>;
+    t = fma_(x, all<W>(0.31830987334251404f * H::inv), all<W>(12582912.0f));
     const W k = add_(t, all<W>(-12582912.0f));
-    W r = fma_(k, all<W>(-3.1415927410125732f), x);
-    r = fma_(k, all<W>(8.742277657347586e-08f), r);
+    W r = fma_(k, all<W>(-3.1415927410125732f * H::pi), x);
+    r = fma_(k, all<W>(8.742277657347586e-08f * H::pi), r);
     const W z = mul_(r, r);
-    W p = fma_(z, all<W>(-2.388586395341008e-08f), all<W>(2.752518867055187e-06f));
-    p = fma_(z, p, all<W>(-0.00019840864115394652f));
-    p = fma_(z, p, all<W>(0.008333330973982811f));
-    p = fma_(z, p, all<W>(-0.1666666716337204f));
+    W p = fma_(z, all<W>(-2.388586395341008e-08f * H::q5), all<W>(2.752518867055187e-06f * H::q4));
+    p = fma_(z, p, all<W>(-0.00019840864115394652f * H::q3));
+    p = fma_(z, p, all<W>(0.008333330973982811f * H::q2));
+    p = fma_(z, p, all<W>(-0.1666666716337204f * H::q1));
     sr = fma_(mul_(r, z), p, r);
 }
 __device__ __forceinline__ float sin_fast(float x)
@@ -110,6 +118,15 @@ __device__ __forceinline__ float2 sin_fast(float2 x)
     sin_core<float2>(x, t, sr);
     return make_float2(__int_as_float(__float_as_int(sr.x) ^ (__float_as_int(t.x) << 31)),
                        __int_as_float(__float_as_int(sr.y) ^ (__float_as_int(t.y) << 31)));
+}
+
+// the chord of the angle x on the unit circle up to its sign: +- |exp(i x) - 1| = +- 2 sin(x/2).  Only its square
+// 2 (1 - cos x) is used (the magnetic term of Eq. 2), so the sign fix-up of sin_fast and the halving of x are left out.
+__device__ __forceinline__ float2 chord_fast(float2 x)
+{
+    float2 t, sr;
+    sin_core<float2, 1>(x, t, sr);
+    return sr;
 }
 
 // arg(x + i y) / 2 pi, in turns, for the winding fast path (ahs_diag_march.cu): two values at once, branch-free.
@@ -245,5 +262,7 @@ __device__ __forceinline__ void sincos_pair(double2 x, double2& s, double2& c)
     sincos_fast(x.y, s.y, c.y);
 }
 __device__ __forceinline__ double2 sin_pair(double2 x) { return make_double2(sin_fast(x.x), sin_fast(x.y)); }
+__device__ __forceinline__ float2 chord_pair(float2 x) { return chord_fast(x); }
+__device__ __forceinline__ double2 chord_pair(double2 x) { return make_double2(2.0 * sin_fast(0.5 * x.x), 2.0 * sin_fast(0.5 * x.y)); }
 
 }  // namespace ahs
