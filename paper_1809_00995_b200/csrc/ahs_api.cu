@@ -353,10 +353,10 @@ ahs_sim* create_sim(const ahs_params* params, const SlabSpec* slab)
             : make_step_march_maps<double>(&s->step_maps[0], slot<double>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
               make_step_march_maps<double>(&s->step_maps[1], slot<double>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes);
         s->diag_map_ok = p.precision == AHS_F32
-            ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
-              make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes)
-            : make_diag_march_map<double>(&s->diag_map[0], slot<double>(s, PHI_RE0), p.N, s->zr.nz_alloc, s->array_bytes) &&
-              make_diag_march_map<double>(&s->diag_map[1], slot<double>(s, PHI_RE1), p.N, s->zr.nz_alloc, s->array_bytes);
+            ? make_diag_march_map<float>(&s->diag_map[0], slot<float>(s, PHI_RE0), slot<float>(s, EPS0 + 1), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_diag_march_map<float>(&s->diag_map[1], slot<float>(s, PHI_RE1), slot<float>(s, EPS0 + 1), p.N, s->zr.nz_alloc, s->array_bytes)
+            : make_diag_march_map<double>(&s->diag_map[0], slot<double>(s, PHI_RE0), slot<double>(s, EPS0 + 1), p.N, s->zr.nz_alloc, s->array_bytes) &&
+              make_diag_march_map<double>(&s->diag_map[1], slot<double>(s, PHI_RE1), slot<double>(s, EPS0 + 1), p.N, s->zr.nz_alloc, s->array_bytes);
     }
 
     // initial condition (L72): everything zero, then phi from Philox

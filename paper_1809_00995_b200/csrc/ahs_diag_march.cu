@@ -129,7 +129,7 @@ template <typename T>
 __global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, DiagCfg<T>::MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
                   unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
-                  const __grid_constant__ CUtensorMap wmap, int use_tma)
+                  const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap emap, int use_tma)
 {
     using C = DiagCfg<T>;
     using G = typename C::G;
@@ -174,13 +174,16 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     const bool right_edge = x0 + TX == N;
     const bool tma_tile = use_tma && (y0 + TY < N);
     const bool wrapR = tma_tile && right_edge;
-    const T* const e1_rows = f.eps[1] + (size_t)(zr.zbase + z0) * N * N + (size_t)x0;   // eps_1 of own plane z0 + p: + p N^2 + y N
+    // eps_1 of own plane z0 + p, rows y0-1 .. y0+TY-1: one tensor copy, except on the bottom tile row (the row below wraps)
+    const bool e1_tma = use_tma && y0 > 0;
     auto issue_plane = [&](int s, int p) {
         const bool own = p < zlen;   // (plane zlen is only read as the +z neighbour: no momenta)
         mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + (wrapR ? (uint32_t)(5 * G::ROWS * V * sizeof(T)) : 0u) + (own ? C::E1_BYTES : 0u));
-        if (own) {
-            const T* pl = e1_rows + (size_t)p * N * N;
-#pragma unroll
+        if (own && e1_tma) {
+            tma_load_4d(stages + s * SE + C::E1_OFF, &emap, x0, y0 - 1, zr.zbase + z0 + p, 0, &full[s]);
+        } else if (own) {
+            const T* pl = f.eps[1] + (size_t)(zr.zbase + z0 + p) * N * N + (size_t)x0;
+#pragma unroll 1
             for (int r = 0; r <= TY; ++r) {
                 const int y = (y0 + r == 0) ? N - 1 : y0 + r - 1;
                 bulk_g2s(stages + s * SE + C::E1_OFF + r * TX, pl + (size_t)y * N, TX * sizeof(T), &full[s]);
@@ -458,7 +461,7 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagC
     memset(&none, 0, sizeof(none));
     const bool use_tma = tmap && opt.staging == AHS_STAGING_TENSOR;
     const DiagMaps& mp = use_tma ? *tmap : none;
-    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zr, nchunks, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, use_tma ? 1 : 0);
+    kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, N, zr, nchunks, c, partials, (unsigned*)list, count, mp.tile, mp.wrap, mp.eps1, use_tma ? 1 : 0);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
     diag_resolve_kernel<T><<<148 * 8, 128, 0, st>>>(f, N, zr.periodic, (const unsigned*)list, count, extra);
     if (cudaGetLastError() != cudaSuccess) return AHS_ERR_CUDA;
@@ -466,17 +469,18 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagC
     return r < 0 ? r : 3;
 }
 
-// the tensor map of one (phi, theta) buffer for the tile shape above: box (TX + V, TY + 1, 1, 5)
+// the tensor maps of one (phi, theta) buffer for the tile shape above: box (TX + V, TY + 1, 1, 5), and of eps_1: box (TX, TY + 1, 1, 1)
 template <typename T>
-bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes)
+bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, const void* eps1_base, int N, int nz_alloc, size_t array_bytes)
 {
     using G = typename DiagCfg<T>::G;
     if (!march_supported<T>(N)) return false;
     return make_tile_map<T>(&out->tile, phi_re_base, N, nz_alloc, array_bytes, 5, G::PITCH, G::ROWS, 5) &&
-           make_tile_map<T>(&out->wrap, phi_re_base, N, nz_alloc, array_bytes, 5, G::V, G::ROWS, 5);
+           make_tile_map<T>(&out->wrap, phi_re_base, N, nz_alloc, array_bytes, 5, G::V, G::ROWS, 5) &&
+           make_tile_map<T>(&out->eps1, eps1_base, N, nz_alloc, array_bytes, 1, G::TX, G::TY + 1, 1);
 }
-template bool make_diag_march_map<float>(DiagMaps*, const void*, int, int, size_t);
-template bool make_diag_march_map<double>(DiagMaps*, const void*, int, int, size_t);
+template bool make_diag_march_map<float>(DiagMaps*, const void*, const void*, int, int, size_t);
+template bool make_diag_march_map<double>(DiagMaps*, const void*, const void*, int, int, size_t);
 
 template int launch_diag_march<float>(const DiagPtrs<float>&, int, const ZRange&, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);
 template int launch_diag_march<double>(const DiagPtrs<double>&, int, const ZRange&, const DiagCoef&, DiagPartial*, int, DiagPartial*, void*, size_t, const DiagMaps*, const MarchOptions&, cudaStream_t);

@@ -120,15 +120,16 @@ template <typename T> bool make_step_march_maps(StepMaps* out, const void* phi_r
 template <typename T> bool march_supported(int N);
 template <typename T> int launch_diag_generic(const DiagPtrs<T>& f, int N, const DiagCoef& c, DiagPartial* partials,
                                               int max_partials, DiagPartial* result, cudaStream_t st);
-// TMA descriptors of the diagnostics march: the five-array forward-halo tile and the V-wide wrapped column of right-edge tiles
-struct DiagMaps { CUtensorMap tile, wrap; };
+// TMA descriptors of the diagnostics march: the five-array forward-halo tile, the V-wide wrapped column of right-edge tiles,
+// and the rows y0-1 .. y0+TY-1 of eps_1
+struct DiagMaps { CUtensorMap tile, wrap, eps1; };
 // `list`: DEVICE scratch of >= 4 N^3 / (16 / sizeof(T)) bytes for the winding doubt list (the dead phi', theta' shadow buffer)
 template <typename T> int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagCoef& c, DiagPartial* partials,
                                             int max_partials, DiagPartial* result, void* list, size_t list_bytes,
                                             const DiagMaps* tmap /* HOST, may be NULL: row copies only */, const MarchOptions& opt,
                                             cudaStream_t st);
-// tensor map (TMA descriptor) of the five level-n arrays of one (phi, theta) buffer for the diagnostics march; false if unavailable
-template <typename T> bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, int N, int nz_alloc, size_t array_bytes);
+// tensor maps (TMA descriptors) of the five level-n arrays of one (phi, theta) buffer and of eps_1 for the diagnostics march; false if unavailable
+template <typename T> bool make_diag_march_map(DiagMaps* out, const void* phi_re_base, const void* eps1_base, int N, int nz_alloc, size_t array_bytes);
 int launch_diag_finish(const DiagPartial* partials, int n, DiagPartial* result, cudaStream_t st);
 template <typename T> int launch_convert_from_double(const double* src, T* dst, int64_t n, cudaStream_t st);
 template <typename T> int launch_convert_to_double(const T* src, double* dst, int64_t n, cudaStream_t st);
