@@ -58,8 +58,9 @@ enum { AHS_OK = 0, AHS_ERR_INVALID_ARG = -1, AHS_ERR_OOM = -2, AHS_ERR_CUDA = -3
 enum { AHS_F32 = 0, AHS_F64 = 1 };                                   /* storage AND arithmetic type of the step */
 enum { AHS_IC_RANDOM_PHASE = 0, AHS_IC_GAUSSIAN = 1, AHS_IC_NONE = 2 /* all fields zero; set them with ahs_set_fields */ };
 enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
-enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2 };   /* ahs_set_option */
+enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2, AHS_OPT_DIAG_TRIG = 3 };   /* ahs_set_option */
 enum { AHS_STAGING_TENSOR = 0, AHS_STAGING_ROWS = 1 };
+enum { AHS_TRIG_HARDWARE = 0, AHS_TRIG_POLYNOMIAL = 1 };
 
 /*
  * Parameters of a simulation (L36: lambda, e, sigma; L51: dx, dt; L68-70: s; L224: a ~ eta^m; L72: IC).
@@ -191,13 +192,20 @@ AHS_API int32_t ahs_get_state(ahs_sim* sim, int64_t* step, double* tau, int64_t*
 /* Which implementation the handle uses: AHS_KERNEL_GENERIC or AHS_KERNEL_MARCH. */
 AHS_API int32_t ahs_kernel_kind(ahs_sim* sim);
 
-/* Tuning of the z-marching kernels (no effect on the one-thread-per-site kernels, none on any result beyond rounding order
- * of the fp64 reduction, which follows the launch shape).  Takes effect at the next launch.
+/* Tuning of the z-marching kernels (no effect on the one-thread-per-site kernels; the first three have none on any result beyond
+ * rounding order of the fp64 reduction, which follows the launch shape).  Takes effect at the next launch.
  *   AHS_OPT_STAGING      AHS_STAGING_TENSOR (default): halo'd tiles of the level-n fields (Eq. 4-5's phi, theta) are staged in
  *                        shared memory by tensor-map TMA copies wherever a tile does not straddle the periodic boundary in y;
  *                        AHS_STAGING_ROWS: by one bulk copy per tile row everywhere (the path tiles on that boundary always take).
  *   AHS_OPT_STEP_CHUNKS  number of z-chunks each (x, y) tile of the step march is cut into, 1..N (0 = the library's choice);
  *   AHS_OPT_DIAG_CHUNKS  the same for the diagnostics march.  Chunks need not divide N.
+ *   AHS_OPT_DIAG_TRIG    how the diagnostics march of an fp32 lattice evaluates the sines and cosines inside the sums of Eqs. 2, 9, 10
+ *                        and 12 (link phases of the gradient term, plaquette angles of the magnetic term):
+ *                        AHS_TRIG_HARDWARE (default): the GPU's special-function unit, absolute error <= 4e-7 per value; the sums
+ *                        then agree with an fp64 evaluation to ~1.5e-7 of their absolute sums (one fp32 rounding; measured,
+ *                        DESIGN.md section 8) instead of ~1e-8;
+ *                        AHS_TRIG_POLYNOMIAL: the 1-2 ulp routines the step kernel uses (the call takes ~17 % longer).
+ *                        The winding (Eq. 11) and the Gauss residual do not depend on it; fp64 lattices always take the polynomials.
  * Returns AHS_ERR_INVALID_ARG for an unknown option or a value out of range. */
 AHS_API int32_t ahs_set_option(ahs_sim* sim, int32_t option, int32_t value);
 

@@ -314,7 +314,7 @@ ahs_sim* create_sim(const ahs_params* params, const SlabSpec* slab)
     s->cur = 0; s->step = 0; s->launches = 0; s->diag_step = -1; s->device = dev;
     s->kernel = (p.kernel == AHS_KERNEL_AUTO) ? (march_ok ? AHS_KERNEL_MARCH : AHS_KERNEL_GENERIC) : p.kernel;
     s->result_host = nullptr;
-    s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0 };
+    s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0, AHS_TRIG_HARDWARE };
 
     const size_t need = (size_t)NUM_SLOTS * s->array_bytes + scratch_bytes();
     if (p.device_buffer) {
@@ -570,6 +570,10 @@ int32_t ahs_set_option(ahs_sim* s, int32_t option, int32_t value)
         case AHS_OPT_DIAG_CHUNKS:
             if (value > s->p.N) return fail(AHS_ERR_INVALID_ARG, "at most N = %d z-chunks per tile", s->p.N);
             (option == AHS_OPT_STEP_CHUNKS ? s->opt.step_chunks : s->opt.diag_chunks) = value;
+            return AHS_OK;
+        case AHS_OPT_DIAG_TRIG:
+            if (value != AHS_TRIG_HARDWARE && value != AHS_TRIG_POLYNOMIAL) return fail(AHS_ERR_INVALID_ARG, "AHS_OPT_DIAG_TRIG takes AHS_TRIG_HARDWARE or AHS_TRIG_POLYNOMIAL");
+            s->opt.diag_trig = value;
             return AHS_OK;
         default:
             return fail(AHS_ERR_INVALID_ARG, "unknown option %d", option);

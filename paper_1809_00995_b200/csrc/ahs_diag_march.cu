@@ -82,6 +82,30 @@ __device__ __forceinline__ float2 link_numbers(float2 as, float2 at, float2 th, 
     tmax = fmaxf(tmax, fmaxf(fabsf(t.x), fabsf(t.y)));
     return n;
 }
+// The trigonometry of the <v^2> sums (link phases of the gradient term, plaquette chords of the magnetic term), by TRIG:
+//   AHS_TRIG_POLYNOMIAL  the Cody-Waite + polynomial routines of ahs_trig.cuh (<= 1-2 ulp), as in the step kernel;
+//   AHS_TRIG_HARDWARE    (fp32 lattices only) the special-function unit's sine / cosine, |error| <= 2^-21.4 / 2^-21.2 for |x| <= pi
+//                        and about |x| 2^-23 beyond (the unit takes x / 2 pi rounded to fp32): a quarter of the kernel's FMA-pipe
+//                        time moves to the otherwise idle XU pipe.  The winding never uses it.
+// sum over the ordered pairs (R12) of 1 - cos Xi = sum over the three plaquettes of |exp(i Xi) - 1|^2 = 4 sin^2(Xi/2): no
+// cancellation at small Xi
+template <int TRIG> struct SumsTrig {
+    template <typename P> __device__ __forceinline__ static void link_phase(P th, P& s, P& c) { sincos_pair(th, s, c); }
+    template <typename P> __device__ __forceinline__ static P plaquettes(P X01, P X02, P X12)
+    {
+        const P h01 = chord_pair(X01), h02 = chord_pair(X02), h12 = chord_pair(X12);   // +- 2 sin(Xi/2)
+        return pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12)));
+    }
+};
+template <> struct SumsTrig<AHS_TRIG_HARDWARE> {
+    __device__ __forceinline__ static void link_phase(float2 th, float2& s, float2& c) { sincos_hw(th, s, c); }
+    __device__ __forceinline__ static float2 plaquettes(float2 X01, float2 X02, float2 X12)
+    {
+        const float2 half = pk::splat(0.5f);
+        const float2 h01 = sin_hw(pk::mul(half, X01)), h02 = sin_hw(pk::mul(half, X02)), h12 = sin_hw(pk::mul(half, X12));
+        return pk::mul(pk::splat(4.0f), pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12))));
+    }
+};
 __device__ __forceinline__ float2 to_float2(float2 v) { return v; }
 __device__ __forceinline__ float2 to_float2(double2 v) { return make_float2((float)v.x, (float)v.y); }
 
@@ -125,7 +149,7 @@ __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N,
     }
 }
 
-template <typename T>
+template <typename T, int TRIG>
 __global__ void __launch_bounds__(DiagCfg<T>::NTHREADS, DiagCfg<T>::MINB)
 diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, DiagPartial* __restrict__ partials, unsigned* __restrict__ doubt_list,
                   unsigned long long* __restrict__ doubt_count, const __grid_constant__ CUtensorMap tmap,
@@ -336,9 +360,9 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
             const P th0 = pk::at<T, V>(t0.v, h), th1 = pk::at<T, V>(t1.v, h), th2 = pk::at<T, V>(t2.v, h);
             const P ep0 = pk::at<T, V>(E0.v, h), ep1 = pk::at<T, V>(E1.v, h), ep2 = pk::at<T, V>(E2.v, h);
             P s0, c0, s1, c1, s2, c2;
-            sincos_pair(th0, s0, c0);
-            sincos_pair(th1, s1, c1);
-            sincos_pair(th2, s2, c2);
+            SumsTrig<TRIG>::link_phase(th0, s0, c0);
+            SumsTrig<TRIG>::link_phase(th1, s1, c1);
+            SumsTrig<TRIG>::link_phase(th2, s2, c2);
             // forward hops U_j phi^{x+k_j} - phi^x, U = cos - i sin:  (c re + s im, c im - s re)
             const P nxr = pk::next<T, V>(pr.v, h, prx_e), nxi = pk::next<T, V>(pi.v, h, pix_e);
             const P d0r = pk::sub(pk::fma(c0, nxr, pk::mul(s0, nxi)), phr), d0i = pk::sub(pk::fma(pk::neg(s0), nxr, pk::mul(c0, nxi)), phi);
@@ -353,13 +377,10 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
             const P K = pk::fma(pmr, pmr, pk::mul(pmi, pmi));
             const P dm = pk::fma(phr, phr, pk::fma(phi, phi, nsigma2));
             const P Vp = pk::mul(pot, pk::mul(dm, dm));
-            // sum over the ordered pairs (R12) of 1 - cos Xi = sum over the three plaquettes of |exp(i Xi) - 1|^2 = 4 sin^2(Xi/2): no
-            // cancellation at small Xi
             const P X01 = pk::sub(pk::add(th0, pk::next<T, V>(t1.v, h, t1x_e)), pk::add(pk::at<T, V>(t0y.v, h), th1));
             const P X02 = pk::sub(pk::add(th0, pk::next<T, V>(t2.v, h, t2x_e)), pk::add(pk::at<T, V>(t0z.v, h), th2));
             const P X12 = pk::sub(pk::add(th1, pk::at<T, V>(t2y.v, h)), pk::add(pk::at<T, V>(t1z.v, h), th2));
-            const P h01 = chord_pair(X01), h02 = chord_pair(X02), h12 = chord_pair(X12);   // +- 2 sin(Xi/2)
-            const P mag = pk::fma(h01, h01, pk::fma(h02, h02, pk::mul(h12, h12)));
+            const P mag = SumsTrig<TRIG>::plaquettes(X01, X02, X12);
             const P e2 = pk::fma(ep0, ep0, pk::fma(ep1, ep1, pk::mul(ep2, ep2)));
             const P El = pk::mul(g_el, e2), Bm = pk::mul(g_mag, mag);   // electric / magnetic energy densities
             const P lag = pk::sub(pk::sub(pk::fma(cE, El, pk::fma(ncB, Bm, K)), Gd), Vp);
@@ -445,9 +466,11 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagC
 {
     using C = DiagCfg<T>;
     if (!march_supported<T>(N) || zr.nz < 1) return AHS_ERR_INVALID_ARG;
-    auto kern = diag_march_kernel<T>;
-    static SmemAttribute attr;   // per device
-    if (!attr.ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
+    // fp64 lattices always take the polynomials (the hardware unit is an fp32 one)
+    const bool hw = sizeof(T) == 4 && opt.diag_trig == AHS_TRIG_HARDWARE;
+    auto kern = hw ? diag_march_kernel<T, sizeof(T) == 4 ? AHS_TRIG_HARDWARE : AHS_TRIG_POLYNOMIAL> : diag_march_kernel<T, AHS_TRIG_POLYNOMIAL>;
+    static SmemAttribute attr[2];   // per device and instantiation
+    if (!attr[hw].ensure(kern, C::SMEM)) return AHS_ERR_CUDA;
     const long tiles = (long)(N / C::TX) * (N / C::TY);
     int nchunks = pick_chunks<T>(N, zr.nz, tiles, max_partials);
     if (opt.diag_chunks > 0 && opt.diag_chunks <= zr.nz && tiles * opt.diag_chunks + 2 <= max_partials) nchunks = opt.diag_chunks;

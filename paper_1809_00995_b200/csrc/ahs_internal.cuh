@@ -90,6 +90,7 @@ struct MarchOptions {
     int staging;       // AHS_STAGING_TENSOR (tensor-map TMA where a tile allows it) or AHS_STAGING_ROWS (row copies only)
     int step_chunks;   // z-chunks per tile of the step march
     int diag_chunks;   // z-chunks per tile of the diagnostics march
+    int diag_trig;     // AHS_TRIG_HARDWARE or AHS_TRIG_POLYNOMIAL: the sines and cosines of the <v^2> sums (fp32 lattices)
 };
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is per device: set it once on every device a kernel is launched on

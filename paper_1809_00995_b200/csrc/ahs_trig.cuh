@@ -129,6 +129,24 @@ __device__ __forceinline__ float2 chord_fast(float2 x)
     return sr;
 }
 
+// ---- the special-function unit's sine / cosine (MUFU.SIN / MUFU.COS behind one multiplication by 1/2pi), two lanes ------------
+// Absolute error <= 2^-21.4 (sine) / 2^-21.2 (cosine) for |x| <= pi; beyond, the unit sees x / 2 pi rounded to fp32, i.e. a
+// phase error of about |x| 2^-23 -- the rounding an fp32 angle of that size carries anyway.  NaN and Inf give NaN.  Used by the
+// diagnostics' <v^2> sums only (AHS_TRIG_HARDWARE), never by the step or the winding.
+__device__ __forceinline__ float2 sin_hw(float2 x)
+{
+    float2 r;
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r.x) : "f"(x.x));
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r.y) : "f"(x.y));
+    return r;
+}
+__device__ __forceinline__ void sincos_hw(float2 x, float2& s, float2& c)
+{
+    s = sin_hw(x);
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(c.x) : "f"(x.x));
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(c.y) : "f"(x.y));
+}
+
 // arg(x + i y) / 2 pi, in turns, for the winding fast path (ahs_diag_march.cu): two values at once, branch-free.
 // q = min/max in [0, 1] (MUFU.RCP and a multiply), odd polynomial of degree 15 in q fitted to atan(q) / 2 pi, then the
 // octant fix-ups, whose constants 1/4 and 1/2 are exact in turns.  Absolute error <= 5e-8 turns in the fp32 emulation of

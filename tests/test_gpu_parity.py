@@ -108,6 +108,12 @@ def check_diag(O, p, sim, prec, snap, n):
     # equation-of-state estimator (Eq. 12): the two Lagrangian-weighted sums, relative to their absolute sums
     K6, G6, L6, V6, El, Bm = O.site_fields6(p, snap, n)
     rho, prs = K6 + G6 + V6 + El + Bm, K6 - G6 / 3 - V6 + (El + Bm) / 3
+    # observed errors of the sums, in units of the absolute sums they are compared against (bar: `rel`)
+    ratio = lambda err, scale: float("%.3g" % (abs(err) / scale)) if scale > 0 else 0.0
+    record("check_diag", prec=prec, N=int(snap.shape[-1]), kernel=sim.kernel_kind, bar=rel,
+           v2_num=ratio(d["v2_num"] - r["v2_num"], np.abs(K * Lg).sum()), v2_den=ratio(d["v2_den"] - r["v2_den"], np.abs(G * Lg).sum()),
+           lagrangian=ratio(d["mean_lagrangian"] - r["mean_lagrangian"], np.abs(Lg).mean()),
+           eos_num=ratio(d["eos_num"] - r["eos_num"], np.abs(prs * L6).sum()), eos_den=ratio(d["eos_den"] - r["eos_den"], np.abs(rho * L6).sum()))
     assert abs(d["eos_num"] - r["eos_num"]) <= rel * np.abs(prs * L6).sum() + 1e-300
     assert abs(d["eos_den"] - r["eos_den"]) <= rel * np.abs(rho * L6).sum() + 1e-300
     if abs(r["eos_den"]) > 0.05 * np.abs(rho * L6).sum():
@@ -598,10 +604,38 @@ def test_options_change_the_launch_shape_not_the_result(ahs, prec, N):
                 assert d[key] == pytest.approx(dref[key], rel=1e-11, abs=1e-11 * abs(dref["v2_den"])), (opts, key)
             assert d["gauss_max"] == dref["gauss_max"], opts
     with ahs.Simulation(N=N, precision=prec) as sim:
-        for bad in ((99, 0), (ahs.AHS_OPT_STAGING, 2), (ahs.AHS_OPT_STEP_CHUNKS, N + 1), (ahs.AHS_OPT_DIAG_CHUNKS, -1)):
+        for bad in ((99, 0), (ahs.AHS_OPT_STAGING, 2), (ahs.AHS_OPT_STEP_CHUNKS, N + 1), (ahs.AHS_OPT_DIAG_CHUNKS, -1), (ahs.AHS_OPT_DIAG_TRIG, 2)):
             with pytest.raises(ahs.AhsError) as e:
                 sim.set_option(*bad)
             assert e.value.code == ahs.AHS_ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("N", [128, 256])
+def test_diag_trig_option_both_settings_against_the_oracle(ahs, oracle, N):
+    """AHS_OPT_DIAG_TRIG: the sums of Eqs. 2, 9, 10, 12 on an fp32 lattice with the special-function unit's sine / cosine (default)
+    and with the polynomial routines, each against the oracle on the same snapshot with the SAME bar (check_diag; 2e-5 of the
+    absolute sums).  Observed (recorded): ~1.5e-7 and ~1e-8.  The winding count and the Gauss residual do not depend on the
+    setting; an fp64 lattice ignores it bit for bit."""
+    O = oracle
+    with ahs.Simulation(N=N, precision="f32", seed=77) as sim:
+        p = oracle_params(O, sim)
+        snap = O.initial_condition(p, seed=77)
+        O.step(p, snap, 0, 12)
+        got = {}
+        for name, v in (("hardware", ahs.AHS_TRIG_HARDWARE), ("polynomial", ahs.AHS_TRIG_POLYNOMIAL)):
+            sim.set_option(ahs.AHS_OPT_DIAG_TRIG, v)
+            got[name], r = check_diag(O, p, sim, "f32", snap, 12)
+        h, q = got["hardware"], got["polynomial"]
+        assert (h["n_pierced"], h["sum_abs_w"], h["gauss_max"]) == (q["n_pierced"], q["sum_abs_w"], q["gauss_max"])
+        assert h["v2_num"] != q["v2_num"]                       # (the two settings really are two code paths)
+        for key in ("v2_num", "v2_den", "eos_num", "eos_den"):
+            assert abs(q[key] - r[key]) <= 2e-7 * abs(r["v2_den"]), key     # the polynomials stay at the 1e-8 level
+    with ahs.Simulation(N=128, precision="f64", seed=77) as sim:
+        sim.step(3)
+        a = sim.diagnostics()
+        sim.set_option(ahs.AHS_OPT_DIAG_TRIG, ahs.AHS_TRIG_POLYNOMIAL)
+        b = sim.diagnostics()
+        assert all(b[k] == a[k] or (a[k] != a[k] and b[k] != b[k]) for k in a)      # (xi_L is NaN while the mean Lagrangian is > 0)
 
 
 def test_two_handles_on_two_streams_interleaved(ahs):
