@@ -27,6 +27,30 @@ def test_sin_fast_fp32_constants():
     assert np.abs(s - np.sin(x.astype(np.float64))).max() < 1.8e-7            # <= 1.9 ulp at |sin| ~ 1 (ahs_trig.cuh)
 
 
+def test_chord_is_the_sine_polynomial_with_power_of_two_scaled_constants():
+    """chord_fast (the magnetic term of the diagnostics) = sin_core<W, 1>: the constants of sin_core scaled by the exact powers of
+    two of HalfAngle<1> (read from the header).  Emulated, it must be twice sin_core at x/2 bit for bit up to its sign, hence
+    |chord| = 2 |sin(x/2)| within twice the sine's bound."""
+    import re
+    src = open(os.path.join(fit_trig.CSRC, "ahs_trig.cuh")).read()
+    m = re.search(r"inv = HALF \? ([\d.]+)f : 1\.0f, pi = HALF \? ([\d.]+)f : 1\.0f;\s*\n\s*static constexpr float q1 = HALF \? ([\d.]+)f : 1\.0f", src)
+    inv, pi2, q1 = (float(g) for g in m.groups())
+    assert (inv, pi2, q1) == (0.5, 2.0, 0.25)
+    k = fit_trig.header_constants("void sin_core(W x")
+    scaled = list(k)
+    scaled[0] = k[0] * inv                                   # 1 / 2 pi
+    scaled[3], scaled[4] = k[3] * pi2, k[4] * pi2            # the two-term split of 2 pi
+    for j, power in zip((5, 6, 7, 8, 9), (5, 4, 3, 2, 1)):   # c_i / 4^i, highest degree first
+        scaled[j] = k[j] * q1 ** power
+    assert all(np.float32(v) == v or abs(np.float32(v) - v) <= abs(v) * 2.0 ** -24 for v in scaled)
+    rng = np.random.default_rng(8)
+    x = np.concatenate([rng.uniform(-20, 20, 400_000), rng.uniform(-300, 300, 100_000), [0.0, np.pi, -np.pi, 1e-8]]).astype(np.float32)
+    chord = fit_trig.emu_sin(x, [np.float32(v) for v in scaled])
+    half = fit_trig.emu_sin((x * np.float32(0.5)).astype(np.float32), k)
+    assert np.array_equal(np.abs(chord), np.abs(2.0 * half).astype(np.float32))
+    assert np.abs(np.abs(chord) - 2.0 * np.abs(np.sin(0.5 * x.astype(np.float64)))).max() < 3.6e-7
+
+
 def test_atan2_turns_constants_stay_inside_the_winding_error_budget():
     rng = np.random.default_rng(4)
     ph = rng.uniform(-np.pi, np.pi, 500_000)
