@@ -25,11 +25,13 @@ PAPER = {  # PAPER.md Table 4 (L211-222), s = 0 rows: context, five-run averages
 }
 
 
-def run(N, m, seed, steps, every, fit_from, precision, c_B, c_E=0.0, s_schedule=(), tau_ref=0.0):
+def run(N, m, seed, steps, every, fit_from, precision, c_B, c_E=0.0, s_schedule=(), tau_ref=0.0, diag_trig=None):
     tau, series = [], {k: [] for k in ("xi", "xi_L", "v2", "v2_V", "v2_omega", "gauss_max")}
     with ahs.Simulation(N=N, precision=precision, m=m, s=0.0, seed=seed, c_B=c_B, c_E=c_E, tau_ref=tau_ref, **COMMON) as sim:
         if s_schedule:
             sim.set_s_schedule(s_schedule)
+        if diag_trig is not None:
+            sim.set_option(ahs.AHS_OPT_DIAG_TRIG, diag_trig)
         for n in range(0, steps + 1, every):
             if n:
                 sim.step(every)
@@ -62,6 +64,8 @@ def main():
                     "e.g. core growth then the true equations: '1:-1,40:-1,48:1'")
     ap.add_argument("--tau-ref", type=float, default=0.0, help="a = (tau/tau_ref)^m; 0 = tau0.  With s = 1 at the end use the end time (R3)")
     ap.add_argument("--eras", default="radiation,matter")
+    ap.add_argument("--diag-trig", default="hardware", choices=["hardware", "polynomial"],
+                    help="AHS_OPT_DIAG_TRIG: where an fp32 lattice's diagnostics evaluate the sines / cosines of their sums (DESIGN.md 7.2)")
     args = ap.parse_args()
     sched = tuple(tuple(float(v) for v in kv.split(":")) for kv in args.s_schedule.split(",") if kv)
     N = args.lattice
@@ -70,8 +74,9 @@ def main():
     for era, m in (("radiation", 1.0), ("matter", 2.0)):
         if era not in args.eras.split(","):
             continue
-        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b, args.c_e, sched, args.tau_ref) for seed in range(1, args.seeds + 1)]
-        line = {"era": era, "m": m, "s": 0.0, "lattice": N, "precision": args.precision, "seeds": args.seeds, "steps": steps, "c_B": args.c_b or 1.0,
+        trig = ahs.AHS_TRIG_HARDWARE if args.diag_trig == "hardware" else ahs.AHS_TRIG_POLYNOMIAL
+        runs = [run(N, m, seed, steps, args.every, args.fit_from, args.precision, args.c_b, args.c_e, sched, args.tau_ref, trig) for seed in range(1, args.seeds + 1)]
+        line = {"era": era, "m": m, "s": 0.0, "lattice": N, "precision": args.precision, "seeds": args.seeds, "steps": steps, "diag_trig": args.diag_trig, "c_B": args.c_b or 1.0,
                 "c_E": args.c_e or 1.0, "s_schedule": sched or "s = 0", "tau_ref": args.tau_ref or COMMON["tau0"],
                 "fit_window_tau": [args.fit_from, COMMON["tau0"] + steps * COMMON["dt"]], "paper_table4": PAPER[era]}
         for k, name in (("xi_L_dot", "xi_L_dot"), ("xi_dot", "xi_W_dot"), ("v2_V", "v2_V"), ("v2", "v2_L"), ("v2_omega", "v2_omega")):
