@@ -68,6 +68,7 @@ def parse_args():
                     "process; 0 = one handle")
     ap.add_argument("--slab-devices", default="", help="comma-separated CUDA ordinals, one per slab (default: all on this rank's GPU)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short runs of BASELINE configs 2, 3 and 5 that the default command adds")
     ap.add_argument("--cpu-lattice", type=int, default=128, help="lattice of the oracle's bounded sample")
     ap.add_argument("--cpu-leapfrog", type=int, default=10)
     return ap.parse_args()
@@ -322,6 +323,9 @@ def run_ours(args):
     if e2e is not None:
         line["e2e"] = e2e
     sim.destroy()
+    default_workload = (N, args.precision, L, args.m, args.s, args.kernel, args.slabs) == (1024, "f32", 50, 1.0, 0.0, "auto", 0)
+    if rank == 0 and world == 1 and default_workload and not args.no_other_configs:
+        line["other_configs"] = other_configs(torch)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # the oracle on all host cores (a sample twice as wide: ~10 s) and, beside it, on one core
         r = oracle_sample(args, threads=0, lattice=2 * args.cpu_lattice)
@@ -332,6 +336,45 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def other_configs(torch):
+    """BASELINE.json's remaining marching configurations (2: 256^3 fp32, 3: 512^3 fp32 matter s = 1 Gaussian IC, 5: 512^3 fp64), each run whole
+    at its own diagnostics cadence with the state resident in HBM and timed with CUDA events on the handle's stream, so that their step times stand
+    beside the headline in the same driver-run line.  They are not the bench value (config 4 is): context, a few seconds in total.
+    Config 3 takes a = (tau / tau_end)^m: read literally (tau_ref = tau0) its s = 1 leaves the leapfrog stability region after ~27 steps (R3)."""
+    from paper_1809_00995_b200 import binding as ahs
+    from paper_1809_00995_b200.synthetic import CONFIGS
+    peak, _ = measured_peak()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    out = []
+    for c in (2, 3, 5):
+        cfg = CONFIGS[c]
+        steps, every, N = cfg["steps"], max(cfg["diag_every"], 1), cfg["N"]
+        tau_ref = COMMON["tau0"] + steps * COMMON["dt"] if c == 3 else 0.0
+        with ahs.Simulation(N=N, precision=cfg["precision"], m=cfg["m"], s=cfg["s"], ic=cfg["ic"], seed=SEED, tau_ref=tau_ref, **COMMON) as sim:
+            sim.step(min(every, 10))                       # warm-up (part of the run: the step count goes on)
+            sim.diagnostics()
+            t_step = t_diag = 0.0
+            done, calls, d = 0, 0, None
+            while done < steps:
+                n = min(every, steps - done)
+                a, b, e = ev(), ev(), ev()
+                a.record(); sim.step(n); b.record()
+                d = sim.diagnostics()
+                e.record()
+                torch.cuda.synchronize()
+                t_step += a.elapsed_time(b); t_diag += b.elapsed_time(e)
+                done += n; calls += 1
+                if d["nonfinite"]:
+                    break
+            bps = BYTES_PER_SITE[cfg["precision"]] * N ** 3 * done / (t_step * 1e-3) / 1e9
+            out.append({"config": c, "lattice": N, "precision": cfg["precision"], "m": cfg["m"], "s": cfg["s"], "ic": cfg["ic"], "tau_ref": tau_ref or COMMON["tau0"],
+                        "steps": done, "diagnostics_calls": calls, "kernel": sim.kernel_kind, "ms_per_leapfrog_step": t_step / done,
+                        "site_updates_per_s": N ** 3 * done / (t_step * 1e-3), "achieved_GBps": bps, "frac_of_measured_copy": bps / peak,
+                        "diagnostics_ms_per_call": t_diag / calls, "diagnostics_overhead_at_its_cadence": t_diag / t_step,
+                        "nonfinite": int(d["nonfinite"]), "n_pierced_last": int(d["n_pierced"]), "gauss_max_last": d["gauss_max"]})
+    return out
 
 
 def run_e2e(args, sim, torch, max_over_ranks, barrier, world):
