@@ -3,19 +3,23 @@
 //
 // Same tile and staging as the step kernel (ahs_step_march.cu): a CTA owns TX x TY sites in (x, y) and marches over a
 // z-chunk; phi_re, phi_im, theta_0..2 of plane k+3 are streamed by the copy engine (one tensor-map TMA copy per plane, row
-// copies on the periodic edge in y) into a 4-stage ring of halo'd shared-memory tiles (one `full` mbarrier per stage; the last
-// warp to finish with a stage re-fills it) while planes k, k+1 are in use; Pi and eps are read with streaming 16-byte loads.
+// copies on the periodic edge in y) into a 4-slot ring of halo'd shared-memory tiles (one `full` mbarrier per slot; the last
+// warp to finish with a slot re-fills it) while planes k, k+1 are in use; eps_1 and the row below it ride in the same slot
+// (one more tensor copy); Pi, eps_0, eps_2 are read with streaming 16-byte loads.  Inside a CTA the four warps sit side by side
+// along x and a warp's lanes are 8 vectors along x by 4 rows.
 // All the estimators need only FORWARD neighbours (x+k_i, x+k_i+k_j) of phi, theta -- except the divergence of eps,
-// whose -x / -y / -z terms come by shuffle, one extra row load and a carried register.
+// whose -x / -y / -z terms come by one scalar load, the staged row below and a carried register.
 //
-// The kernel is bound by instruction issue, not by HBM (profiles/r2_diag1024_f32_full.md: 85 % of the issue slots, 47 % of
-// the DRAM bandwidth), so ALL its arithmetic runs on pairs of neighbouring sites with sm_100's packed fp32 instructions
-// (ahs_pack.cuh; for fp64 lattices the same expressions element by element).
+// The kernel is bound by fp32 arithmetic, not by HBM (profiles/r5_diag1024_f32_full.md), so ALL its arithmetic runs on pairs
+// of neighbouring sites with sm_100's packed fp32 instructions (ahs_pack.cuh; for fp64 lattices the same expressions element
+// by element), and the sines / cosines inside the <v^2> sums may go to the special-function unit (SumsTrig below).
 //
-// Winding.  Every thread evaluates arg phi / 2 pi (branch-free atan2_turns) at the ten points of plane k+1 its V sites need
-// and carries them to the next plane in registers; there is NO exchange between warps and therefore no CTA barrier in the
-// march: the warps of a CTA drift freely and meet only at the stage ring's `full` mbarriers (an earlier version
-// computed each phase once into a shared arg tile and lost 31 % of its issue slots at the per-plane barrier, profiles/r2).
+// Winding.  arg phi / 2 pi (branch-free atan2_turns) is needed at the ten points of plane k+1 around a thread's V sites.  On
+// fp32 lattices a warp evaluates each phase of its 32 x 4 region and of that region's halo once and hands them round through
+// a private shared-memory tile (__syncwarp only); on fp64 lattices every thread evaluates its ten itself.  Either way there is
+// NO exchange between warps and therefore no CTA barrier in the march: the warps of a CTA drift freely and meet only at the
+// stage ring's `full` mbarriers (an earlier version computed each phase once per CTA into a shared arg tile and lost 31 % of
+// its issue slots at the per-plane barrier, profiles/r2).  The phases are carried to the next plane in registers.
 // The link numbers n_i^x = rint(t), t = arg^{x+k_i}/2pi - arg^x/2pi - theta_i^x/2pi, are formed in fp32 and
 // W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x) is summed exactly.  The decision is the fp64 one:
 //   |t - t_exact| <= 2 eps_a + 3e-8 + 1.6e-7 (1 + |t|) turns with eps_a <= 7.6e-8 turns per phase (atan2_turns, ahs_trig.cuh;
@@ -64,7 +68,19 @@ struct DiagCfg {
     static constexpr uint32_t E1_BYTES = E1_ELEMS * sizeof(T);
     static_assert(E1_BYTES % 128 == 0, "slots stay 128-byte aligned");
     static constexpr int SLOT_STRIDE = E1_OFF + E1_ELEMS;   // a ring slot = a stage, its side buffer, the eps_1 rows
-    static constexpr size_t SMEM = 128 + sizeof(T) * (size_t)(NSTAGE * SLOT_STRIDE);
+    // A warp covers WX columns x TY rows of the tile (lane = 8 vectors in x by 4 rows).  Its phase tile holds arg phi / 2 pi of one plane at
+    // those sites plus the row above and the column to the right ((TY + 1) x (WX + 1) values, rows PP apart): each phase is evaluated
+    // once per warp instead of by every thread that needs it.
+    static constexpr int NWARPS = NTHREADS / 32;
+    static constexpr int WX = 8 * V;
+    static constexpr int PP = WX + 4;                          // row pitch: the row vectors stay 16-byte aligned, rows fall in different banks
+    static constexpr int PT_FLOATS = (TY + 1) * PP;
+    static constexpr int NEXTRA = WX + 1 + TY;                 // the halo of a warp's region: row TY (WX + 1 values), column WX of rows 0 .. TY-1
+    static constexpr bool SHARE_PHASES = sizeof(T) == 4;       // fp64 lattices (half as many sites per warp) are faster without: 3.48 vs 3.57 ms at 512^3
+    static_assert(TY == 4 && TX == NWARPS * WX, "4 rows of 8 lanes; the warps side by side span the tile");
+    static_assert(NEXTRA <= 64, "two halo phases per lane");
+    static constexpr size_t RING_BYTES = sizeof(T) * (size_t)(NSTAGE * SLOT_STRIDE);
+    static constexpr size_t SMEM = 128 + RING_BYTES + sizeof(float) * (size_t)(NWARPS * PT_FLOATS);
 };
 
 // Link numbers of two links s -> t with angles th, fast path, all in fp32 and in turns: t = (at - as) - th / 2 pi from the
@@ -163,11 +179,14 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
 
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);    // full[s]: the bulk copies of stage s have landed
-    unsigned* released = reinterpret_cast<unsigned*>(full + NS);   // released[s]: how many of the TY warps have finished reading stage s
+    unsigned* released = reinterpret_cast<unsigned*>(full + NS);   // released[s]: how many of the CTA's warps have finished reading stage s
     T* stages = reinterpret_cast<T*>(smem + 128);          // ring slot s at stages + s SE: the stage, then (right-edge tiles under
                                                            // TMA) the side buffer of the wrapped column at + STAGE_STRIDE
 
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    // lane -> (lx, w): 8 vectors along x by 4 rows; the CTA's warps sit side by side along x.  A quarter-warp reads 128 contiguous bytes.
+    const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
+    const int lx = lane & 7, w = lane >> 3;
+    float* const ptile = reinterpret_cast<float*>(smem + 128 + C::RING_BYTES) + wq * C::PT_FLOATS;   // this warp's phase tile
     const int tiles_x = N / TX, tiles_y = N / TY;
     int bid = blockIdx.x;
     const int tx = bid % tiles_x;
@@ -176,7 +195,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     // z-chunk zc of nchunks: own planes [zc nz / nchunks, (zc + 1) nz / nchunks)
     const int x0 = tx * TX, y0 = ty * TY, z0 = (int)((long long)zc * zr.nz / nchunks);
     const int zlen = (int)((long long)(zc + 1) * zr.nz / nchunks) - z0;
-    const int xi = V * lane;
+    const int xi = wq * C::WX + V * lx;   // column of this thread's vector inside the tile
 
     const T* const src[5] = { f.phi_re, f.phi_im, f.th[0], f.th[1], f.th[2] };
     const P inv_dx2 = pk::splat((T)kd.inv_dx2), g_el = pk::splat((T)kd.gauge_norm), g_mag = pk::splat((T)(kd.gauge_norm * kd.inv_dx2));
@@ -222,28 +241,60 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     };
     // element (array a, row w + dr) right of this thread's vector: column xi + V (= TX for the last lane, which on a
     // right-edge tile under TMA reads the side buffer instead).  The offsets from the slot base are per-thread constants.
-    const bool side = wrapR && lane == 31;
+    const bool side = wrapR && xi + V == TX;
     auto edge_off = [&](int a, int r) { return side ? C::STAGE_STRIDE + (a * G::ROWS + r) * V : G::idx(a, r, xi + V); };
     const int eo_re = edge_off(0, w), eo_im = edge_off(1, w), eo_rey = edge_off(0, w + 1), eo_imy = edge_off(1, w + 1);
     const int eo_t1 = edge_off(3, w), eo_t2 = edge_off(4, w);
-    if (w == 0 && elect_one()) {
+    if (wq == 0 && elect_one()) {
 #pragma unroll
         for (int p = 0; p < NS; ++p)
             if (p <= zlen) issue_plane(p, p);
     }
+    // The halo of this warp's region, two sites per lane: halo site e <= WX is (row TY, column e), the others (row e - WX - 1, column WX).
+    // Offsets of phi_re of those sites inside a slot (phi_im is one array further) and where their phases go in the tile (-1: nothing).
+    int hx_src[2], hx_im[2], hx_dst[2];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const int e = 2 * lane + j;
+        const bool used = e < C::NEXTRA;
+        const int r = !used ? 0 : (e <= C::WX ? TY : e - C::WX - 1), c = !used ? 0 : (e <= C::WX ? e : C::WX);
+        const int col = wq * C::WX + c;   // column inside the CTA's tile (TX = the wrapped column of a right-edge tile)
+        hx_src[j] = (wrapR && col == TX) ? C::STAGE_STRIDE + r * V : G::idx(0, r, col);
+        hx_im[j] = (wrapR && col == TX) ? G::ROWS * V : G::ARR_ELEMS;
+        hx_dst[j] = used ? r * C::PP + c : -1;
+    }
 
-    // arg phi / 2 pi at the V sites of this thread (pairs p0: row w, p1: row w+1) and at the site right of them (pe = rows
-    // w, w+1).  Every thread evaluates the ten phases it needs itself (2.5 per site instead of 1): no exchange, hence no CTA
-    // barrier anywhere in the march -- the warps of a CTA drift freely and only meet at the stage ring's mbarriers.
+    // arg phi / 2 pi of one plane at the V sites of this thread (p0), in the row above (p1) and right of the vector (pe = rows w, w+1).
+    // fp32 lattices: every thread evaluates the phases of its own sites and of two sites of the warp's halo, the warp exchanges them through
+    // its phase tile and the thread reads p1, pe back: 1.5 evaluations per site instead of the 2.5 of every thread for itself, and still
+    // no exchange between warps -- the warps of a CTA drift freely and only meet at the stage ring's mbarriers.
     auto phases_of = [&](const T* st, float2 (&p0)[NP], float2 (&p1)[NP], float2& pe) {
         const VecT pr = lds_vec<T, V>(st + G::idx(0, w, xi)), pi = lds_vec<T, V>(st + G::idx(1, w, xi));
-        const VecT pry = lds_vec<T, V>(st + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(st + G::idx(1, w + 1, xi));
+        if constexpr (!C::SHARE_PHASES) {   // fp64 lattices: every thread evaluates the ten phases it needs itself (measured faster there)
+            const VecT pry = lds_vec<T, V>(st + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(st + G::idx(1, w + 1, xi));
+#pragma unroll
+            for (int h = 0; h < NP; ++h) {
+                p0[h] = atan2_turns(to_float2(pk::at<T, V>(pi.v, h)), to_float2(pk::at<T, V>(pr.v, h)));
+                p1[h] = atan2_turns(to_float2(pk::at<T, V>(piy.v, h)), to_float2(pk::at<T, V>(pry.v, h)));
+            }
+            pe = atan2_turns(make_float2((float)st[eo_im], (float)st[eo_imy]), make_float2((float)st[eo_re], (float)st[eo_rey]));
+            return;
+        }
+        __syncwarp();   // every lane has read the previous plane's phases before anyone overwrites the tile
 #pragma unroll
         for (int h = 0; h < NP; ++h) {
             p0[h] = atan2_turns(to_float2(pk::at<T, V>(pi.v, h)), to_float2(pk::at<T, V>(pr.v, h)));
-            p1[h] = atan2_turns(to_float2(pk::at<T, V>(piy.v, h)), to_float2(pk::at<T, V>(pry.v, h)));
+            *reinterpret_cast<float2*>(ptile + w * C::PP + V * lx + 2 * h) = p0[h];
         }
-        pe = atan2_turns(make_float2((float)st[eo_im], (float)st[eo_imy]), make_float2((float)st[eo_re], (float)st[eo_rey]));
+        const float2 hx = atan2_turns(make_float2((float)st[hx_src[0] + hx_im[0]], (float)st[hx_src[1] + hx_im[1]]),
+                                      make_float2((float)st[hx_src[0]], (float)st[hx_src[1]]));
+        if (hx_dst[0] >= 0) ptile[hx_dst[0]] = hx.x;
+        if (hx_dst[1] >= 0) ptile[hx_dst[1]] = hx.y;
+        __syncwarp();
+        const float* up = ptile + (w + 1) * C::PP + V * lx;
+#pragma unroll
+        for (int h = 0; h < NP; ++h) p1[h] = *reinterpret_cast<const float2*>(up + 2 * h);
+        pe = make_float2(ptile[w * C::PP + V * lx + V], up[V]);
     };
     // the pair of phases one site to the right of pair h: (p[2h+1], p[2h+2]), the last one being the edge phase
     auto shifted = [&](const float2 (&p)[NP], int h, float e) { return make_float2(p[h].y, h + 1 < NP ? p[h + 1 < NP ? h + 1 : h].x : e); };
@@ -420,7 +471,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
             nonfinite += bad ? 1u : 0u;
         }
         E2m = E2;
-        // This warp is done with stage `ring` (plane it).  The LAST of the TY warps to say so re-fills it with plane it + NS: nobody
+        // This warp is done with stage `ring` (plane it).  The LAST of the CTA's warps to say so re-fills it with plane it + NS: nobody
         // ever waits for a stage to become free.  (An earlier version let a rotating warp spin on an `empty` mbarrier before issuing:
         // its elected lane and its 31 siblings then ran the rest of the plane as two groups, every instruction issued twice, and a
         // __syncwarp() there made the whole warp wait instead -- profiles/r4_diag1024_f32_full.md.)  The acq_rel counter orders all
@@ -429,7 +480,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
         if (lane == 0) {
             unsigned before;
             asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(before) : "r"(smem_u32(&released[ring])) : "memory");
-            if (before == TY - 1) {
+            if (before == C::NWARPS - 1) {
                 released[ring] = 0u;
                 if (it + NS <= zlen) {
                     fence_proxy_async();
