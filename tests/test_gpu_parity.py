@@ -520,6 +520,40 @@ def test_full_size_1024_sampled_windows_and_closed_forms(ahs, oracle):
         assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"])
 
 
+def test_full_size_512_fp64_sampled_windows(ahs, oracle):
+    """configs[4] (512^3 fp64, m = 1, s = 1, the configuration bench.py --lattice 512 --precision f64 times) at full size, north_star's
+    20 steps: sampled windows as in the 1024^3 test (the oracle steps each window as a periodic 56^3 lattice from the Philox initial
+    condition of that window; compared on the 16^3 interior the wrong wrap cannot have reached).  Interiors sit on tile corners of the
+    fp64 march (x multiple of 64, y multiple of 4), on its z-chunk boundaries (z multiple of 32) and on the periodic corner.  Strict
+    norm: max |d| / max |oracle| <= 1e-12 over the interior, per field array; then the diagnostics' closed forms and Gauss's law."""
+    N, nsteps, halo, inner = 512, 20, 20, 16
+    seed, B = 180900995, inner + 2 * halo
+    with ahs.Simulation(N=N, precision="f64", m=1.0, s=1.0, seed=seed) as sim:
+        assert sim.kernel_kind == "march"
+        sim.step(nsteps)
+        rng = np.random.default_rng(9)
+        interiors = [(-8, -8, -8), (64 - 8, 4 - 8, 32 - 8), (256 - 2, 300 + 1, 96 - 6), (512 - 64 - 5, 512 - 4 - 6, 480),
+                     (448 - 8, 256 - 8, 512 - 32 - 8), (-8, 200, 224 - 8)]
+        interiors += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(2)]
+        pw = oracle.Params(N=B, m=1.0, s=1.0)
+        sl = slice(halo, halo + inner)
+        worst = np.zeros(10)
+        for io in interiors:
+            origin = tuple(v - halo for v in io)
+            ref = oracle.initial_condition_window(pw, seed, N, origin)
+            oracle.step(pw, ref, 0, nsteps)
+            got = _gather_window(sim, origin, B)
+            for k in range(10):
+                d = np.abs(got[k][sl, sl, sl] - ref[k][sl, sl, sl]).max() / np.abs(ref[k][sl, sl, sl]).max()
+                worst[k] = max(worst[k], d)
+                assert d <= TOL["f64"], (io, oracle.FIELD_NAMES[k], d)
+        record("full_size_512_fp64_windows", nsteps=nsteps, windows=len(interiors), inner=inner, halo=halo, max_strict=float(worst.max()),
+               strict_per_field={n: float("%.3g" % e) for n, e in zip(oracle.FIELD_NAMES, worst)})
+        d = sim.diagnostics()
+        assert d["nonfinite"] == 0 and d["step"] == nsteps
+        assert d["gauss_max"] <= 1e-12 * max(1.0, d["gauss_rhs_rms"])
+
+
 def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
     """Regression for a shared-memory race of the marching step kernel (profiles/r2_race.md): a tensor / bulk copy
     issued right after __syncthreads() could overwrite a stage other warps were still reading -- about one corrupted
