@@ -62,7 +62,8 @@ def parse_args():
     ap.add_argument("--tau-ref", type=float, default=0.0, help="a = (tau/tau_ref)^m; 0 = tau0 (DESIGN.md R3: s != 0 runs leave the "
                     "stability region after ~80 steps at m=1 unless tau_ref is the end time)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "march"])
-    ap.add_argument("--e2e-steps", type=int, default=4, help="timed end-to-end steps (each uploads the full state)")
+    ap.add_argument("--e2e-steps", type=int, default=10, help="timed end-to-end steps (each uploads the full state; the two-handle pipeline's "
+                    "drain, one evolution without an upload behind it, is inside the timed region and is amortised over them)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--slabs", type=int, default=0, help="cut the lattice into this many z-slabs (ahs_group, DESIGN.md 10) driven by this one "
                     "process; 0 = one handle")
