@@ -49,8 +49,8 @@ template <typename T> struct StepCoefT { T c1, c2, c3, d1, d2, d3, dt, sigma2; }
 //   double: 4 rows, 2 CTAs/SM (255 registers: at 168 the kernel spills ~100 B per thread and plane and waits on the reloads,
 //           profiles/r4_step512_f64_full.md), 4 stages (two CTAs leave room for a deeper ring)
 template <typename T> struct StepShape;
-template <> struct StepShape<float> { static constexpr int TY = 4, MINB = 3, NS = 3; };
-template <> struct StepShape<double> { static constexpr int TY = 4, MINB = 2, NS = 4; };
+template <> struct StepShape<float> { static constexpr int TY = 4, MINB = 3, NS = 3; static constexpr bool LATE_WAIT = true; };
+template <> struct StepShape<double> { static constexpr int TY = 4, MINB = 2, NS = 4; static constexpr bool LATE_WAIT = false; };
 
 template <typename T, int TY_, int NS_>
 struct MarchCfg {
@@ -89,6 +89,8 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
     uint64_t* xch = full + NS;   // exchange barrier: one phase per plane, every thread arrives
+    uint64_t* t2full = xch + 1;  // t2full[slot]: theta_2 of a plane has landed in its ring slot (its own barriers: theta_2 of the CURRENT plane
+                                 // is needed at the top of the plane, the stage of the NEXT plane only half-way through it)
     T* stages = reinterpret_cast<T*>(smem + 128);
     T* th2ring = stages + NS * SE;
     T* wrapS = th2ring + C::T2_SLOTS * C::T2_STRIDE;      // side buffers of the wrapped halo column (x-edge tiles under TMA)
@@ -113,6 +115,8 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+#pragma unroll
+        for (int s = 0; s < C::T2_SLOTS; ++s) mbar_init(&t2full[s], 1);
         mbar_init(xch, C::NTHREADS);
         mbar_fence_init();
     }
@@ -142,12 +146,13 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
             issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
         }
     };
-    auto issue_th2 = [&](int slot, int bar, int p) {   // theta_2 of march plane p -> ring slot, completion on full[bar]
+    auto issue_th2 = [&](int slot, int p) {   // theta_2 of march plane p -> ring slot, completion on t2full[slot]
+        mbar_arrive_expect_tx(&t2full[slot], G::ARR_BYTES + wrap2_tx);
         if (tma_tile) {
-            tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &full[bar]);
-            if (wrapL || wrapR) tma_load_4d(wrapT + slot * C::WRAP2_STRIDE, &map_wth2, xw, y0 - 1, plane_of(p), 4, &full[bar]);
+            tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &t2full[slot]);
+            if (wrapL || wrapR) tma_load_4d(wrapT + slot * C::WRAP2_STRIDE, &map_wth2, xw, y0 - 1, plane_of(p), 4, &t2full[slot]);
         } else {
-            issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &full[bar], src2, N, x0, y0, plane_of(p));
+            issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &t2full[slot], src2, N, x0, y0, plane_of(p));
         }
     };
     // column x0-1 (array a, row r) of a staged plane / of a theta_2 slot, and the element right of this thread's vector
@@ -160,11 +165,10 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     if (w == 0) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
-            const bool t2 = i < T2S;   // theta_2 of the first planes rides on the barrier of its own plane
             if (i <= zlen + 1 && elect_one()) {   // (planes 0 .. zlen+1 are all this chunk reads; nothing may be in flight at exit)
-                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx + (t2 ? G::ARR_BYTES + wrap2_tx : 0u));
+                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx);
                 issue_stage(i, i);
-                if (t2) issue_th2(i, i, i);
+                if (i < T2S && i <= zlen) issue_th2(i, i);   // (theta_2 is read of planes 0 .. zlen only)
             }
         }
     }
@@ -175,6 +179,7 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     // ---- prologue: z-products of plane z0-1 (needs planes z0-1 and z0) ---------------------------------------------
     mbar_wait(&full[0], 0);
     mbar_wait(&full[1], 0);
+    mbar_wait(&t2full[0], 0);
     {
         const T* sc = stages;
         const T* sn = stages + SE;
@@ -231,15 +236,19 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
         if (((w + it) % TY) == ISSUER && it + NS - 1 <= zlen + 1 && elect_one()) {
             const int s = (it + NS - 1) % NS;   // with it: theta_2 of plane it+NS-2 -> the slot that held plane it-1
             fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1 / of the prologue: all reads of that stage are done)
-            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + G::ARR_BYTES + wrap_tx + wrap2_tx);
+            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + wrap_tx);
             issue_stage(s, it + NS - 1);
-            issue_th2((it + NS - 2) % T2S, s, it + NS - 2);   // (it is read at iteration it+NS-2, after the wait on this barrier)
+            if (it + NS - 2 <= zlen) issue_th2((it + NS - 2) % T2S, it + NS - 2);   // (read at iteration it+NS-2, after the wait on its own barrier)
         }
 
         const size_t g = gnext;                                         // plane z0 + it - 1
         const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested one plane ago
 
-        mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
+        mbar_wait(&t2full[it % T2S], (it / T2S) & 1);   // theta_2 of this plane (requested NS-2 planes ago)
+        // The stage of the NEXT plane is needed for the +z neighbours only.  fp32: wait for it after the trigonometry of the in-plane links (a
+        // third of the plane's work later: the copy has that much longer to land; 15.3 -> 15.05 ms at 1024^3 on a 1.49 GHz board); fp64: here
+        // (measured: no gain from waiting later, profiles/r5_step1024_f32_full.md)
+        if constexpr (!StepShape<T>::LATE_WAIT) mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
 
         // ---- halo products, shared out over the warps (no dedicated producer warp).  Row y0-1: one site per lane, every
         //      HSTRIDE-th warp in rotation; column x0-1: one warp per plane.  Called before the exchange barrier is signalled.
@@ -281,8 +290,6 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
             const VecT t0 = lds_vec<T, V>(sc + G::idx(2, w, xi)), t1 = lds_vec<T, V>(sc + G::idx(3, w, xi)), t2 = lds_vec<T, V>(t2c + G::idx(0, w, xi));
             const VecT pry = lds_vec<T, V>(sc + G::idx(0, w + 1, xi)), piy = lds_vec<T, V>(sc + G::idx(1, w + 1, xi));
             const VecT t0y = lds_vec<T, V>(sc + G::idx(2, w + 1, xi)), t2y = lds_vec<T, V>(t2c + G::idx(0, w + 1, xi));
-            const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
-            const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
             const T prx_e = edgeR(sc, wsc, 0, w, xi + V), pix_e = edgeR(sc, wsc, 1, w, xi + V);
             const T t1x_e = edgeR(sc, wsc, 3, w, xi + V), t2x_e = edgeR(t2c, wtc, 0, w, xi + V);
             T lfr[V], lfi[V], J0[V], J1[V], J2[V], b0r[V], b0i[V], S01[V], S02[V], S12[V], b2r[V], b2i[V];
@@ -293,15 +300,22 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
             sincos_vec<V>(t1.v, s1, c1);
             sincos_vec<V>(t2.v, s2, c2);
             {
-                // Xi_ij^x = th_i^x + th_j^{x+k_i} - th_i^{x+k_j} - th_j^x  (Eq. 3)
-                T X01[V], X02[V], X12[V];
+                // Xi_ij^x = th_i^x + th_j^{x+k_i} - th_i^{x+k_j} - th_j^x  (Eq. 3): the plaquette inside the plane first
+                T X01[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) X01[v] = t0.v[v] + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - t1.v[v];
+                sin_vec<V>(X01, S01);
+            }
+            if constexpr (StepShape<T>::LATE_WAIT) mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
+            const VecT prz = lds_vec<T, V>(sn + G::idx(0, w, xi)), piz = lds_vec<T, V>(sn + G::idx(1, w, xi));
+            const VecT t0z = lds_vec<T, V>(sn + G::idx(2, w, xi)), t1z = lds_vec<T, V>(sn + G::idx(3, w, xi));
+            {
+                T X02[V], X12[V];
 #pragma unroll
                 for (int v = 0; v < V; ++v) {
-                    X01[v] = t0.v[v] + next_x<T, V>(t1, v, t1x_e) - t0y.v[v] - t1.v[v];
                     X02[v] = t0.v[v] + next_x<T, V>(t2, v, t2x_e) - t0z.v[v] - t2.v[v];
                     X12[v] = t1.v[v] + t2y.v[v] - t1z.v[v] - t2.v[v];
                 }
-                sin_vec<V>(X01, S01);
                 sin_vec<V>(X02, S02);
                 sin_vec<V>(X12, S12);
             }
