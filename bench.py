@@ -43,8 +43,8 @@ FALLBACK_HBM_GBS = 6650.0                         # B200_PROFILING.md fallback i
 # the line then carries "traffic": null.  A capture is only listed while the kernel it was taken on is the one that ships
 # (the capture names its commit).
 NCU_TRAFFIC = {
-    ("march", "f32", 1024): (88.51e9, "profiles/r5_step1024_f32_full.md (45.61 GB read + 42.90 GB written per launch; capture of the step kernel that ships)"),
-    ("march", "f64", 512): (21.81e9, "profiles/r5_step512_f64_full.md (11.12 GB read + 10.69 GB written per launch; capture of the step kernel that ships)"),
+    ("march", "f32", 1024): (89.21e9, "profiles/r6_step1024_f32_full.md (46.31 GB read + 42.90 GB written per launch; capture of the step kernel that ships)"),
+    ("march", "f64", 512): (21.80e9, "profiles/r6_step512_f64_full.md (11.11 GB read + 10.69 GB written per launch; capture of the step kernel that ships)"),
 }
 
 
