@@ -49,8 +49,12 @@ template <typename T> struct StepCoefT { T c1, c2, c3, d1, d2, d3, dt, sigma2; }
 //   double: 4 rows, 2 CTAs/SM (255 registers: at 168 the kernel spills ~100 B per thread and plane and waits on the reloads,
 //           profiles/r4_step512_f64_full.md), 4 stages (two CTAs leave room for a deeper ring)
 template <typename T> struct StepShape;
-template <> struct StepShape<float> { static constexpr int TY = 4, MINB = 3, NS = 3; static constexpr bool LATE_WAIT = true; };
-template <> struct StepShape<double> { static constexpr int TY = 4, MINB = 2, NS = 4; static constexpr bool LATE_WAIT = false; };
+//   LATE_WAIT: wait for the next plane's stage behind the in-plane trigonometry (float: -2 % under the power cap; double: no gain)
+//   T2_RING  : slots of the theta_2 ring.  NS - 1 (theta_2 is never read one plane ahead) with a barrier of its own keeps the float kernel at
+//              63.9 KB per CTA, inside the SM's 196 KB shared-memory configuration (profiles/r6_step1024_f32_full.md); the double kernel, two CTAs
+//              per SM, has room for NS slots, theta_2 then rides on its plane's stage barrier one plane earlier (4.69 -> 4.62 ms at 512^3)
+template <> struct StepShape<float> { static constexpr int TY = 4, MINB = 3, NS = 3, T2_RING = 2; static constexpr bool LATE_WAIT = true; };
+template <> struct StepShape<double> { static constexpr int TY = 4, MINB = 2, NS = 4, T2_RING = 4; static constexpr bool LATE_WAIT = false; };
 
 template <typename T, int TY_, int NS_>
 struct MarchCfg {
@@ -58,7 +62,9 @@ struct MarchCfg {
     static constexpr int TY = TY_;
     static constexpr int NSTAGE = NS_;                       // plane it + NSTAGE - 1 is in flight while planes it, it + 1 are read
     using G = TileGeom<T, V, TY, 4, NSTAGE>;                // a stage: phi_re, phi_im, theta_0, theta_1 of one plane
-    static constexpr int T2_SLOTS = NSTAGE - 1;              // theta_2 is never read one plane ahead: its ring is one slot shorter
+    static constexpr int T2_SLOTS = StepShape<T>::T2_RING;   // NSTAGE - 1 (own barriers) or NSTAGE (theta_2 rides on its plane's stage barrier)
+    static constexpr bool T2_OWN = T2_SLOTS < NSTAGE;
+    static_assert(T2_SLOTS == NSTAGE || T2_SLOTS == NSTAGE - 1, "theta_2 ring");
     static constexpr int TX = G::TX;
     static constexpr int NTHREADS = TY * 32;
     static constexpr int YEX_ELEMS = 4 * TY * TX;         // b1.re, b1.im, S01, S12 of rows -1 .. TY-2 (one parity)
@@ -146,15 +152,18 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
             issue_rows<G, 4>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
         }
     };
-    auto issue_th2 = [&](int slot, int p) {   // theta_2 of march plane p -> ring slot, completion on t2full[slot]
-        mbar_arrive_expect_tx(&t2full[slot], G::ARR_BYTES + wrap2_tx);
+    // theta_2 of march plane p -> ring slot p % T2S; completion on t2full[slot], or (T2S = NS: same slot index as the stage) on full[slot]
+    auto issue_th2 = [&](int slot, int p) {
+        uint64_t* bar = C::T2_OWN ? &t2full[slot] : &full[slot];
+        if (C::T2_OWN) mbar_arrive_expect_tx(bar, G::ARR_BYTES + wrap2_tx);
         if (tma_tile) {
-            tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, &t2full[slot]);
-            if (wrapL || wrapR) tma_load_4d(wrapT + slot * C::WRAP2_STRIDE, &map_wth2, xw, y0 - 1, plane_of(p), 4, &t2full[slot]);
+            tma_load_4d(th2ring + slot * C::T2_STRIDE, &map_th2, x0 - V, y0 - 1, plane_of(p), 4, bar);
+            if (wrapL || wrapR) tma_load_4d(wrapT + slot * C::WRAP2_STRIDE, &map_wth2, xw, y0 - 1, plane_of(p), 4, bar);
         } else {
-            issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, &t2full[slot], src2, N, x0, y0, plane_of(p));
+            issue_rows<G, 1>(th2ring + slot * C::T2_STRIDE, bar, src2, N, x0, y0, plane_of(p));
         }
     };
+    const uint32_t stage_tx = G::STAGE_BYTES + wrap_tx + (C::T2_OWN ? 0u : G::ARR_BYTES + wrap2_tx);
     // column x0-1 (array a, row r) of a staged plane / of a theta_2 slot, and the element right of this thread's vector
     auto colL = [&](const T* st, const T* side, int a, int r) -> T {
         return wrapL ? side[(a * G::ROWS + r + 1) * V + V - 1] : st[G::idx(a, r, -1)];
@@ -166,9 +175,9 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
             if (i <= zlen + 1 && elect_one()) {   // (planes 0 .. zlen+1 are all this chunk reads; nothing may be in flight at exit)
-                mbar_arrive_expect_tx(&full[i], G::STAGE_BYTES + wrap_tx);
+                mbar_arrive_expect_tx(&full[i], stage_tx);
                 issue_stage(i, i);
-                if (i < T2S && i <= zlen) issue_th2(i, i);   // (theta_2 is read of planes 0 .. zlen only)
+                if (!C::T2_OWN || (i < T2S && i <= zlen)) issue_th2(i, i);   // (own ring: theta_2 is read of planes 0 .. zlen only)
             }
         }
     }
@@ -179,7 +188,7 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     // ---- prologue: z-products of plane z0-1 (needs planes z0-1 and z0) ---------------------------------------------
     mbar_wait(&full[0], 0);
     mbar_wait(&full[1], 0);
-    mbar_wait(&t2full[0], 0);
+    if (C::T2_OWN) mbar_wait(&t2full[0], 0);
     {
         const T* sc = stages;
         const T* sn = stages + SE;
@@ -236,15 +245,16 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
         if (((w + it) % TY) == ISSUER && it + NS - 1 <= zlen + 1 && elect_one()) {
             const int s = (it + NS - 1) % NS;   // with it: theta_2 of plane it+NS-2 -> the slot that held plane it-1
             fence_proxy_async();   // (this thread waited on the exchange barrier of plane it-1 / of the prologue: all reads of that stage are done)
-            mbar_arrive_expect_tx(&full[s], G::STAGE_BYTES + wrap_tx);
+            mbar_arrive_expect_tx(&full[s], stage_tx);
             issue_stage(s, it + NS - 1);
-            if (it + NS - 2 <= zlen) issue_th2((it + NS - 2) % T2S, it + NS - 2);   // (read at iteration it+NS-2, after the wait on its own barrier)
+            if (C::T2_OWN) issue_th2((it + NS - 2) % T2S, it + NS - 2);   // (read at iteration it+NS-2, after the wait on its own barrier)
+            else issue_th2(s, it + NS - 1);
         }
 
         const size_t g = gnext;                                         // plane z0 + it - 1
         const VecT Pr = nPr, Pi = nPi, E0 = nE0, E1 = nE1, E2 = nE2;   // requested one plane ago
 
-        mbar_wait(&t2full[it % T2S], (it / T2S) & 1);   // theta_2 of this plane (requested NS-2 planes ago)
+        if (C::T2_OWN) mbar_wait(&t2full[it % T2S], (it / T2S) & 1);   // theta_2 of this plane (requested NS-2 planes ago)
         // The stage of the NEXT plane is needed for the +z neighbours only.  fp32: wait for it after the trigonometry of the in-plane links (a
         // third of the plane's work later: the copy has that much longer to land; 15.3 -> 15.05 ms at 1024^3 on a 1.49 GHz board); fp64: here
         // (measured: no gain from waiting later, profiles/r5_step1024_f32_full.md)
