@@ -239,7 +239,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
             issue_rows<G, 5>(stages + s * SE, &full[s], src, N, x0, y0, plane_of(p));
         }
     };
-    // element (array a, row w + dr) right of this thread's vector: column xi + V (= TX for the last lane, which on a
+    // element (array a, row w + dr) right of this thread's vector: column xi + V (= TX for the last vector of a row, which on a
     // right-edge tile under TMA reads the side buffer instead).  The offsets from the slot base are per-thread constants.
     const bool side = wrapR && xi + V == TX;
     auto edge_off = [&](int a, int r) { return side ? C::STAGE_STRIDE + (a * G::ROWS + r) * V : G::idx(a, r, xi + V); };
@@ -318,7 +318,7 @@ diag_march_kernel(DiagPtrs<T> f, int N, ZRange zr, int nchunks, DiagCoef kd, Dia
     }
 
     // The momenta (no halo) come straight from global memory: g = element offset of this thread's vector in plane z0 + it, a
-    // running offset; the row below (eps_1^{x-k_1}) and the site left of the tile (eps_0^{x-k_0}, lane 0) sit at fixed distances.
+    // running offset; the site left of the vector (eps_0^{x-k_0}; wrapped for the first vector of the lattice) sits at a fixed distance.
     const size_t plane_stride = (size_t)N * N;
     size_t g = ((size_t)(zr.zbase + z0) * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
     const ptrdiff_t d_site_left = (x0 + xi == 0) ? (ptrdiff_t)(N - 1) : -(ptrdiff_t)1;
