@@ -554,6 +554,22 @@ def test_full_size_512_fp64_sampled_windows(ahs, oracle):
         assert d["gauss_max"] <= 1e-12 * max(1.0, d["gauss_rhs_rms"])
 
 
+@pytest.mark.parametrize("prec,N", [("f32", 256), ("f64", 128)])
+def test_repeated_diagnostics_are_bit_identical(ahs, prec, N):
+    """The diagnostics march hands phases round inside a warp through shared memory (fp32) and re-fills its stage ring from whichever warp
+    releases a slot last: 100 calls on one snapshot must return the same record bit for bit (integer counts; fp64 sums in a fixed order
+    for a fixed launch shape), under both staging modes.  A race in either mechanism would show as a count or a sum that moves."""
+    with ahs.Simulation(N=N, precision=prec, seed=5) as sim:
+        sim.step(15)
+        for staging in (ahs.AHS_STAGING_TENSOR, ahs.AHS_STAGING_ROWS):
+            sim.set_option(ahs.AHS_OPT_STAGING, staging)
+            first = sim.diagnostics()
+            assert first["n_pierced"] > 0 and first["nonfinite"] == 0
+            for _ in range(100):
+                d = sim.diagnostics()
+                assert all(d[k] == first[k] or (d[k] != d[k] and first[k] != first[k]) for k in first), [k for k in first if d[k] != first[k]]
+
+
 def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
     """Regression for a shared-memory race of the marching step kernel (profiles/r2_race.md): a tensor / bulk copy
     issued right after __syncthreads() could overwrite a stage other warps were still reading -- about one corrupted
