@@ -254,6 +254,59 @@ AHS_API int32_t ahs_group_slab_count(ahs_group* group);
 AHS_API ahs_sim* ahs_group_slab(ahs_group* group, int32_t r);
 AHS_API int32_t ahs_group_destroy(ahs_group* group);                                 /* NULL is allowed */
 
+/*
+ * ---- diagnostics of a snapshot the caller holds, without any allocation --------------------------------------------------------
+ * Who this is for.  An evolution code that keeps its own ten field arrays on the GPU and wants the winding count (Eq. 11),
+ * the <v^2> sums (Eqs. 9-10, 12) and the Gauss residual (L72, L181) of them every few steps, from a place where it may not allocate:
+ *   - a production run that has sized its lattice to the last gigabyte of HBM, so that a cudaMalloc in the middle of the run can
+ *     fail after hours of evolution (a handle would ask for 15 N^3 values of its own plus pinned host memory);
+ *   - an analysis hook called from inside another framework's step loop (a PyTorch caching allocator that owns all free memory, a
+ *     job whose device memory was partitioned up front), where cudaMalloc / cudaFree also stall every stream of the device;
+ *   - a latency-critical loop that must not enter the driver's allocator at all.
+ * ahs_create_ex always allocates (pinned host memory for the result, and device memory unless device_buffer is given) and copies the
+ * fields into its own layout.  This call takes the caller's arrays where they are and calls no cudaMalloc, cudaMallocHost, cudaFree,
+ * stream / event creation or any other allocating routine, on the host or on the device.
+ *
+ * Scratch.  The per-block records of the reduction (and the final record before it is read back) live in one array that is part of
+ * the library image: AHS_STATIC_SCRATCH_BYTES (444.25 KiB) of device memory on EVERY GPU on which this process uses libahs, held from
+ * the moment the library's code is loaded onto that GPU until the process exits, whether this function is ever called or not.  It is
+ * the same one-thread-per-site kernel that AHS_KERNEL_GENERIC handles run, launched with the same shape (at most
+ * AHS_STATIC_MAX_RECORDS blocks of 128 threads, one record each), so on the same snapshot it returns what such a handle returns, bit
+ * for bit; it is about 8 x slower than the z-marching kernel of a handle (see N above).
+ *
+ * Limits.  4 <= N <= AHS_STATIC_MAX_N: the array holds a record for every block of the largest launch this kernel is given, so no
+ * lattice the library accepts is too big for it; any other N, and any launch that would need more than AHS_STATIC_MAX_RECORDS
+ * records, is refused with AHS_ERR_INVALID_ARG and a message naming the limit -- nothing is ever written past the array.  s is the
+ * constant params->s (no s(tau) schedule).
+ *
+ * First call.  The first call on each device looks up the device address of the array (cudaGetSymbolAddress, with that device
+ * current; this is also what makes the driver load the library's code, and with it the array, onto that GPU) and keeps it for later
+ * calls.  Make that first call during set-up, before any stream capture is begun on that device.  Later calls only launch three
+ * kernels (clear the result record, the site kernel, the finishing block) and copy 96 bytes back.
+ *
+ * Sharing.  There is ONE array per device and every call on that device uses it; it keeps whatever the last call left.  Nothing in it
+ * has to start at zero for correctness -- each call writes every record before it reads it and reads only the records of its own
+ * launch -- but the 96-byte result record is cleared first all the same, so that a result can never be a leftover of the call
+ * before.  Two calls whose kernels can run on the GPU at the same time (different streams, different host threads, another process's
+ * context does not count: it has its own copy) overwrite each other's records: the caller serialises calls per device.  A call
+ * returns only after its own result has been read back, so calls made one after the other from one thread never overlap.
+ *
+ * Arguments.
+ *   params    HOST.  Used: N, precision, dx, dt, lambda, e, sigma, m, s, tau0, tau_ref, c_B, c_E (meaning as for ahs_create_ex) and
+ *             stream (the kernels and the read-back run on it; NULL = the legacy default stream).  Ignored: ic_kind, kernel, seed,
+ *             device_buffer, device_buffer_bytes.
+ *   fields10  HOST array of ten DEVICE pointers in the field order at the top of this file (phi_re ... eps_2), each to N^3 values of
+ *             the storage type, site index x + N (y + N z), on the CURRENT device.  Read only; the caller keeps ownership and must
+ *             not change them until the call returns.  Arrays taken from a handle with ahs_field_device_ptr qualify.
+ *   step      n >= 0: the snapshot is { phi^n, theta^n at tau0 + n dt ; Pi^(n-1/2), eps^(n-1/2) }; sets the scale factors.
+ *   out       HOST, filled as by ahs_diagnostics_ex.
+ * Returns AHS_OK, AHS_ERR_NONFINITE (out still filled), AHS_ERR_INVALID_ARG (nothing launched) or AHS_ERR_CUDA.  Synchronises the
+ * stream.
+ */
+enum { AHS_STATIC_MAX_RECORDS = 4736, AHS_STATIC_MAX_N = 2048, AHS_STATIC_SCRATCH_BYTES = 96 * (4736 + 1) + 160 /* = 454912, a multiple of 256 */ };
+AHS_API int32_t ahs_diagnostics_static(const ahs_params* params /* HOST */, const void* const* fields10 /* HOST array of 10 DEVICE pointers */,
+                                       int64_t step, ahs_diag* out /* HOST */);
+
 /* Message of the last failure on this thread ("" if none). Never NULL. */
 AHS_API const char* ahs_last_error(void);
 

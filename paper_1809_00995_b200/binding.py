@@ -32,7 +32,9 @@ SYMBOLS = (
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
     "ahs_group_create", "ahs_group_step", "ahs_group_diagnostics", "ahs_group_get_fields_native", "ahs_group_set_fields_native",
     "ahs_group_synchronize", "ahs_group_slab_count", "ahs_group_slab", "ahs_group_destroy",
+    "ahs_diagnostics_static",
 )
+AHS_STATIC_MAX_RECORDS, AHS_STATIC_MAX_N, AHS_STATIC_SCRATCH_BYTES = 4736, 2048, 96 * (4736 + 1) + 160
 
 
 class ahs_params(C.Structure):
@@ -101,6 +103,7 @@ def load(path: str | None = None):
     lib.ahs_group_slab_count.argtypes = [vp]; lib.ahs_group_slab_count.restype = i32
     lib.ahs_group_slab.argtypes = [vp, i32]; lib.ahs_group_slab.restype = vp
     lib.ahs_group_destroy.argtypes = [vp]; lib.ahs_group_destroy.restype = i32
+    lib.ahs_diagnostics_static.argtypes = [C.POINTER(ahs_params), C.POINTER(vp), i64, C.POINTER(ahs_diag)]; lib.ahs_diagnostics_static.restype = i32
     _lib = lib
     return lib
 
@@ -376,6 +379,27 @@ class Group:
             _check(lib.ahs_get_state(C.c_void_p(lib.ahs_group_slab(self._g, r)), None, None, C.byref(nl)))
             tot += nl.value
         return tot
+
+
+def diagnostics_static(fields10, N, step, precision="f32", dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, m=1.0, s=0.0, tau0=1.0,
+                       tau_ref=0.0, c_B=0.0, c_E=0.0, stream=0, allow_nonfinite=True) -> dict:
+    """ahs_diagnostics_static: the diagnostics of ten field arrays the caller already holds on the current device, for callers that
+    cannot allocate (a run that has filled the GPU's memory, a hook inside another framework's loop where cudaMalloc would fail or
+    stall the device).  The library allocates nothing: its reduction scratch is a fixed 444 KiB array inside libahs.so, one per GPU,
+    shared by all calls -- so do not overlap two calls on one GPU, and make the first call on each GPU during set-up.
+    fields10: ten device addresses (ints) or objects with .data_ptr() (torch tensors), order FIELD_NAMES, N^3 values each of the
+    storage type.  `stream` is a cudaStream_t as an integer (0 = the default stream).  Returns the same dict as
+    Simulation.diagnostics()."""
+    if len(fields10) != 10:
+        raise ValueError("fields10 must hold ten device pointers")
+    p = ahs_params()
+    p.N, p.precision = int(N), _prec(precision)
+    p.dx, p.dt, p.lambda_, p.e, p.sigma, p.m, p.s, p.tau0, p.tau_ref = dx, dt, lambda0, e0, sigma, m, s, tau0, tau_ref
+    p.c_B, p.c_E, p.stream = c_B, c_E, int(stream)
+    ptrs = (C.c_void_p * 10)(*[int(f.data_ptr()) if hasattr(f, "data_ptr") else int(f) for f in fields10])
+    d = ahs_diag()
+    _check(load().ahs_diagnostics_static(C.byref(p), ptrs, int(step), C.byref(d)), allow=(AHS_ERR_NONFINITE,) if allow_nonfinite else ())
+    return {k: getattr(d, k) for k, _ in ahs_diag._fields_ if k != "reserved"}
 
 
 def create(N, dx, dt, lambda0, e0, sigma, m, s, tau0, seed):

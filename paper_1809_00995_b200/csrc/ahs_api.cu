@@ -851,3 +851,126 @@ ahs_sim* ahs_group_slab(ahs_group* g, int32_t r)
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// ahs_diagnostics_static (include/ahs.h): the diagnostics of a snapshot the CALLER holds, for callers that may not allocate -- a run
+// that has filled HBM, a hook inside another framework's step loop, a loop that must stay out of the driver's allocator (cudaMalloc
+// and cudaFree also stall every stream of the device).  No handle, no cudaMalloc / cudaMallocHost / cudaFree, no stream or event
+// creation: the reduction's per-block records, which a handle keeps behind its field arrays, live in the array below, which is part
+// of the library image.  The kernel is the one-thread-per-site diagnostics kernel of AHS_KERNEL_GENERIC handles, unchanged and with
+// the same launch shape, given the array's device address instead of a handle's scratch.
+// ---------------------------------------------------------------------------------------------------------------------------
+static_assert(sizeof(DiagPartial) == 96, "AHS_STATIC_SCRATCH_BYTES in include/ahs.h counts 96-byte records");
+static_assert(AHS_STATIC_SCRATCH_BYTES >= sizeof(DiagPartial) * (AHS_STATIC_MAX_RECORDS + 1) && AHS_STATIC_SCRATCH_BYTES % 256 == 0,
+              "the array holds AHS_STATIC_MAX_RECORDS block records and the result record");
+
+// AHS_STATIC_MAX_RECORDS block records followed by the result record.  Every GPU this process uses libahs on holds these 444.25 KiB
+// from the moment this file's code is loaded onto it until the process exits.  One array per device, shared by every call: it keeps
+// the last call's contents, and calls that overlap on the GPU race on it (see the header).
+// In HOST code the name g_static_scratch is only the key cudaGetSymbolAddress takes.  It is not a device address: a kernel handed
+// `g_static_scratch` (or &g_static_scratch[k]) from the host would be reading and writing host memory, or faulting.  Host code passes
+// static_scratch_address()'s result; device code of this file may use the name itself (static_clear_result does).
+static __device__ __align__(256) unsigned char g_static_scratch[AHS_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+// the array's device address on each device (every device has its own copy at its own address); NULL = not looked up yet
+std::atomic<void*> g_static_address[kStaticMaxDevices];
+
+// Set-up, once per device, with that device current (`device` is the caller's current device): the first call asks the runtime for
+// the address of this device's copy -- which also makes the driver load this file's code, and the array with it, onto the GPU, so it
+// belongs before any stream capture -- later calls read the stored pointer.  Two threads racing on the first call both look the
+// address up and store the same value.
+int static_scratch_address(int device, DiagPartial** out)
+{
+    if (device < 0 || device >= kStaticMaxDevices)
+        return fail(AHS_ERR_INVALID_ARG, "ahs_diagnostics_static serves device ordinals 0..%d (current device: %d)", kStaticMaxDevices - 1, device);
+    void* p = g_static_address[device].load(std::memory_order_acquire);
+    if (!p) {
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(AHS_ERR_CUDA, "cudaGetSymbolAddress(static scratch) on device %d: %s", device, cudaGetErrorString(e));
+        }
+        g_static_address[device].store(p, std::memory_order_release);
+    }
+    *out = static_cast<DiagPartial*>(p);
+    return AHS_OK;
+}
+
+// The result record of the call before must not be readable as this call's: zero it (device code names the array directly).
+__global__ void static_clear_result()
+{
+    unsigned long long* rec = reinterpret_cast<unsigned long long*>(g_static_scratch + sizeof(DiagPartial) * AHS_STATIC_MAX_RECORDS);
+    if (threadIdx.x < sizeof(DiagPartial) / sizeof(unsigned long long)) rec[threadIdx.x] = 0ull;
+}
+
+// how many block records the one-thread-per-site diagnostics kernel writes for an N^3 lattice (launch_diag_generic's grid)
+int64_t static_records_needed(int64_t N)
+{
+    const int64_t blocks = (N * N * N + 127) / 128;
+    return blocks < 148 * 32 ? blocks : 148 * 32;
+}
+
+template <typename T>
+int static_diag(const ahs_params& p, const void* const* fields10, const DiagCoef& c, DiagPartial* scratch, cudaStream_t st)
+{
+    DiagPtrs<T> f;
+    f.phi_re = (const T*)fields10[0]; f.phi_im = (const T*)fields10[1];
+    f.pi_re = (const T*)fields10[2]; f.pi_im = (const T*)fields10[3];
+    for (int i = 0; i < 3; ++i) { f.th[i] = (const T*)fields10[4 + i]; f.eps[i] = (const T*)fields10[7 + i]; }
+    return launch_diag_generic<T>(f, p.N, c, scratch, AHS_STATIC_MAX_RECORDS, scratch + AHS_STATIC_MAX_RECORDS, st);
+}
+
+}  // namespace
+
+extern "C" int32_t ahs_diagnostics_static(const ahs_params* params, const void* const* fields10, int64_t step, ahs_diag* out)
+{
+    if (!params || !fields10 || !out) return fail(AHS_ERR_INVALID_ARG, "params, fields10 and out must not be NULL");
+    const ahs_params& p = *params;
+    if (p.N < 4 || p.N > AHS_STATIC_MAX_N)
+        return fail(AHS_ERR_INVALID_ARG, "N = %d is outside 4..%d, the lattice sizes ahs_diagnostics_static accepts", p.N, (int)AHS_STATIC_MAX_N);
+    const int64_t need = static_records_needed(p.N);
+    if (need > AHS_STATIC_MAX_RECORDS)
+        return fail(AHS_ERR_INVALID_ARG, "N = %d needs %lld reduction records, the static scratch array holds %d (%d bytes)", p.N,
+                    (long long)need, (int)AHS_STATIC_MAX_RECORDS, (int)AHS_STATIC_SCRATCH_BYTES);
+    if (p.precision != AHS_F32 && p.precision != AHS_F64) return fail(AHS_ERR_INVALID_ARG, "precision must be AHS_F32 or AHS_F64");
+    if (!(p.dx > 0) || !(p.dt > 0) || !(p.lambda > 0) || !(p.e > 0) || !(p.sigma > 0)) return fail(AHS_ERR_INVALID_ARG, "dx, dt, lambda, e, sigma must be > 0");
+    if (!std::isfinite(p.m) || !std::isfinite(p.s) || !std::isfinite(p.tau0) || !std::isfinite(p.tau_ref) || p.tau_ref < 0)
+        return fail(AHS_ERR_INVALID_ARG, "m, s, tau0 must be finite and tau_ref >= 0");
+    if (p.m != 0.0 && !(p.tau0 - 0.5 * p.dt > 0)) return fail(AHS_ERR_INVALID_ARG, "tau0 - dt/2 must be > 0 when m != 0");
+    if (!std::isfinite(p.c_B) || p.c_B < 0 || !std::isfinite(p.c_E) || p.c_E < 0) return fail(AHS_ERR_INVALID_ARG, "c_B, c_E must be finite and >= 0 (0 = default 1)");
+    if (step < 0) return fail(AHS_ERR_INVALID_ARG, "step must be >= 0");
+
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce != cudaSuccess) { cudaGetLastError(); return fail(AHS_ERR_CUDA, "no CUDA device: %s (libahs has no CPU fallback)", cudaGetErrorString(ce)); }
+    for (int k = 0; k < 10; ++k) {
+        if (!fields10[k]) return fail(AHS_ERR_INVALID_ARG, "fields10[%d] is NULL", k);
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, fields10[k]) != cudaSuccess || (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) ||
+            (pa.type == cudaMemoryTypeDevice && pa.device != dev)) {
+            cudaGetLastError();
+            return fail(AHS_ERR_INVALID_ARG, "fields10[%d] is not device memory of the current device (%d)", k, dev);
+        }
+    }
+    DiagPartial* scratch = nullptr;
+    if (int r = static_scratch_address(dev, &scratch)) return r;
+
+    ahs_sim shell{};            // carries the parameters to diag_coefficients (host only: no s(tau) schedule, nothing allocated)
+    shell.p = p;
+    const DiagCoef c = diag_coefficients(&shell, step);
+    cudaStream_t st = (cudaStream_t)p.stream;
+    static_clear_result<<<1, 32, 0, st>>>();
+    AHS_CUDA(cudaGetLastError());
+    const int launched = p.precision == AHS_F32 ? static_diag<float>(p, fields10, c, scratch, st) : static_diag<double>(p, fields10, c, scratch, st);
+    if (launched < 0) return fail(launched, "diagnostics kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    DiagPartial rec;            // pageable host memory on this frame: the copy is staged by the driver, the synchronise below ends it
+    AHS_CUDA(cudaMemcpyAsync(&rec, scratch + AHS_STATIC_MAX_RECORDS, sizeof(rec), cudaMemcpyDeviceToHost, st));
+    AHS_CUDA(cudaStreamSynchronize(st));
+    fill_diag(out, p, step, (double)p.N * p.N * p.N, rec);
+    if (out->nonfinite) return fail(AHS_ERR_NONFINITE, "the snapshot holds non-finite field values at step %lld (%llu sites flagged)",
+                                    (long long)step, (unsigned long long)rec.nonfinite);
+    return AHS_OK;
+}
