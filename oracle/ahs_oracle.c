@@ -142,7 +142,8 @@ static double aho_u53(uint32_t hi, uint32_t lo)
  *   kind 1: Gaussian (BASELINE config 3; not in the paper): Box-Muller,
  *           u1 = u(r0,r1) + 2^-54, u2 = u(r2,r3), phi = sigma/sqrt2 * sqrt(-2 ln u1) * exp(i 2 pi u2)
  * pinned by: Philox KAT; |phi| = sigma exactly-to-rounding; pierced fraction 1/3 (four i.i.d.
- * uniform corner phases); Gauss residual identically 0 at n = 0; sample moments of kind 1.
+ * uniform corner phases); Gauss residual identically 0 at n = 0; sample moments of kind 1 and two
+ * sites of kind 1 by hand (Box-Muller written out in Python from the Philox words).
  * -------------------------------------------------------------------------------------------- */
 static void aho_ic_site(const aho_params* p, const uint32_t key[2], int64_t site, int32_t kind, double* re, double* im)
 {

@@ -168,6 +168,26 @@ def test_ic_gaussian_moments(oracle):
     assert abs(np.mean(re * im)) < 5 * 0.5 / math.sqrt(n)
 
 
+def test_ic_gaussian_two_sites_by_hand(oracle):
+    """The word-to-variate map of the Gaussian branch (oracle header, kind 1; BASELINE config 3 -- not in the paper, so the oracle's
+    own stated recipe is what is fixed): u1 = u53(r0, r1) + 2^-54 feeds the radius, u2 = u53(r2, r3) the angle, re = cos, im = sin,
+    Box-Muller written out here in Python.  The moments above cannot see a swap of the word pairs or of cos / sin; this does (the
+    alternatives are asserted to be far away, so the pin has teeth)."""
+    sigma, seed = 1.7, 180900995
+    p = oracle.Params(N=32, sigma=sigma)
+    f = oracle.initial_condition(p, seed=seed, kind=oracle.IC_GAUSSIAN)
+    phi = (f[0] + 1j * f[1]).reshape(-1)
+    u53 = lambda hi, lo: ((hi << 32 | lo) >> 11) * 2.0 ** -53
+    for site in (0, 31 * 32 * 32 + 5):
+        r = oracle.philox4x32_10((site, 0, 0, 0), (seed, 0))
+        u1, u2 = u53(r[0], r[1]) + 2.0 ** -54, u53(r[2], r[3])
+        z = sigma / math.sqrt(2.0) * math.sqrt(-2.0 * math.log(u1)) * cmath.exp(1j * TWO_PI * u2)
+        assert abs(phi[site] - z) < 4e-15 * max(1.0, abs(z))
+        swapped_words = sigma / math.sqrt(2.0) * math.sqrt(-2.0 * math.log(u2 + 2.0 ** -54)) * cmath.exp(1j * TWO_PI * (u1 - 2.0 ** -54))
+        swapped_parts = complex(z.imag, z.real)
+        assert abs(phi[site] - swapped_words) > 1e-3 and abs(phi[site] - swapped_parts) > 1e-3
+
+
 # ------------------------------------------------------------------------------------------------
 # P1  Gauss's law preserved to machine precision (PAPER.md L181)
 # ------------------------------------------------------------------------------------------------
