@@ -106,7 +106,8 @@ typedef struct {
 typedef struct {
     int64_t step;             /* n                                                                         */
     double tau;               /* tau_n = tau0 + n dt                                                       */
-    uint64_t n_pierced;       /* plaquettes with W != 0, Eq. 11 (L88-93), bit-exact integer                */
+    uint64_t n_pierced;       /* plaquettes with W != 0, Eq. 11 (L88-93), bit-exact integer (fp32 lattices on the
+                                 z-marching kernel: for |phi_re|, |phi_im| < 2^126; beyond, the sums overflow too) */
     uint64_t sum_abs_w;       /* sum |W| over the 3 N^3 plaquettes                                         */
     double L;                 /* (pi/6) dx n_pierced (L93)                                                 */
     double xi;                /* sqrt((N dx)^3 / L); +inf if n_pierced == 0                                */
@@ -197,7 +198,8 @@ AHS_API int32_t ahs_kernel_kind(ahs_sim* sim);
  *   AHS_OPT_STAGING      AHS_STAGING_TENSOR (default): halo'd tiles of the level-n fields (Eq. 4-5's phi, theta) are staged in
  *                        shared memory by tensor-map TMA copies wherever a tile does not straddle the periodic boundary in y;
  *                        AHS_STAGING_ROWS: by one bulk copy per tile row everywhere (the path tiles on that boundary always take).
- *   AHS_OPT_STEP_CHUNKS  number of z-chunks each (x, y) tile of the step march is cut into, 1..N (0 = the library's choice);
+ *   AHS_OPT_STEP_CHUNKS  number of z-chunks each (x, y) tile of the step march is cut into, 1..N (a slab of an ahs_group: 1..N / nslabs;
+ *                        0 = the library's choice);
  *   AHS_OPT_DIAG_CHUNKS  the same for the diagnostics march.  Chunks need not divide N.
  *   AHS_OPT_DIAG_TRIG    how the diagnostics march of an fp32 lattice evaluates the sines and cosines inside the sums of Eqs. 2, 9, 10
  *                        and 12 (link phases of the gradient term, plaquette angles of the magnetic term):
@@ -237,11 +239,15 @@ AHS_API int32_t ahs_destroy(ahs_sim* sim);
  * step.  CUDA events order step n+1 of a slab behind step n of its two neighbours; nothing waits on the device.  Results are those
  * of a single handle: fields bit for bit, counts exactly, sums to the rounding order of the final reduction.
  * params: as for ahs_create_ex with device_buffer = stream = NULL and N % 128 == 0 (fp32) / N % 64 == 0 (fp64); nslabs in 1..64
- * must divide N.  Slabs on different devices need peer access between neighbours.  One host thread drives a group.
+ * must divide N, and a slab holds at most 2047 planes (N = 2048 needs nslabs >= 2).  Slabs on different devices need peer access
+ * between neighbours.  One host thread drives a group.
  */
 typedef struct ahs_group ahs_group;
 AHS_API ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int32_t* devices /* HOST, may be NULL */);
-AHS_API int32_t ahs_group_step(ahs_group* group, int32_t n);                         /* asynchronous, like ahs_step */
+/* n steps, asynchronous like ahs_step.  If a launch or an event call fails part-way through a step, some slabs have run that step and
+ * others have not: the group then refuses ahs_group_step, ahs_group_diagnostics and ahs_group_get_fields_native with AHS_ERR_STATE
+ * until ahs_group_set_fields_native has set the fields again (or the group is destroyed). */
+AHS_API int32_t ahs_group_step(ahs_group* group, int32_t n);
 AHS_API int32_t ahs_group_diagnostics(ahs_group* group, ahs_diag* out /* HOST */);   /* every slab's pass, combined; synchronises */
 /* The whole lattice in the storage type, 10 N^3 values in the field order above, gathered from / scattered to the slabs (HOST
  * pointers; ahs_group_set_fields_native also sets the step counter and fills the ghost planes).  Synchronise. */
@@ -249,8 +255,9 @@ AHS_API int32_t ahs_group_get_fields_native(ahs_group* group, void* host10);
 AHS_API int32_t ahs_group_set_fields_native(ahs_group* group, const void* host10, int64_t step);
 AHS_API int32_t ahs_group_synchronize(ahs_group* group);
 AHS_API int32_t ahs_group_slab_count(ahs_group* group);
-/* The handle of slab r (owned by the group: for ahs_set_option, ahs_get_state, ahs_kernel_kind; its fields are read and written
- * through the group).  NULL if r is out of range. */
+/* The handle of slab r (owned by the group: for ahs_set_option, ahs_set_s_schedule, ahs_get_state, ahs_kernel_kind, ahs_coefficients,
+ * ahs_synchronize).  It is stepped, measured and its fields are read and written through the group only: ahs_step, ahs_diagnostics*,
+ * ahs_get_fields* and ahs_set_fields* on it return AHS_ERR_STATE.  NULL if r is out of range. */
 AHS_API ahs_sim* ahs_group_slab(ahs_group* group, int32_t r);
 AHS_API int32_t ahs_group_destroy(ahs_group* group);                                 /* NULL is allowed */
 

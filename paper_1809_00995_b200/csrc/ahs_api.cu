@@ -387,6 +387,7 @@ ahs_sim* ahs_create(int32_t N, double dx, double dt, double lambda, double e, do
 int32_t ahs_step(ahs_sim* s, int32_t n)
 {
     AHS_ENTER(s);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab is stepped through its ahs_group (ahs_group_step keeps the slabs' buffers and ghost planes in step)");
     if (n < 0) return fail(AHS_ERR_INVALID_ARG, "n must be >= 0");
     for (int32_t k = 0; k < n; ++k) {
         const int r = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
@@ -401,6 +402,7 @@ int32_t ahs_step(ahs_sim* s, int32_t n)
 int32_t ahs_diagnostics_launch(ahs_sim* s)
 {
     AHS_ENTER(s);
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's diagnostics are taken through its ahs_group (ahs_group_diagnostics combines the slabs' sums)");
     const int r = s->p.precision == AHS_F32 ? do_diag<float>(s) : do_diag<double>(s);
     if (r < 0) return fail(r, "diagnostics kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     s->launches += r;
@@ -412,6 +414,7 @@ int32_t ahs_diagnostics_fetch(ahs_sim* s, ahs_diag* out)
 {
     AHS_ENTER(s);
     if (!out) return fail(AHS_ERR_INVALID_ARG, "out is NULL");
+    if (!s->zr.periodic) return fail(AHS_ERR_STATE, "a z-slab's diagnostics are taken through its ahs_group (ahs_group_diagnostics combines the slabs' sums)");
     if (s->diag_step < 0) return fail(AHS_ERR_STATE, "no diagnostics launch is pending");
     AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
     AHS_CUDA(cudaStreamSynchronize(s->stream));
@@ -568,7 +571,7 @@ int32_t ahs_set_option(ahs_sim* s, int32_t option, int32_t value)
             return AHS_OK;
         case AHS_OPT_STEP_CHUNKS:
         case AHS_OPT_DIAG_CHUNKS:
-            if (value > s->p.N) return fail(AHS_ERR_INVALID_ARG, "at most N = %d z-chunks per tile", s->p.N);
+            if (value > s->zr.nz) return fail(AHS_ERR_INVALID_ARG, "at most %d z-chunks per tile (the z-planes this handle owns)", s->zr.nz);
             (option == AHS_OPT_STEP_CHUNKS ? s->opt.step_chunks : s->opt.diag_chunks) = value;
             return AHS_OK;
         case AHS_OPT_DIAG_TRIG:
@@ -620,6 +623,7 @@ struct ahs_group {
     int parity;                         // parity of the NEXT step's events
     bool have_prev;
     int64_t step;
+    bool poisoned;                      // a step failed after some slabs had already run it: fields inconsistent until they are set again
 };
 
 namespace {
@@ -632,7 +636,9 @@ char* plane_ptr(const ahs_sim* s, int slot_index, int local_plane)
     return s->base + (size_t)slot_index * s->array_bytes + (size_t)local_plane * s->p.N * s->p.N * s->elem;
 }
 
-// slab r's next launch runs behind the last step (and anything enqueued after it) of its two neighbours
+// slab r's next launch runs behind everything its two neighbours had enqueued when they last recorded done[] -- their last step, or the
+// diagnostics pass after it (ahs_group_diagnostics records the event again behind its kernels).  cudaStreamWaitEvent covers only work
+// enqueued BEFORE that cudaEventRecord: whatever touches a slab's arrays or ghost planes later must record the event again.
 int wait_for_neighbours(ahs_group* g, int r)
 {
     if (!g->have_prev) return AHS_OK;
@@ -694,6 +700,9 @@ ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int3
     if (nslabs < 1 || nslabs > 64 || !valid_N(params->N) || params->N % nslabs != 0) {
         fail(AHS_ERR_INVALID_ARG, "nslabs must be in 1..64 and divide N"); return nullptr;
     }
+    if (params->N / nslabs > 2047) {   // the diagnostics march addresses a slab's planes (ghost plane below included) with 11 bits
+        fail(AHS_ERR_INVALID_ARG, "a slab holds at most 2047 z-planes: cut N = %d into at least 2 slabs", params->N); return nullptr;
+    }
     if (params->device_buffer || params->stream) { fail(AHS_ERR_INVALID_ARG, "a group owns its memory and streams: device_buffer and stream must be NULL"); return nullptr; }
     int ndev = 0, home = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || cudaGetDevice(&home) != cudaSuccess) {
@@ -702,7 +711,7 @@ ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int3
     }
     ahs_group* g = new (std::nothrow) ahs_group();
     if (!g) { fail(AHS_ERR_OOM, "host allocation failed"); return nullptr; }
-    g->p = *params; g->P = nslabs; g->parity = 0; g->have_prev = false; g->step = 0;
+    g->p = *params; g->P = nslabs; g->parity = 0; g->have_prev = false; g->step = 0; g->poisoned = false;
     g->slab.assign(nslabs, nullptr);
     g->done[0].assign(nslabs, nullptr); g->done[1].assign(nslabs, nullptr);
     const int nz = params->N / nslabs;
@@ -753,21 +762,39 @@ ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int3
     return g;
 }
 
+namespace {
+
+const char kPoisoned[] = "an earlier ahs_group_step failed part-way through a step: the slabs' fields are inconsistent until ahs_group_set_fields_native sets them again";
+
+// one slab's share of one step: wait for the neighbours' last step, launch, record
+int step_slab(ahs_group* g, int r)
+{
+    ahs_sim* s = g->slab[r];
+    DeviceGuard guard(s->device);
+    if (!guard.ok()) return fail(AHS_ERR_CUDA, "cannot make device %d current", s->device);
+    if (int e = wait_for_neighbours(g, r)) return e;
+    const int rc = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
+    if (rc < 0) return fail(rc, "step kernel launch failed on slab %d at step %lld: %s", r, (long long)s->step, cudaGetErrorString(cudaGetLastError()));
+    s->launches += rc;
+    AHS_CUDA(cudaEventRecord(g->done[g->parity][r], s->stream));
+    return AHS_OK;
+}
+
+}  // namespace
+
 int32_t ahs_group_step(ahs_group* g, int32_t n)
 {
     if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
+    if (g->poisoned) return fail(AHS_ERR_STATE, "%s", kPoisoned);
     if (n < 0) return fail(AHS_ERR_INVALID_ARG, "n must be >= 0");
     for (int32_t k = 0; k < n; ++k) {
-        for (int r = 0; r < g->P; ++r) {
-            ahs_sim* s = g->slab[r];
-            DeviceGuard guard(s->device);
-            if (!guard.ok()) return fail(AHS_ERR_CUDA, "cannot make device %d current", s->device);
-            if (int e = wait_for_neighbours(g, r)) return e;
-            const int rc = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
-            if (rc < 0) return fail(rc, "step kernel launch failed on slab %d at step %lld: %s", r, (long long)s->step, cudaGetErrorString(cudaGetLastError()));
-            s->launches += rc;
-            AHS_CUDA(cudaEventRecord(g->done[g->parity][r], s->stream));
-        }
+        for (int r = 0; r < g->P; ++r)
+            if (int e = step_slab(g, r)) {
+                // slabs 0..r-1 have kicked their momenta in place and stored into their neighbours' ghost planes, the others have
+                // not, and no buffer has been flipped: a retry would step those slabs twice.  Refuse further work on these fields.
+                g->poisoned = true;
+                return e;
+            }
         for (ahs_sim* s : g->slab) { s->cur ^= 1; s->step += 1; }
         g->parity ^= 1;
         g->have_prev = true;
@@ -779,6 +806,7 @@ int32_t ahs_group_step(ahs_group* g, int32_t n)
 int32_t ahs_group_diagnostics(ahs_group* g, ahs_diag* out)
 {
     if (!g || !out) return fail(AHS_ERR_INVALID_ARG, "null group or out");
+    if (g->poisoned) return fail(AHS_ERR_STATE, "%s", kPoisoned);
     for (int r = 0; r < g->P; ++r) {
         ahs_sim* s = g->slab[r];
         DeviceGuard guard(s->device);
@@ -788,6 +816,16 @@ int32_t ahs_group_diagnostics(ahs_group* g, ahs_diag* out)
         s->launches += rc;
         AHS_CUDA(cudaMemcpyAsync(s->result_host, s->result, sizeof(DiagPartial), cudaMemcpyDeviceToHost, s->stream));
     }
+    // The neighbours' next step stores into this slab's ghost planes, and eps_2's ghost plane -- which this pass's Gauss residual reads
+    // -- is single-buffered: that step must run behind this pass.  Record the event the neighbours will wait on again, behind the
+    // diagnostics kernels (after every slab's waits above were enqueued, so that the passes themselves do not wait for one another);
+    // the ordering then holds without the host synchronise below.
+    for (int r = 0; r < g->P; ++r) {
+        ahs_sim* s = g->slab[r];
+        DeviceGuard guard(s->device);
+        AHS_CUDA(cudaEventRecord(g->done[g->parity ^ 1][r], s->stream));
+    }
+    g->have_prev = true;
     DiagPartial t;
     std::memset(&t, 0, sizeof(t));
     for (int r = 0; r < g->P; ++r) {   // fixed order: the result does not depend on which slab finishes first
@@ -808,6 +846,7 @@ int32_t ahs_group_diagnostics(ahs_group* g, ahs_diag* out)
 int32_t ahs_group_get_fields_native(ahs_group* g, void* host10)
 {
     if (!g || !host10) return fail(AHS_ERR_INVALID_ARG, "null group or host10");
+    if (g->poisoned) return fail(AHS_ERR_STATE, "%s", kPoisoned);
     const size_t field = (size_t)g->p.N * g->p.N * g->p.N * g->slab[0]->elem;
     for (ahs_sim* s : g->slab) {
         DeviceGuard guard(s->device);
@@ -833,7 +872,9 @@ int32_t ahs_group_set_fields_native(ahs_group* g, const void* host10, int64_t st
         s->step = step;
     }
     g->step = step;
-    return refresh_ghosts(g);
+    const int rc = refresh_ghosts(g);
+    if (rc == AHS_OK) g->poisoned = false;   // every live field, ghost plane and step counter has just been written
+    return rc;
 }
 
 int32_t ahs_group_synchronize(ahs_group* g)

@@ -517,6 +517,9 @@ int launch_diag_march(const DiagPtrs<T>& f, int N, const ZRange& zr, const DiagC
 {
     using C = DiagCfg<T>;
     if (!march_supported<T>(N) || zr.nz < 1) return AHS_ERR_INVALID_ARG;
+    // a doubt-list entry keeps the LOCAL plane index in its top 11 bits: the last own plane must be <= 2047 (a whole 2048^3 lattice
+    // is; a single slab of 2048 planes with its ghost plane below is not -- ahs_group_create refuses it)
+    if (zr.zbase + zr.nz > 2048) return AHS_ERR_INVALID_ARG;
     // fp64 lattices always take the polynomials (the hardware unit is an fp32 one)
     const bool hw = sizeof(T) == 4 && opt.diag_trig == AHS_TRIG_HARDWARE;
     auto kern = hw ? diag_march_kernel<T, sizeof(T) == 4 ? AHS_TRIG_HARDWARE : AHS_TRIG_POLYNOMIAL> : diag_march_kernel<T, AHS_TRIG_POLYNOMIAL>;

@@ -151,7 +151,9 @@ __device__ __forceinline__ void sincos_hw(float2 x, float2& s, float2& c)
 // q = min/max in [0, 1] (MUFU.RCP and a multiply), odd polynomial of degree 15 in q fitted to atan(q) / 2 pi, then the
 // octant fix-ups, whose constants 1/4 and 1/2 are exact in turns.  Absolute error <= 5e-8 turns in the fp32 emulation of
 // tests/tools/fit_trig.py (the fast path's error budget assumes <= 7.6e-8 turns = 4.8e-7 rad).  atan2_turns(0, 0) and
-// non-finite inputs give NaN, which sends the link to the fp64 evaluation.
+// non-finite inputs give NaN, which sends the link to the fp64 evaluation.  Range: max(|x|, |y|) < 2^126 -- above it the approximate
+// reciprocal flushes to zero and q = 0 comes out without a NaN, so such a link is NOT re-evaluated (field values of that size, 10^38
+// times the vacuum expectation value, also overflow every sum of the pass; include/ahs.h states the range at n_pierced).
 __device__ __forceinline__ float rcp_approx(float x)
 {
     float r;

@@ -554,6 +554,63 @@ def test_full_size_512_fp64_sampled_windows(ahs, oracle):
         assert d["gauss_max"] <= 1e-12 * max(1.0, d["gauss_rhs_rms"])
 
 
+def test_config3_gaussian_ic_fields_after_20_steps(ahs, oracle):
+    """BASELINE config 3 as configured except for the size: fp32, matter era (m = 2), true equations (s = 1), literal a = (tau/tau0)^m,
+    GAUSSIAN initial condition (amplitudes from 0 to ~3 sigma, not |phi| = sigma) -- the whole 128^3 lattice against the oracle after
+    north_star's 20 steps, from the oracle's Gaussian IC uploaded to the device.  R14 norm asserted; the strict absolute norm is
+    recorded and bounded by 2e-4 x the field's own maximum (eps grows to ~30 in these 20 steps, SURVEY 8(c) 'Config consequences of
+    G3': 2e-4 absolute is below one fp32 ulp of such a value)."""
+    N, nsteps = 128, 20
+    with ahs.Simulation(N=N, precision="f32", m=2.0, s=1.0, ic="none") as sim:
+        p = oracle_params(oracle, sim)
+        ref = rounded(oracle.initial_condition(p, 180900995, kind=oracle.IC_GAUSSIAN), "f32")
+        assert np.abs(np.hypot(ref[0], ref[1]) - 1.0).max() > 0.5          # not the random-phase IC
+        sim.set_fields(ref, 0)
+        sim.step(nsteps)
+        got = sim.get_fields()
+        oracle.step(p, ref, 0, nsteps)
+        assert_fields("config3_gaussian_128", got, ref, "f32", oracle.FIELD_NAMES, strict=False, N=N, m=2.0, s=1.0, kernel=sim.kernel_kind, nsteps=nsteps)
+        d = sim.diagnostics()
+        assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"])
+        check_diag(oracle, p, sim, "f32", ref, nsteps)
+
+
+def test_full_size_512_config3_sampled_windows(ahs, oracle):
+    """configs[2] (BASELINE config 3) as configured and at full size: 512^3 fp32, m = 2, s = 1, a = (tau/tau0)^m read literally, the
+    DEVICE's own Gaussian initial condition (ahs_ic.cu), 20 steps.  Sampled windows as in the 1024^3 test: the oracle generates the
+    Gaussian IC of each 56^3 window from the Philox specification (aho_ic_window, kind 1), steps it 20 times as a small periodic
+    lattice and is compared on the 16^3 interior the wrong wrap cannot have reached.  Interiors sit on tile corners of the fp32 march
+    (x multiple of 128, y multiple of 4), on z-chunk boundaries and on the periodic corner.  R14 norm asserted (max |d| /
+    max(1, max |oracle|) <= 2e-4); the strict absolute maximum is recorded."""
+    N, nsteps, halo, inner = 512, 20, 20, 16
+    seed, B = 180900995, inner + 2 * halo
+    with ahs.Simulation(N=N, precision="f32", m=2.0, s=1.0, ic="gaussian", seed=seed) as sim:
+        assert sim.kernel_kind == "march"
+        sim.step(nsteps)
+        rng = np.random.default_rng(13)
+        interiors = [(-8, -8, -8), (128 - 8, 4 - 8, 32 - 8), (256 - 2, 300 + 1, 96 - 6), (512 - 128 - 5, 512 - 4 - 6, 480),
+                     (384 - 8, 256 - 8, 512 - 16 - 8), (-8, 200, 224 - 8)]
+        interiors += [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(2)]
+        pw = oracle.Params(N=B, m=2.0, s=1.0)
+        sl = slice(halo, halo + inner)
+        worst, worst_r14 = np.zeros(10), np.zeros(10)
+        for io in interiors:
+            origin = tuple(v - halo for v in io)
+            ref = rounded(oracle.initial_condition_window(pw, seed, N, origin, kind=oracle.IC_GAUSSIAN), "f32")
+            oracle.step(pw, ref, 0, nsteps)
+            got = _gather_window(sim, origin, B)
+            for k in range(10):
+                d = np.abs(got[k][sl, sl, sl] - ref[k][sl, sl, sl]).max()
+                r14 = d / max(1.0, np.abs(ref[k][sl, sl, sl]).max())
+                worst[k], worst_r14[k] = max(worst[k], d), max(worst_r14[k], r14)
+                assert r14 <= TOL["f32"], (io, oracle.FIELD_NAMES[k], d, r14)
+        record("full_size_512_config3_windows", nsteps=nsteps, windows=len(interiors), inner=inner, halo=halo, max_r14=float(worst_r14.max()),
+               max_strict=float(worst.max()), strict_per_field={n: float("%.3g" % e) for n, e in zip(oracle.FIELD_NAMES, worst)})
+        d = sim.diagnostics()
+        assert d["nonfinite"] == 0 and d["step"] == nsteps and d["n_pierced"] > 0
+        assert d["gauss_max"] <= 2e-5 * max(1.0, d["gauss_rhs_rms"])
+
+
 @pytest.mark.parametrize("prec,N", [("f32", 256), ("f64", 128)])
 def test_repeated_diagnostics_are_bit_identical(ahs, prec, N):
     """The diagnostics march hands phases round inside a warp through shared memory (fp32) and re-fills its stage ring from whichever warp
@@ -820,6 +877,91 @@ def test_slab_group_from_uploaded_fields_and_options(ahs, oracle):
         ahs.Group(N=N, nslabs=3)                                                          # must divide N
     with pytest.raises(ahs.AhsError):
         ahs.Group(N=N, nslabs=2, devices=[0, 99])
+
+
+def test_slab_handles_are_driven_through_their_group(ahs):
+    """A slab's handle (ahs_group_slab) takes options and reports state, but stepping it, measuring it or touching its fields on its
+    own would leave the group's buffers and ghost planes out of step: those calls return AHS_ERR_STATE and change nothing.  Chunk
+    counts are bounded by the planes the slab owns, not by N."""
+    import ctypes as C
+    N, P = 128, 2
+    lib = ahs.load()
+    with ahs.Simulation(N=N, precision="f32", seed=5) as ref, ahs.Group(N=N, nslabs=P, precision="f32", seed=5) as g:
+        h = C.c_void_p(lib.ahs_group_slab(g._g, 1))
+        d = ahs.ahs_diag()
+        buf = np.zeros((10, N, N, N), dtype=np.float32)
+        assert lib.ahs_step(h, 1) == ahs.AHS_ERR_STATE and "ahs_group" in ahs.last_error()
+        assert lib.ahs_diagnostics_launch(h) == ahs.AHS_ERR_STATE
+        assert lib.ahs_diagnostics_ex(h, C.byref(d)) == ahs.AHS_ERR_STATE
+        assert lib.ahs_diagnostics_fetch(h, C.byref(d)) == ahs.AHS_ERR_STATE
+        assert lib.ahs_get_fields_native(h, buf.ctypes.data) == ahs.AHS_ERR_STATE
+        assert lib.ahs_set_fields_native(h, buf.ctypes.data, 0) == ahs.AHS_ERR_STATE
+        assert lib.ahs_set_option(h, ahs.AHS_OPT_STEP_CHUNKS, N // P + 1) == ahs.AHS_ERR_INVALID_ARG     # 64 planes per slab
+        assert lib.ahs_set_option(h, ahs.AHS_OPT_DIAG_CHUNKS, N // P + 1) == ahs.AHS_ERR_INVALID_ARG
+        assert lib.ahs_set_option(h, ahs.AHS_OPT_STEP_CHUNKS, N // P) == ahs.AHS_OK
+        st = C.c_int64(-1)
+        assert lib.ahs_get_state(h, C.byref(st), None, None) == ahs.AHS_OK and st.value == 0             # none of the refused calls stepped it
+        ref.step(6)
+        g.step(3)
+        g.diagnostics()
+        g.step(3)
+        assert np.array_equal(g.get_fields_native(), ref.get_fields_native())
+    with pytest.raises(ahs.AhsError) as e:
+        ahs.Group(N=2048, nslabs=1)                                # refused before any memory is asked for
+    assert "at least 2 slabs" in str(e.value)
+
+
+def _device_count():
+    import torch
+    return torch.cuda.device_count()
+
+
+def test_slab_group_on_several_devices_bit_for_bit(ahs):
+    """The path a one-GPU box never reaches: slabs on different GPUs (peer access between neighbours, the step kernel's stores into
+    the neighbours' ghost planes over NVLink, events waited for across devices, the per-device shared-memory attribute).  Same bar
+    as on one GPU: the single lattice bit for bit."""
+    ndev = _device_count()
+    if ndev < 2:
+        pytest.skip("needs at least 2 CUDA devices, this box has %d: the multi-device slab path stays unmeasured here" % ndev)
+    N, nsteps = 256, 12
+    with ahs.Simulation(N=N, precision="f32", m=1.0, s=0.0, seed=77) as ref:
+        ref.step(nsteps)
+        want, dref = ref.get_fields_native(), ref.diagnostics()
+    for P, devices in ((2, [0, 1]), (4, [d % ndev for d in range(4)]), (ndev, list(range(ndev)))):
+        if N % P:
+            continue
+        with ahs.Group(N=N, nslabs=P, devices=devices, precision="f32", m=1.0, s=0.0, seed=77) as g:
+            g.step(5)
+            d5 = g.diagnostics()
+            g.step(nsteps - 5)
+            got, d = g.get_fields_native(), g.diagnostics()
+            assert np.array_equal(got, want), (devices, [int((got[k] != want[k]).sum()) for k in range(10)])
+            assert d5["step"] == 5 and (d["n_pierced"], d["sum_abs_w"], d["nonfinite"]) == (dref["n_pierced"], dref["sum_abs_w"], 0), devices
+            assert d["v2_num"] == pytest.approx(dref["v2_num"], rel=1e-11) and d["gauss_max"] == dref["gauss_max"], devices
+
+
+def test_handles_on_two_devices_driven_from_one_thread(ahs):
+    """include/ahs.h: a handle belongs to the device that was current when it was created, and every later call switches to that
+    device for its own duration -- one host thread drives handles on several GPUs without calling cudaSetDevice itself."""
+    import torch
+    if _device_count() < 2:
+        pytest.skip("needs at least 2 CUDA devices, this box has %d" % _device_count())
+    kw = dict(N=128, precision="f32", m=1.0, s=0.0, seed=11)
+    home = torch.cuda.current_device()
+    with torch.cuda.device(1):
+        far = ahs.Simulation(**kw)
+    near = ahs.Simulation(**kw)
+    try:
+        for _ in range(3):                                          # interleaved, never switching devices here
+            near.step(2)
+            far.step(2)
+        dn, df = near.diagnostics(), far.diagnostics()
+        assert torch.cuda.current_device() == home
+        assert np.array_equal(near.get_fields_native(), far.get_fields_native())
+        assert dn == df
+    finally:
+        far.destroy()
+        near.destroy()
 
 
 @pytest.mark.parametrize("prec,N,kernel", [("f64", 64, "auto"), ("f32", 128, "auto"), ("f64", 20, "generic")])
