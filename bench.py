@@ -178,11 +178,18 @@ def run_reference(args):
     while args.cpu_lattice ** 3 * args.cpu_leapfrog * (steps + warm) > 6e8 and args.cpu_lattice > 32:
         args.cpu_lattice //= 2
     r = oracle_sample(args, steps=steps, warmup=warm, threads=0)     # all host cores
+    # the config names what this arm RAN (a bounded fp64 sample of the workload on the host cores), and which workload it samples
+    target = workload_config(args)
+    config = {"workload": "bounded sample on the host cores: %d^3 periodic lattice, f64, same physics, %d leapfrog steps + 1 diagnostics per "
+                          "bench step -- a sample of: %s" % (args.cpu_lattice, args.cpu_leapfrog, target["workload"]),
+              "lattice": args.cpu_lattice, "leapfrog_per_step": args.cpu_leapfrog, "diagnostics_per_step": 1,
+              "sample": r["sample"], "workload_lattice": target["lattice"], "workload_leapfrog_per_step": target["leapfrog_per_step"],
+              "parallelism": "host threads x%d (rank 0 only)" % r["cores"]}
     line = {
         "impl": "reference", "metric": "lattice site-updates/sec per leapfrog step", "value": r["value"], "unit": "site-updates/s",
         "n_gpus": args.gpus, "steps": steps, "warmup": warm, "ms_per_step": 1e3 * r["seconds"] / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(args),
+        "config": config,
         "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
         "e2e": {"value": r["value"], "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,

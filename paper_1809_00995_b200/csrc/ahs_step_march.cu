@@ -1,10 +1,13 @@
 // ahs_step_march.cu -- the fused leapfrog step (Eqs. 4-7) as a 2.5D z-march for sm_100a.
 //
 // One CTA owns a tile of TX x TY sites in (x, y) (TX = 32 lanes x one 16-byte vector, TY rows = TY warps) and
-// marches over `zlen` planes.  The level-n fields phi, theta (5 arrays) of plane k+2 are streamed into a 3-stage
-// ring of halo'd shared-memory tiles with cp.async.bulk (UBLKCP) + mbarrier while planes k, k+1 are in use
-// (ahs_stage.cuh; the issuing warp rotates); Pi and eps (no halo) are read with streaming 16-byte loads and all ten
-// outputs leave as 16-byte stores.
+// marches over `zlen` planes.  The level-n fields of the planes ahead are streamed into rings of halo'd shared-memory
+// tiles that complete on mbarriers while planes k, k+1 are in use: phi_re, phi_im, theta_0, theta_1 in an NS-stage ring
+// (float 3, double 4), theta_2 in a ring of its own (StepShape::T2_RING).  A tile that does not touch the periodic
+// boundary in y is fetched by tensor-map TMA (cp.async.bulk.tensor, UTMALDG: one copy for the four-array stage, one for
+// theta_2, plus a V-wide copy of the wrapped halo column for x-edge tiles); tiles on the y boundary, lattices one tile
+// wide and AHS_STAGING_ROWS use one bulk copy per tile row (cp.async.bulk, UBLKCP; ahs_stage.cuh).  The issuing warp
+// rotates.  Pi and eps (no halo) are read with streaming 16-byte loads and all ten outputs leave as 16-byte stores.
 //
 // Compute-once form.  Each site owner computes, from raw phi, theta of the site and of its FORWARD neighbours only,
 //   U_j = exp(-i theta_j)                         3 sincos       (link phases, Eq. 3 / L46-51, q = +1)
@@ -23,12 +26,15 @@
 //   curl_2 = (S02^{-x} - S02) + (S12^{-y} - S12)                                            (Eq. 5)
 // followed by the kicks and the drift into the other (phi, theta) buffer (Eqs. 6-7).
 //
-// One CTA barrier per plane.  Phase 1 (before the barrier) does all the trigonometry and folds every term that the
-// thread owns -- including the -x terms obtained by shuffle and the -z terms carried in registers -- into partial
-// results (q = Pi' without the -y / halo hops, phi + dt q, eps' and theta + dt eps' without the -y / halo sines).
-// Phase 2 (after the barrier) adds the few terms that crossed a warp boundary and stores.  The exchange rows are
-// double-buffered by plane parity so that the barrier of plane k+1 also orders "everyone has read plane k's
-// exchange" before it is overwritten at plane k+2.
+// One exchange point per plane, and it is an mbarrier (`xch`, one phase per plane, every thread arrives), not a
+// __syncthreads: a thread ARRIVES as soon as its exchange-row / halo-column stores and its stage reads have been issued and
+// WAITS only where it needs the other warps' products, so the trigonometry of the in-plane links sits between the two.
+// Phase 1 (before the wait) does all the trigonometry and folds every term that the thread owns -- including the -x terms
+// obtained by shuffle and the -z terms carried in registers -- into partial results (q = Pi' without the -y / halo hops,
+// phi + dt q, eps' and theta + dt eps' without the -y / halo sines).  Phase 2 (after the wait) adds the few terms that
+// crossed a warp boundary and stores.  The exchange rows are double-buffered by plane parity so that the phase of plane
+// k+1 also orders "everyone has read plane k's exchange" before it is overwritten at plane k+2; the same phase tells the
+// issuing warp that a stage slot has been read by all and may be re-filled.
 // The paper's kernels stage raw fields per kernel and recompute every phase (L107-109); this is a different design.
 #include <cstring>
 
@@ -45,7 +51,8 @@ namespace {
 template <typename T> struct StepCoefT { T c1, c2, c3, d1, d2, d3, dt, sigma2; };
 
 // Launch shape per storage type: rows per tile (= warps per CTA), CTAs per SM the register budget is cut for, ring depth.
-//   float : 4 rows, 3 CTAs/SM (168 registers), 3 stages -- measured fastest (profiles/r2, r3)
+//   float : 4 rows, 3 CTAs/SM (register budget 65536 / (3 x 128) = 170, i.e. at most 168; ptxas uses 160 in the build that ships,
+//           profiles/r6_sass_histogram.md), 3 stages -- measured fastest (profiles/r6_step1024_f32_full.md)
 //   double: 4 rows, 2 CTAs/SM (255 registers: at 168 the kernel spills ~100 B per thread and plane and waits on the reloads,
 //           profiles/r4_step512_f64_full.md), 4 stages (two CTAs leave room for a deeper ring)
 template <typename T> struct StepShape;
