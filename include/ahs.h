@@ -67,7 +67,7 @@ enum { AHS_TRIG_HARDWARE = 0, AHS_TRIG_POLYNOMIAL = 1 };
  *   N               lattice is N^3, periodic, 4 <= N <= 2048.  The z-marching kernels (TMA-staged tiles, the ones that run near
  *                   the HBM roofline) need N % 128 == 0 (fp32) or N % 64 == 0 (fp64) and are chosen automatically when that
  *                   holds.  Any other N runs on the one-thread-per-site kernels, which are about 6 x slower on the step and
- *                   8 x slower on the diagnostics (profiles/r1_launches_1024.md); ahs_kernel_kind tells which one a handle uses.
+ *                   8 x slower on the diagnostics (profiles/HISTORY.md r1); ahs_kernel_kind tells which one a handle uses.
  *   dx, dt          lattice spacing and conformal time step, > 0.
  *   lambda, e, sigma  lambda_0, e_0 of Eq. 8 and the vacuum expectation value, > 0.
  *   m               a(tau) = (tau/tau_ref)^m : 0 static, 1 radiation, 2 matter.

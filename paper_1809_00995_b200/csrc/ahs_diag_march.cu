@@ -19,7 +19,7 @@
 // a private shared-memory tile (__syncwarp only); on fp64 lattices every thread evaluates its ten itself.  Either way there is
 // NO exchange between warps and therefore no CTA barrier in the march: the warps of a CTA drift freely and meet only at the
 // stage ring's `full` mbarriers (an earlier version computed each phase once per CTA into a shared arg tile and lost 31 % of
-// its issue slots at the per-plane barrier, profiles/r2).  The phases are carried to the next plane in registers.
+// its issue slots at the per-plane barrier, profiles/HISTORY.md r2).  The phases are carried to the next plane in registers.
 // The link numbers n_i^x = rint(t), t = arg^{x+k_i}/2pi - arg^x/2pi - theta_i^x/2pi, are formed in fp32 and
 // W_ij = -(n_i^x + n_j^{x+k_i} - n_i^{x+k_j} - n_j^x) is summed exactly.  The decision is the fp64 one:
 //   |t - t_exact| <= 2 eps_a + 3e-8 + 1.6e-7 (1 + |t|) turns with eps_a <= 7.6e-8 turns per phase (atan2_turns, ahs_trig.cuh;
@@ -129,7 +129,7 @@ __device__ __forceinline__ float2 to_float2(double2 v) { return make_float2((flo
 // in fp64 straight from global memory (same arithmetic as diag_generic_kernel), added to one extra partial record.
 // Integer sums: the order of the atomics does not matter.  ~4e-4 of the thread-planes end up here on smooth or random
 // fields; resolving them in-line (an out-of-line call inside the march) made every warp of the CTA wait for the one
-// that took the slow path (profiles/r2: 30 % of the issue slots), a separate pass costs ~0.1 ms at 1024^3.
+// that took the slow path (profiles/HISTORY.md r2: 30 % of the issue slots), a separate pass costs ~0.1 ms at 1024^3.
 template <typename T>
 __global__ void __launch_bounds__(128) diag_resolve_kernel(DiagPtrs<T> f, int N, int periodic_z, const unsigned* __restrict__ list,
                                                            const unsigned long long* __restrict__ count, DiagPartial* __restrict__ extra)

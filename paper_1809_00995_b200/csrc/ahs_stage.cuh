@@ -107,7 +107,7 @@ __device__ __forceinline__ void stg_vec(T* p, const Vec<T, V>& v)
     using NV = typename NativeVec<T>::type;
     NV n;
     memcpy(&n, &v, sizeof(n));
-    *reinterpret_cast<NV*>(p) = n;   // (st.global.cs measured: no difference, profiles/r3_step1024_f32_full.md)
+    *reinterpret_cast<NV*>(p) = n;   // (st.global.cs measured: no difference, profiles/HISTORY.md r3)
 }
 
 // element v+1 of a vector, or the scalar `edge` (the first element of the next vector) for the last one
@@ -142,7 +142,7 @@ struct TileGeom {
 // Issue the copies of one z-plane of NA arrays into NA consecutive array slots at `dst`.  Called by ONE thread, after
 // it has posted the expected byte count on `bar` (mbar_arrive_expect_tx).  cp.async.bulk takes its operands from
 // uniform registers, so copies issued by several lanes of a warp are serialised by a per-lane loop of ~15
-// instructions each (profiles/r1_step1024_f32_full.md: 15 % of all instructions executed); a single thread walking the rows with
+// instructions each (profiles/HISTORY.md r1: 15 % of all instructions executed); a single thread walking the rows with
 // running pointers costs a third of that.
 //   src[a]  : global base pointers of the arrays
 //   z       : plane (already wrapped into [0, N))

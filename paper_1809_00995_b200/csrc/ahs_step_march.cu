@@ -222,7 +222,7 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
     // exchange barrier once its prologue reads have been issued (the arrive travels down the same shared-memory pipe
     // behind them, release semantics) and waits for the phase to complete, so the thread that re-fills the stage at plane 1
     // has synchronised with every reader before its fence.proxy.async.  (A __syncthreads() here was not enough on sm_100:
-    // profiles/r2_race.md.)  Phase 0 of `xch` = prologue, phase it = plane it.
+    // profiles/HISTORY.md, "r2 race".)  Phase 0 of `xch` = prologue, phase it = plane it.
     mbar_arrive(xch);
     mbar_wait(xch, 0);
 
@@ -230,7 +230,7 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
 
     // The momenta (no halo) are streamed with 16-byte loads, software-pipelined by one plane: those of plane it+1 are
     // requested right after the barrier of plane it, where register pressure is lowest, and consumed at the end of phase 1
-    // of plane it+1 (profiles/r1: requested at the top of their own plane they cost 15 % of the issue slots in stalls).
+    // of plane it+1 (profiles/HISTORY.md r1: requested at the top of their own plane they cost 15 % of the issue slots in stalls).
     const size_t plane_stride = (size_t)N * N;
     size_t gnext = ((size_t)(zr.zbase + z0) * N + (size_t)(y0 + w)) * N + (size_t)(x0 + xi);
     const size_t in_plane = (size_t)(y0 + w) * N + (size_t)(x0 + xi);   // offset inside a plane: for the neighbours' ghost planes
@@ -264,7 +264,7 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
         if (C::T2_OWN) mbar_wait(&t2full[it % T2S], (it / T2S) & 1);   // theta_2 of this plane (requested NS-2 planes ago)
         // The stage of the NEXT plane is needed for the +z neighbours only.  fp32: wait for it after the trigonometry of the in-plane links (a
         // third of the plane's work later: the copy has that much longer to land; 15.3 -> 15.05 ms at 1024^3 on a 1.49 GHz board); fp64: here
-        // (measured: no gain from waiting later, profiles/r5_step1024_f32_full.md)
+        // (measured: no gain from waiting later, profiles/HISTORY.md r5)
         if constexpr (!StepShape<T>::LATE_WAIT) mbar_wait(&full[(it + 1) % NS], ((it + 1) / NS) & 1);
 
         // ---- halo products, shared out over the warps (no dedicated producer warp).  Row y0-1: one site per lane, every

@@ -4,7 +4,7 @@
 // (x, y, z, array) with byte strides (sizeof T, N sizeof T, N^2 sizeof T, array_bytes).  A box of
 // (PITCH, ROWS, 1, NA) elements of it is exactly the shared-memory layout of TileGeom (array-major, then rows of
 // PITCH elements), so cp.async.bulk.tensor.4d (SASS UTMALDG) fills a stage that took 25-30 row copies (UBLKCP) before.
-// Measured reason (profiles/r2): the copy engine serves ~35 bulk requests per microsecond and SM; with 3 CTAs x 25-90
+// Measured reason (profiles/HISTORY.md r2): the copy engine serves ~35 bulk requests per microsecond and SM; with 3 CTAs x 25-90
 // row copies per plane the marching kernels waited for their stages 30 % of the time.
 // TMA fills out-of-bounds elements with zeros, it does not wrap: tiles that touch the periodic boundary keep the
 // row-copy path of ahs_stage.cuh (1/8 of the tiles at 1024^3).

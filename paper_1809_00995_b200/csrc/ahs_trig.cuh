@@ -26,7 +26,7 @@ namespace ahs {
 // The arithmetic is written once over a lane type W: float, or float2 evaluated with Blackwell's packed fp32
 // instructions (FFMA2 / FMUL2 / FADD2 on sm_100: two IEEE fp32 operations per issued instruction, constants broadcast from
 // immediates).  Both give bit-identical results per lane; the marching kernels use the packed form on pairs of sites,
-// which takes a quarter of the instructions out of the step kernel's trigonometry (profiles/r3_step1024_f32_full.md).
+// which takes a quarter of the instructions out of the step kernel's trigonometry (profiles/HISTORY.md r3).
 namespace lanes {
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ float mul_(float a, float b) { return a * b; }

@@ -628,7 +628,7 @@ def test_repeated_diagnostics_are_bit_identical(ahs, prec, N):
 
 
 def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
-    """Regression for a shared-memory race of the marching step kernel (profiles/r2_race.md): a tensor / bulk copy
+    """Regression for a shared-memory race of the marching step kernel (profiles/HISTORY.md, "r2 race"): a tensor / bulk copy
     issued right after __syncthreads() could overwrite a stage other warps were still reading -- about one corrupted
     site per 500 launches at 512^3, visible as a Gauss-law violation of 1e-2 and as run-to-run differences.  Two runs of
     60 back-to-back launches must agree bit for bit and keep Gauss's law at fp32 roundoff."""
@@ -644,7 +644,7 @@ def test_long_window_is_deterministic_and_keeps_gauss_law(ahs):
 
 
 def test_chunk_starts_under_stress_are_bit_identical(ahs):
-    """The hand-over of the prologue's stages to the copy engine at every z-chunk start (profiles/r2_race.md): 1000 launches at
+    """The hand-over of the prologue's stages to the copy engine at every z-chunk start (profiles/HISTORY.md, "r2 race"): 1000 launches at
     256^3 with 128 chunks per tile -- a chunk start every second plane, 3.4e7 hand-overs per run, 64 x the default shape's -- in both
     staging modes.  A stage overwritten while a slower warp still reads it corrupts a site; the fields must instead equal the
     default launch shape's bit for bit (they do not depend on where the chunk boundaries fall) and Gauss's law must hold."""
