@@ -28,14 +28,20 @@ IC_RANDOM_PHASE, IC_GAUSSIAN = 0, 1
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no fast-math, no FMA contraction).  -fopenmp only marks the independent site loops
-    parallel (results do not depend on the thread count); without libgomp the pragmas are ignored: one thread."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + ".tmp.%d" % os.getpid()
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c11", "-D_GNU_SOURCE", "-o", tmp, _SRC, "-lm"]
+    parallel (results do not depend on the thread count); without libgomp the pragmas are ignored: one thread.
+    AHS_ORACLE_SANITIZE=1 builds a second library with -fsanitize=address,undefined next to the plain one (same source, same
+    arithmetic flags) and loads that instead; the process then needs the sanitizer runtimes preloaded (profiles/r7_sanitizers.md has
+    the command)."""
+    san = os.environ.get("AHS_ORACLE_SANITIZE", "") not in ("", "0")
+    out = _LIB[:-3] + "_san.so" if san else _LIB
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        tmp = out + ".tmp.%d" % os.getpid()
+        extra = ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"] if san else []
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c11", "-D_GNU_SOURCE"] + extra + ["-o", tmp, _SRC, "-lm"]
         if subprocess.call(cmd[:1] + ["-fopenmp"] + cmd[1:], stderr=subprocess.DEVNULL) != 0:
             subprocess.check_call(cmd)
-        os.replace(tmp, _LIB)
-    return _LIB
+        os.replace(tmp, out)
+    return out
 
 
 class _Params(C.Structure):
