@@ -260,6 +260,11 @@ AHS_API int32_t ahs_group_slab_count(ahs_group* group);
  * ahs_get_fields* and ahs_set_fields* on it return AHS_ERR_STATE.  NULL if r is out of range. */
 AHS_API ahs_sim* ahs_group_slab(ahs_group* group, int32_t r);
 AHS_API int32_t ahs_group_destroy(ahs_group* group);                                 /* NULL is allowed */
+/* The slab rules ahs_group_create applies, as numbers; needs no GPU (for drivers that spread slabs over processes and for the host
+ * tests).  out5 (HOST, 5 ints) = { first own global plane, own planes nz, slab below, slab above (both periodic), planes allocated
+ * = nz + 2 }: own planes sit at local indices 1 .. nz, local plane 0 mirrors the top own plane of the slab below, local plane nz + 1
+ * the bottom own plane of the slab above.  AHS_ERR_INVALID_ARG unless nslabs in 1..64 divides N and 0 <= r < nslabs. */
+AHS_API int32_t ahs_slab_layout(int32_t N, int32_t nslabs, int32_t r, int32_t* out5);
 
 /*
  * ---- diagnostics of a snapshot the caller holds, without any allocation --------------------------------------------------------

@@ -32,7 +32,7 @@ SYMBOLS = (
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
     "ahs_group_create", "ahs_group_step", "ahs_group_diagnostics", "ahs_group_get_fields_native", "ahs_group_set_fields_native",
     "ahs_group_synchronize", "ahs_group_slab_count", "ahs_group_slab", "ahs_group_destroy",
-    "ahs_diagnostics_static",
+    "ahs_diagnostics_static", "ahs_slab_layout",
 )
 AHS_STATIC_MAX_RECORDS, AHS_STATIC_MAX_N, AHS_STATIC_SCRATCH_BYTES = 4736, 2048, 96 * (4736 + 1) + 160
 
@@ -103,6 +103,7 @@ def load(path: str | None = None):
     lib.ahs_group_slab_count.argtypes = [vp]; lib.ahs_group_slab_count.restype = i32
     lib.ahs_group_slab.argtypes = [vp, i32]; lib.ahs_group_slab.restype = vp
     lib.ahs_group_destroy.argtypes = [vp]; lib.ahs_group_destroy.restype = i32
+    lib.ahs_slab_layout.argtypes = [i32, i32, i32, C.POINTER(i32)]; lib.ahs_slab_layout.restype = i32
     lib.ahs_diagnostics_static.argtypes = [C.POINTER(ahs_params), C.POINTER(vp), i64, C.POINTER(ahs_diag)]; lib.ahs_diagnostics_static.restype = i32
     _lib = lib
     return lib
@@ -379,6 +380,13 @@ class Group:
             _check(lib.ahs_get_state(C.c_void_p(lib.ahs_group_slab(self._g, r)), None, None, C.byref(nl)))
             tot += nl.value
         return tot
+
+
+def slab_layout(N: int, nslabs: int, r: int) -> tuple:
+    """ahs_slab_layout: (z_offset, nz, lo, hi, nz_alloc) of slab r -- the library's own slab rules; needs no GPU."""
+    out = (C.c_int32 * 5)()
+    _check(load().ahs_slab_layout(int(N), int(nslabs), int(r), out))
+    return tuple(out)
 
 
 def diagnostics_static(fields10, N, step, precision="f32", dx=0.5, dt=0.1, lambda0=2.0, e0=1.0, sigma=1.0, m=1.0, s=0.0, tau0=1.0,

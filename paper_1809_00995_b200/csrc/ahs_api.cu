@@ -628,8 +628,19 @@ struct ahs_group {
 
 namespace {
 
-int lo_of(const ahs_group* g, int r) { return (r + g->P - 1) % g->P; }
-int hi_of(const ahs_group* g, int r) { return (r + 1) % g->P; }
+// THE slab rules (ahs_slab_layout exports them; slabs.py and the multi-process host tests read them from there): slab r of P owns the
+// global planes [r N/P, (r+1) N/P) at its local planes 1 .. N/P, between a ghost plane below (local 0: the top own plane of slab r-1,
+// periodically) and above (local N/P + 1: the bottom own plane of slab r+1).
+struct SlabLayout { int z_offset, nz, lo, hi, nz_alloc; };
+bool slab_layout(int N, int P, int r, SlabLayout* out)
+{
+    if (!valid_N(N) || P < 1 || P > 64 || N % P != 0 || r < 0 || r >= P) return false;
+    const int nz = N / P;
+    *out = SlabLayout{ r * nz, nz, (r + P - 1) % P, (r + 1) % P, nz + 2 };
+    return true;
+}
+int lo_of(const ahs_group* g, int r) { SlabLayout l{}; slab_layout(g->p.N, g->P, r, &l); return l.lo; }
+int hi_of(const ahs_group* g, int r) { SlabLayout l{}; slab_layout(g->p.N, g->P, r, &l); return l.hi; }
 
 char* plane_ptr(const ahs_sim* s, int slot_index, int local_plane)
 {
@@ -714,14 +725,15 @@ ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int3
     g->p = *params; g->P = nslabs; g->parity = 0; g->have_prev = false; g->step = 0; g->poisoned = false;
     g->slab.assign(nslabs, nullptr);
     g->done[0].assign(nslabs, nullptr); g->done[1].assign(nslabs, nullptr);
-    const int nz = params->N / nslabs;
     for (int r = 0; r < nslabs; ++r) {
         const int dev = devices ? devices[r] : home;
         if (dev < 0 || dev >= ndev) { fail(AHS_ERR_INVALID_ARG, "device %d of slab %d does not exist (%d devices)", dev, r, ndev); ahs_group_destroy(g); return nullptr; }
         DeviceGuard guard(dev);
         ahs_params p = *params;
         p.kernel = AHS_KERNEL_MARCH;
-        SlabSpec spec = { nz, r * nz };
+        SlabLayout lay{};
+        slab_layout(params->N, nslabs, r, &lay);
+        SlabSpec spec = { lay.nz, lay.z_offset };
         g->slab[r] = create_sim(&p, &spec);
         if (!g->slab[r]) { ahs_group_destroy(g); return nullptr; }
         for (int k = 0; k < 2; ++k)
@@ -881,6 +893,15 @@ int32_t ahs_group_synchronize(ahs_group* g)
 {
     if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
     return group_sync(g);
+}
+
+int32_t ahs_slab_layout(int32_t N, int32_t nslabs, int32_t r, int32_t* out5)
+{
+    SlabLayout l{};
+    if (!out5) return fail(AHS_ERR_INVALID_ARG, "out5 is NULL");
+    if (!slab_layout(N, nslabs, r, &l)) return fail(AHS_ERR_INVALID_ARG, "nslabs must be in 1..64 and divide N (4..2048), and 0 <= r < nslabs");
+    out5[0] = l.z_offset; out5[1] = l.nz; out5[2] = l.lo; out5[3] = l.hi; out5[4] = l.nz_alloc;
+    return AHS_OK;
 }
 
 int32_t ahs_group_slab_count(ahs_group* g) { return g ? g->P : fail(AHS_ERR_INVALID_ARG, "null group"); }

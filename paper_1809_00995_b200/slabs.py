@@ -1,7 +1,8 @@
 """z-slab bookkeeping of an ahs_group: which planes a slab owns, who its neighbours are, and
 which plane of which slab feeds which ghost plane after every step.
 
-Index arithmetic only -- the same rules `ahs_group_create` wires into the step kernel's peer stores (csrc/ahs_api.cu): slab r of P
+The rules themselves live in ONE place, csrc/ahs_api.cu (`slab_layout`, which `ahs_group_create` wires into the step kernel's peer
+stores); `layout` below reads them through the C ABI (`ahs_slab_layout`, no GPU needed) and only wraps them in records: slab r of P
 owns the global planes [r N/P, (r+1) N/P) at its local planes 1 .. N/P; local plane 0 is the ghost below (the top own plane of slab
 r-1, periodically), local plane N/P + 1 the ghost above (the bottom own plane of slab r+1).  `binding.Group.layout` returns these
 records; a driver that spreads the slabs over several processes (one rank per GPU) uses `owner` and `exchange_plan` to know which
@@ -26,10 +27,7 @@ class Slab:
     nz: int            # own planes
     lo: int            # slab below (periodic)
     hi: int            # slab above (periodic)
-
-    @property
-    def nz_alloc(self) -> int:
-        return self.nz + 2
+    nz_alloc: int      # planes allocated per array: own planes at local 1 .. nz between the two ghost planes
 
     def local_plane(self, z_global: int) -> int:
         """Local index of an own global plane."""
@@ -44,10 +42,11 @@ class Slab:
 
 
 def layout(N: int, nslabs: int) -> list:
-    if nslabs < 1 or N % nslabs != 0:
-        raise ValueError("nslabs must divide N")
-    nz = N // nslabs
-    return [Slab(r, nslabs, N, r * nz, nz, (r - 1) % nslabs, (r + 1) % nslabs) for r in range(nslabs)]
+    from . import binding
+    try:
+        return [Slab(r, nslabs, N, *binding.slab_layout(N, nslabs, r)) for r in range(max(nslabs, 1))]
+    except binding.AhsError as e:
+        raise ValueError(str(e))
 
 
 def exchange_plan(N: int, nslabs: int) -> list:
