@@ -205,8 +205,10 @@ def workload_config(args) -> dict:
                         % (N, args.precision, args.m, args.s, SEED, args.leapfrog, name, ", tau_ref=%g" % args.tau_ref if args.tau_ref else ""),
             "lattice": N, "leapfrog_per_step": args.leapfrog, "diagnostics_per_step": 1,
             "l2": "inputs larger than L2 (%.1f GB of fields streamed per leapfrog launch)" % (N ** 3 * BYTES_PER_SITE[args.precision] / 1e9),
-            "parallelism": "replicas x%d" % args.gpus + (", each lattice cut into %d z-slabs on devices [%s]" % (args.slabs, args.slab_devices or "this rank's GPU")
-                                                          if args.slabs else "")}
+            "parallelism": ("z-slabs x%d on devices [%s] of one process (one lattice, exchange inside the step kernel)" % (args.slabs, args.slab_devices)
+                            if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) == 1 and args.slabs else
+                            "replicas x%d" % args.gpus + (", each lattice cut into %d z-slabs on devices [%s]" % (args.slabs, args.slab_devices or "this rank's GPU")
+                                                          if args.slabs else ""))}
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -262,6 +264,16 @@ def run_ours(args):
 
     N, L, K, W = args.lattice, args.leapfrog, args.steps, args.warmup
     sites = N ** 3
+    # ONE process asked for several GPUs (no torchrun: WORLD_SIZE unset): the lattice is cut into z-slabs over them (ahs_group,
+    # DESIGN.md 10) -- total work fixed, "strong" scaling.  Under torchrun every rank keeps a whole lattice of its own (replicas).
+    strong = world == 1 and args.gpus > 1
+    if strong:
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit("bench.py --gpus %d in one process cuts the lattice into z-slabs over %d GPUs, but this box has %d; "
+                             "launch it with torchrun for independent replicas" % (args.gpus, args.gpus, torch.cuda.device_count()))
+        args.slabs = args.slabs or args.gpus
+        if not args.slab_devices:
+            args.slab_devices = ",".join(str(i * args.gpus // args.slabs) for i in range(args.slabs))   # contiguous blocks of slabs per GPU
     if args.slabs:
         devs = [int(d) for d in args.slab_devices.split(",")] if args.slab_devices else [local] * args.slabs
         sim = ahs.Group(N=N, nslabs=args.slabs, devices=devs, precision=args.precision, m=args.m, s=args.s, seed=SEED + rank,
@@ -297,10 +309,15 @@ def run_ours(args):
     t1 = time.time()
     clk = clocks.stop(t0, t1)
     launches = sim.kernel_launches - launches0
+    per_device = None
+    if args.slabs:
+        per_device = {}
+        for d, n in zip(devs, sim.launches_per_slab()):
+            per_device[str(d)] = per_device.get(str(d), 0) + int(n)     # (since creation: IC and warm-up launches included)
     total_ms = max_ranks(start.elapsed_time(stop))
     step_ms = sum(a.elapsed_time(b) for a, b, _ in marks)       # the leapfrog launches only
     diag_ms = sum(b.elapsed_time(c) for _, b, c in marks)
-    value = whole_job_value(world, sites, L, K, total_ms)
+    value = whole_job_value(world, sites, L, K, total_ms)       # (z-slabs in one process: world = 1, ONE lattice on args.gpus GPUs)
 
     launch_s = step_ms * 1e-3 / (K * L)
     peak, peak_src = measured_peak()
@@ -320,8 +337,8 @@ def run_ours(args):
         e2e = run_e2e(args, sim, torch, max_ranks, barrier, world)
 
     line = {
-        "metric": "lattice site-updates/sec per leapfrog step", "value": value, "unit": "site-updates/s", "n_gpus": world,
-        "steps": K, "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+        "metric": "lattice site-updates/sec per leapfrog step", "value": value, "unit": "site-updates/s", "n_gpus": args.gpus if strong else world,
+        "steps": K, "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "strong" if strong else "weak",
         "vs_baseline": None, "dtype": args.precision, "data": "synthetic", "config": workload_config(args),
         "roofline": roofline, "clocks": clk, "gpu_launches": int(launches),
         "ms_per_leapfrog_step": launch_s * 1e3, "step_only_site_updates_per_s": sites / launch_s,
@@ -330,6 +347,9 @@ def run_ours(args):
     }
     if e2e is not None:
         line["e2e"] = e2e
+    if per_device is not None:
+        line["gpu_launches_per_device_since_create"] = per_device
+        line["slab_faces_by_copies"] = sim.copied_faces
     sim.destroy()
     default_workload = (N, args.precision, L, args.m, args.s, args.kernel, args.slabs) == (1024, "f32", 50, 1.0, 0.0, "auto", 0)
     if rank == 0 and world == 1 and default_workload and not args.no_other_configs:

@@ -61,6 +61,7 @@ enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
 enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2, AHS_OPT_DIAG_TRIG = 3 };   /* ahs_set_option */
 enum { AHS_STAGING_TENSOR = 0, AHS_STAGING_ROWS = 1 };
 enum { AHS_TRIG_HARDWARE = 0, AHS_TRIG_POLYNOMIAL = 1 };
+enum { AHS_EXCHANGE_STORES = 0, AHS_EXCHANGE_COPIES = 1 };           /* ahs_group_set_exchange */
 
 /*
  * Parameters of a simulation (L36: lambda, e, sigma; L51: dx, dt; L68-70: s; L224: a ~ eta^m; L72: IC).
@@ -239,8 +240,9 @@ AHS_API int32_t ahs_destroy(ahs_sim* sim);
  * step.  CUDA events order step n+1 of a slab behind step n of its two neighbours; nothing waits on the device.  Results are those
  * of a single handle: fields bit for bit, counts exactly, sums to the rounding order of the final reduction.
  * params: as for ahs_create_ex with device_buffer = stream = NULL and N % 128 == 0 (fp32) / N % 64 == 0 (fp64); nslabs in 1..64
- * must divide N, and a slab holds at most 2047 planes (N = 2048 needs nslabs >= 2).  Slabs on different devices need peer access
- * between neighbours.  One host thread drives a group.
+ * must divide N, and a slab holds at most 2047 planes (N = 2048 needs nslabs >= 2).  Neighbouring slabs on two GPUs without peer
+ * access to one another exchange that face by cudaMemcpyPeerAsync behind the step instead (5 + 5 + 1 plane copies per slab and step,
+ * same values; see ahs_group_set_exchange).  One host thread drives a group.
  */
 typedef struct ahs_group ahs_group;
 AHS_API ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int32_t* devices /* HOST, may be NULL */);
@@ -254,6 +256,12 @@ AHS_API int32_t ahs_group_diagnostics(ahs_group* group, ahs_diag* out /* HOST */
 AHS_API int32_t ahs_group_get_fields_native(ahs_group* group, void* host10);
 AHS_API int32_t ahs_group_set_fields_native(ahs_group* group, const void* host10, int64_t step);
 AHS_API int32_t ahs_group_synchronize(ahs_group* group);
+/* How the faces travel.  AHS_EXCHANGE_STORES (default): the step kernel's own stores into the neighbours' ghost planes wherever the two
+ * GPUs have peer access (always on one GPU), copies elsewhere.  AHS_EXCHANGE_COPIES: every face by cudaMemcpyPeerAsync behind the step
+ * (what a pair of GPUs without peer access gets anyway; selectable so that this path can be exercised and timed on any box).  The
+ * fields are the same bit for bit.  Synchronises the group.  ahs_group_exchange_faces: how many of the 2 nslabs faces go by copies. */
+AHS_API int32_t ahs_group_set_exchange(ahs_group* group, int32_t mode);
+AHS_API int32_t ahs_group_exchange_faces(ahs_group* group, int32_t* copied_faces /* HOST */);
 AHS_API int32_t ahs_group_slab_count(ahs_group* group);
 /* The handle of slab r (owned by the group: for ahs_set_option, ahs_set_s_schedule, ahs_get_state, ahs_kernel_kind, ahs_coefficients,
  * ahs_synchronize).  It is stepped, measured and its fields are read and written through the group only: ahs_step, ahs_diagnostics*,

@@ -21,6 +21,7 @@ AHS_KERNEL_AUTO, AHS_KERNEL_GENERIC, AHS_KERNEL_MARCH = 0, 1, 2
 AHS_OPT_STAGING, AHS_OPT_STEP_CHUNKS, AHS_OPT_DIAG_CHUNKS, AHS_OPT_DIAG_TRIG = 0, 1, 2, 3
 AHS_STAGING_TENSOR, AHS_STAGING_ROWS = 0, 1
 AHS_TRIG_HARDWARE, AHS_TRIG_POLYNOMIAL = 0, 1
+AHS_EXCHANGE_STORES, AHS_EXCHANGE_COPIES = 0, 1
 
 FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "theta_0", "theta_1", "theta_2", "eps_0", "eps_1", "eps_2")
 
@@ -32,7 +33,7 @@ SYMBOLS = (
     "ahs_synchronize", "ahs_destroy", "ahs_last_error", "ahs_version",
     "ahs_group_create", "ahs_group_step", "ahs_group_diagnostics", "ahs_group_get_fields_native", "ahs_group_set_fields_native",
     "ahs_group_synchronize", "ahs_group_slab_count", "ahs_group_slab", "ahs_group_destroy",
-    "ahs_diagnostics_static", "ahs_slab_layout",
+    "ahs_diagnostics_static", "ahs_slab_layout", "ahs_group_set_exchange", "ahs_group_exchange_faces",
 )
 AHS_STATIC_MAX_RECORDS, AHS_STATIC_MAX_N, AHS_STATIC_SCRATCH_BYTES = 4736, 2048, 96 * (4736 + 1) + 160
 
@@ -103,6 +104,8 @@ def load(path: str | None = None):
     lib.ahs_group_slab_count.argtypes = [vp]; lib.ahs_group_slab_count.restype = i32
     lib.ahs_group_slab.argtypes = [vp, i32]; lib.ahs_group_slab.restype = vp
     lib.ahs_group_destroy.argtypes = [vp]; lib.ahs_group_destroy.restype = i32
+    lib.ahs_group_set_exchange.argtypes = [vp, i32]; lib.ahs_group_set_exchange.restype = i32
+    lib.ahs_group_exchange_faces.argtypes = [vp, C.POINTER(i32)]; lib.ahs_group_exchange_faces.restype = i32
     lib.ahs_slab_layout.argtypes = [i32, i32, i32, C.POINTER(i32)]; lib.ahs_slab_layout.restype = i32
     lib.ahs_diagnostics_static.argtypes = [C.POINTER(ahs_params), C.POINTER(vp), i64, C.POINTER(ahs_diag)]; lib.ahs_diagnostics_static.restype = i32
     _lib = lib
@@ -353,6 +356,24 @@ class Group:
 
     def synchronize(self):
         _check(load().ahs_group_synchronize(self._g))
+
+    def set_exchange(self, mode: int):
+        """ahs_group_set_exchange: AHS_EXCHANGE_STORES (the step kernel's stores where the GPUs have peer access) or AHS_EXCHANGE_COPIES."""
+        _check(load().ahs_group_set_exchange(self._g, int(mode)))
+
+    @property
+    def copied_faces(self) -> int:
+        n = C.c_int32()
+        _check(load().ahs_group_exchange_faces(self._g, C.byref(n)))
+        return n.value
+
+    def launches_per_slab(self) -> list:
+        lib, out = load(), []
+        for r in range(lib.ahs_group_slab_count(self._g)):
+            nl = C.c_int64()
+            _check(lib.ahs_get_state(C.c_void_p(lib.ahs_group_slab(self._g, r)), None, None, C.byref(nl)))
+            out.append(nl.value)
+        return out
 
     @property
     def layout(self):

@@ -43,6 +43,13 @@ struct ahs_sim {
     void* ghost_lo[2][5];
     void* ghost_hi[2][5];
     void* ghost_eps2_hi;
+    // A face the step kernel may NOT store through (no peer access between the two GPUs, or ahs_group_set_exchange asked for copies):
+    // its ghost_* pointers above stay NULL and the same planes travel by cudaMemcpyPeerAsync behind the step, to these targets
+    bool copy_lo, copy_hi;
+    void* copy_lo_dst[2][5];
+    void* copy_hi_dst[2][5];
+    void* copy_eps2_dst;
+    int lo_device, hi_device;
     // time-dependent s(tau) of Eq. 8 (ahs_set_s_schedule; R23): knots, empty = the constant p.s
     std::vector<double> sched_tau, sched_s;
 };
@@ -306,6 +313,11 @@ ahs_sim* create_sim(const ahs_params* params, const SlabSpec* slab)
     std::memset(s->ghost_lo, 0, sizeof(s->ghost_lo));
     std::memset(s->ghost_hi, 0, sizeof(s->ghost_hi));
     s->ghost_eps2_hi = nullptr;
+    s->copy_lo = s->copy_hi = false;
+    std::memset(s->copy_lo_dst, 0, sizeof(s->copy_lo_dst));
+    std::memset(s->copy_hi_dst, 0, sizeof(s->copy_hi_dst));
+    s->copy_eps2_dst = nullptr;
+    s->lo_device = s->hi_device = -1;
     if (slab) {
         if (!march_ok || p.device_buffer) { fail(AHS_ERR_INVALID_ARG, "a z-slab needs the z-marching kernels (N %% %d == 0) and library-owned memory", p.precision == AHS_F32 ? 128 : 64); delete s; return nullptr; }
         if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) { fail(AHS_ERR_CUDA, "cudaStreamCreate: %s", cudaGetErrorString(cudaGetLastError())); delete s; return nullptr; }
@@ -623,6 +635,7 @@ struct ahs_group {
     int parity;                         // parity of the NEXT step's events
     bool have_prev;
     int64_t step;
+    std::vector<char> no_peer_lo, no_peer_hi;   // slab r cannot reach the GPU of the slab below / above: that face always goes by copies
     bool poisoned;                      // a step failed after some slabs had already run it: fields inconsistent until they are set again
 };
 
@@ -639,6 +652,7 @@ bool slab_layout(int N, int P, int r, SlabLayout* out)
     *out = SlabLayout{ r * nz, nz, (r + P - 1) % P, (r + 1) % P, nz + 2 };
     return true;
 }
+void wire_faces(ahs_group* g, bool copies);   // defined with the step, below
 int lo_of(const ahs_group* g, int r) { SlabLayout l{}; slab_layout(g->p.N, g->P, r, &l); return l.lo; }
 int hi_of(const ahs_group* g, int r) { SlabLayout l{}; slab_layout(g->p.N, g->P, r, &l); return l.hi; }
 
@@ -741,40 +755,75 @@ ahs_group* ahs_group_create(const ahs_params* params, int32_t nslabs, const int3
                 fail(AHS_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(cudaGetLastError())); ahs_group_destroy(g); return nullptr;
             }
     }
-    // peer access between neighbouring slabs on different devices, then the ghost targets of every slab
+    // peer access between neighbouring slabs on different devices (a pair without it exchanges by copies), then every slab's targets
+    g->no_peer_lo.assign(nslabs, 0); g->no_peer_hi.assign(nslabs, 0);
     for (int r = 0; r < nslabs; ++r)
-        for (int nb : { lo_of(g, r), hi_of(g, r) }) {
+        for (int side = 0; side < 2; ++side) {
+            const int nb = side ? hi_of(g, r) : lo_of(g, r);
             const int a = g->slab[r]->device, b = g->slab[nb]->device;
             if (a == b) continue;
             int can = 0;
             DeviceGuard guard(a);
             if (cudaDeviceCanAccessPeer(&can, a, b) != cudaSuccess || !can) {
                 cudaGetLastError();
-                fail(AHS_ERR_CUDA, "device %d cannot access device %d: slabs on different GPUs need peer access (NVLink / NVSwitch)", a, b);
-                ahs_group_destroy(g); return nullptr;
+                (side ? g->no_peer_hi : g->no_peer_lo)[r] = 1;
+                continue;
             }
             const cudaError_t e = cudaDeviceEnablePeerAccess(b, 0);
             if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) { fail(AHS_ERR_CUDA, "cudaDeviceEnablePeerAccess: %s", cudaGetErrorString(e)); ahs_group_destroy(g); return nullptr; }
             cudaGetLastError();
         }
-    for (int r = 0; r < nslabs; ++r) {
-        ahs_sim* s = g->slab[r];
-        const ahs_sim* lo = g->slab[lo_of(g, r)];
-        const ahs_sim* hi = g->slab[hi_of(g, r)];
-        for (int ob = 0; ob < 2; ++ob) {
-            const int b = ob ? PHI_RE1 : PHI_RE0;
-            for (int i = 0; i < 5; ++i) {
-                s->ghost_lo[ob][i] = plane_ptr(lo, b + i, lo->zr.nz + 1);   // my bottom plane is the lower neighbour's ghost above
-                s->ghost_hi[ob][i] = plane_ptr(hi, b + i, 0);               // my top plane is the upper neighbour's ghost below
-            }
-        }
-        s->ghost_eps2_hi = plane_ptr(hi, EPS2, 0);
-    }
+    wire_faces(g, false);
     if (group_sync(g) != AHS_OK) { ahs_group_destroy(g); return nullptr; }
     return g;
 }
 
 namespace {
+
+// Where each slab's boundary planes go.  A face takes the step kernel's own stores into the neighbour's ghost planes (peer memory
+// when the neighbour lives on another GPU) unless the two GPUs have no peer access or `copies` is set; then the kernel gets no
+// pointer for that face and step_slab sends the same planes with cudaMemcpyPeerAsync (which needs no peer access: the driver
+// stages through the host if it must).  Same values either way: the fields do not depend on the mode.
+void wire_faces(ahs_group* g, bool copies)
+{
+    for (int r = 0; r < g->P; ++r) {
+        ahs_sim* s = g->slab[r];
+        const ahs_sim* lo = g->slab[lo_of(g, r)];
+        const ahs_sim* hi = g->slab[hi_of(g, r)];
+        s->copy_lo = copies || g->no_peer_lo[r];
+        s->copy_hi = copies || g->no_peer_hi[r];
+        s->lo_device = lo->device;
+        s->hi_device = hi->device;
+        for (int ob = 0; ob < 2; ++ob) {
+            const int b = ob ? PHI_RE1 : PHI_RE0;
+            for (int i = 0; i < 5; ++i) {
+                void* to_lo = plane_ptr(lo, b + i, lo->zr.nz + 1);   // my bottom plane is the lower neighbour's ghost above
+                void* to_hi = plane_ptr(hi, b + i, 0);               // my top plane is the upper neighbour's ghost below
+                s->ghost_lo[ob][i] = s->copy_lo ? nullptr : to_lo;
+                s->ghost_hi[ob][i] = s->copy_hi ? nullptr : to_hi;
+                s->copy_lo_dst[ob][i] = s->copy_lo ? to_lo : nullptr;
+                s->copy_hi_dst[ob][i] = s->copy_hi ? to_hi : nullptr;
+            }
+        }
+        void* eps2_to_hi = plane_ptr(hi, EPS2, 0);
+        s->ghost_eps2_hi = s->copy_hi ? nullptr : eps2_to_hi;
+        s->copy_eps2_dst = s->copy_hi ? eps2_to_hi : nullptr;
+    }
+}
+
+// the faces that go by copies: the new (phi, theta) of the bottom / top own plane (and eps_2 of the top plane) of the buffer the step
+// just wrote, enqueued on the slab's stream behind the step kernel and in front of the event its neighbours wait for
+int copy_faces(ahs_sim* s, int out_buffer)
+{
+    const size_t plane = (size_t)s->p.N * s->p.N * s->elem;
+    const int b = out_buffer ? PHI_RE1 : PHI_RE0;
+    for (int i = 0; i < 5; ++i) {
+        if (s->copy_lo) AHS_CUDA(cudaMemcpyPeerAsync(s->copy_lo_dst[out_buffer][i], s->lo_device, plane_ptr(s, b + i, 1), s->device, plane, s->stream));
+        if (s->copy_hi) AHS_CUDA(cudaMemcpyPeerAsync(s->copy_hi_dst[out_buffer][i], s->hi_device, plane_ptr(s, b + i, s->zr.nz), s->device, plane, s->stream));
+    }
+    if (s->copy_hi) AHS_CUDA(cudaMemcpyPeerAsync(s->copy_eps2_dst, s->hi_device, plane_ptr(s, EPS2, s->zr.nz), s->device, plane, s->stream));
+    return AHS_OK;
+}
 
 const char kPoisoned[] = "an earlier ahs_group_step failed part-way through a step: the slabs' fields are inconsistent until ahs_group_set_fields_native sets them again";
 
@@ -788,6 +837,8 @@ int step_slab(ahs_group* g, int r)
     const int rc = s->p.precision == AHS_F32 ? do_step<float>(s) : do_step<double>(s);
     if (rc < 0) return fail(rc, "step kernel launch failed on slab %d at step %lld: %s", r, (long long)s->step, cudaGetErrorString(cudaGetLastError()));
     s->launches += rc;
+    if (s->copy_lo || s->copy_hi)
+        if (int e = copy_faces(s, s->cur ^ 1)) return e;
     AHS_CUDA(cudaEventRecord(g->done[g->parity][r], s->stream));
     return AHS_OK;
 }
@@ -893,6 +944,24 @@ int32_t ahs_group_synchronize(ahs_group* g)
 {
     if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
     return group_sync(g);
+}
+
+int32_t ahs_group_set_exchange(ahs_group* g, int32_t mode)
+{
+    if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
+    if (mode != AHS_EXCHANGE_STORES && mode != AHS_EXCHANGE_COPIES) return fail(AHS_ERR_INVALID_ARG, "mode must be AHS_EXCHANGE_STORES or AHS_EXCHANGE_COPIES");
+    if (int r = group_sync(g)) return r;      // no step in flight while the targets change
+    wire_faces(g, mode == AHS_EXCHANGE_COPIES);
+    return AHS_OK;
+}
+
+int32_t ahs_group_exchange_faces(ahs_group* g, int32_t* copied_faces)
+{
+    if (!g) return fail(AHS_ERR_INVALID_ARG, "null group");
+    int n = 0;
+    for (const ahs_sim* s : g->slab) n += (s->copy_lo ? 1 : 0) + (s->copy_hi ? 1 : 0);
+    if (copied_faces) *copied_faces = n;
+    return AHS_OK;
 }
 
 int32_t ahs_slab_layout(int32_t N, int32_t nslabs, int32_t r, int32_t* out5)

@@ -911,6 +911,30 @@ def test_slab_handles_are_driven_through_their_group(ahs):
     assert "at least 2 slabs" in str(e.value)
 
 
+@pytest.mark.parametrize("prec,N,P", [("f32", 256, 4), ("f64", 128, 2)])
+def test_slab_group_exchange_by_copies_is_bit_identical(ahs, prec, N, P):
+    """AHS_EXCHANGE_COPIES -- what two GPUs without peer access to one another get: the faces travel by cudaMemcpyPeerAsync behind the
+    step instead of the kernel's own stores.  Same bar: the single lattice bit for bit, also when the mode changes in mid-run."""
+    with ahs.Simulation(N=N, precision=prec, m=1.0, s=0.0, seed=21) as ref, ahs.Group(N=N, nslabs=P, precision=prec, m=1.0, s=0.0, seed=21) as g:
+        assert g.copied_faces == 0                                   # one GPU: every face by the kernel's stores
+        g.set_exchange(ahs.AHS_EXCHANGE_COPIES)
+        assert g.copied_faces == 2 * P
+        ref.step(7)
+        g.step(4)
+        d4 = g.diagnostics()
+        g.step(3)
+        assert d4["step"] == 4 and np.array_equal(g.get_fields_native(), ref.get_fields_native())
+        g.set_exchange(ahs.AHS_EXCHANGE_STORES)
+        assert g.copied_faces == 0
+        ref.step(5)
+        g.step(5)
+        assert np.array_equal(g.get_fields_native(), ref.get_fields_native())
+        d, dref = g.diagnostics(), ref.diagnostics()
+        assert (d["n_pierced"], d["sum_abs_w"], d["gauss_max"]) == (dref["n_pierced"], dref["sum_abs_w"], dref["gauss_max"])
+        with pytest.raises(ahs.AhsError):
+            g.set_exchange(2)
+
+
 def _device_count():
     import torch
     return torch.cuda.device_count()
@@ -931,6 +955,8 @@ def test_slab_group_on_several_devices_bit_for_bit(ahs):
         if N % P:
             continue
         with ahs.Group(N=N, nslabs=P, devices=devices, precision="f32", m=1.0, s=0.0, seed=77) as g:
+            if P == 4:
+                g.set_exchange(ahs.AHS_EXCHANGE_COPIES)             # the path of GPUs without peer access, across real devices
             g.step(5)
             d5 = g.diagnostics()
             g.step(nsteps - 5)
