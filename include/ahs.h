@@ -58,7 +58,7 @@ enum { AHS_OK = 0, AHS_ERR_INVALID_ARG = -1, AHS_ERR_OOM = -2, AHS_ERR_CUDA = -3
 enum { AHS_F32 = 0, AHS_F64 = 1 };                                   /* storage AND arithmetic type of the step */
 enum { AHS_IC_RANDOM_PHASE = 0, AHS_IC_GAUSSIAN = 1, AHS_IC_NONE = 2 /* all fields zero; set them with ahs_set_fields */ };
 enum { AHS_KERNEL_AUTO = 0, AHS_KERNEL_GENERIC = 1, AHS_KERNEL_MARCH = 2 };
-enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2, AHS_OPT_DIAG_TRIG = 3 };   /* ahs_set_option */
+enum { AHS_OPT_STAGING = 0, AHS_OPT_STEP_CHUNKS = 1, AHS_OPT_DIAG_CHUNKS = 2, AHS_OPT_DIAG_TRIG = 3, AHS_OPT_STEP_PDL = 4 };   /* ahs_set_option */
 enum { AHS_STAGING_TENSOR = 0, AHS_STAGING_ROWS = 1 };
 enum { AHS_TRIG_HARDWARE = 0, AHS_TRIG_POLYNOMIAL = 1 };
 enum { AHS_EXCHANGE_STORES = 0, AHS_EXCHANGE_COPIES = 1 };           /* ahs_group_set_exchange */
@@ -209,6 +209,10 @@ AHS_API int32_t ahs_kernel_kind(ahs_sim* sim);
  *                        DESIGN.md section 8) instead of ~1e-8;
  *                        AHS_TRIG_POLYNOMIAL: the 1-2 ulp routines the step kernel uses (the call takes ~17 % longer).
  *                        The winding (Eq. 11) and the Gauss residual do not depend on it; fp64 lattices always take the polynomials.
+ *   AHS_OPT_STEP_PDL     1: the step march is launched with programmatic stream serialization -- the CTAs of step n + 1 may take the SM
+ *                        slots that step n's last wave leaves free and run their set-up (barrier initialisation) there; they wait for
+ *                        step n to complete before they touch global memory, so the fields are the same bit for bit.  0 (default): plain
+ *                        stream order.  Matters for small lattices, where a launch lasts a fraction of a millisecond.
  * Returns AHS_ERR_INVALID_ARG for an unknown option or a value out of range. */
 AHS_API int32_t ahs_set_option(ahs_sim* sim, int32_t option, int32_t value);
 

@@ -18,7 +18,7 @@ AHS_OK, AHS_ERR_INVALID_ARG, AHS_ERR_OOM, AHS_ERR_CUDA, AHS_ERR_NONFINITE, AHS_E
 AHS_F32, AHS_F64 = 0, 1
 AHS_IC_RANDOM_PHASE, AHS_IC_GAUSSIAN, AHS_IC_NONE = 0, 1, 2
 AHS_KERNEL_AUTO, AHS_KERNEL_GENERIC, AHS_KERNEL_MARCH = 0, 1, 2
-AHS_OPT_STAGING, AHS_OPT_STEP_CHUNKS, AHS_OPT_DIAG_CHUNKS, AHS_OPT_DIAG_TRIG = 0, 1, 2, 3
+AHS_OPT_STAGING, AHS_OPT_STEP_CHUNKS, AHS_OPT_DIAG_CHUNKS, AHS_OPT_DIAG_TRIG, AHS_OPT_STEP_PDL = 0, 1, 2, 3, 4
 AHS_STAGING_TENSOR, AHS_STAGING_ROWS = 0, 1
 AHS_TRIG_HARDWARE, AHS_TRIG_POLYNOMIAL = 0, 1
 AHS_EXCHANGE_STORES, AHS_EXCHANGE_COPIES = 0, 1

@@ -326,7 +326,7 @@ ahs_sim* create_sim(const ahs_params* params, const SlabSpec* slab)
     s->cur = 0; s->step = 0; s->launches = 0; s->diag_step = -1; s->device = dev;
     s->kernel = (p.kernel == AHS_KERNEL_AUTO) ? (march_ok ? AHS_KERNEL_MARCH : AHS_KERNEL_GENERIC) : p.kernel;
     s->result_host = nullptr;
-    s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0, AHS_TRIG_HARDWARE };
+    s->opt = MarchOptions{ AHS_STAGING_TENSOR, 0, 0, AHS_TRIG_HARDWARE, 0 };
 
     const size_t need = (size_t)NUM_SLOTS * s->array_bytes + scratch_bytes();
     if (p.device_buffer) {
@@ -589,6 +589,10 @@ int32_t ahs_set_option(ahs_sim* s, int32_t option, int32_t value)
         case AHS_OPT_DIAG_TRIG:
             if (value != AHS_TRIG_HARDWARE && value != AHS_TRIG_POLYNOMIAL) return fail(AHS_ERR_INVALID_ARG, "AHS_OPT_DIAG_TRIG takes AHS_TRIG_HARDWARE or AHS_TRIG_POLYNOMIAL");
             s->opt.diag_trig = value;
+            return AHS_OK;
+        case AHS_OPT_STEP_PDL:
+            if (value > 1) return fail(AHS_ERR_INVALID_ARG, "AHS_OPT_STEP_PDL takes 0 or 1");
+            s->opt.step_pdl = value;
             return AHS_OK;
         default:
             return fail(AHS_ERR_INVALID_ARG, "unknown option %d", option);

@@ -91,6 +91,7 @@ struct MarchOptions {
     int step_chunks;   // z-chunks per tile of the step march
     int diag_chunks;   // z-chunks per tile of the diagnostics march
     int diag_trig;     // AHS_TRIG_HARDWARE or AHS_TRIG_POLYNOMIAL: the sines and cosines of the <v^2> sums (fp32 lattices)
+    int step_pdl;      // launch the step march with programmatic stream serialization (its prologue overlaps the previous kernel's tail)
 };
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is per device: set it once on every device a kernel is launched on

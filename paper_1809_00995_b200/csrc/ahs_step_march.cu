@@ -134,6 +134,13 @@ step_march_kernel(FieldPtrs<T> f, GhostPtrs<T> gh, int N, ZRange zr, int nchunks
         mbar_fence_init();
     }
     __syncthreads();
+    // Programmatic dependent launch (AHS_OPT_STEP_PDL): everything above -- the CTA's index arithmetic and barrier initialisation -- may
+    // run while the previous kernel of the stream is still draining its last wave.  From here on the kernel touches global memory
+    // (the previous step's output is this step's input, and this step overwrites the previous step's input): wait until that kernel
+    // has completed and its stores are visible.  The trigger lets the NEXT launch's CTAs take the SM slots this grid no longer needs
+    // once every CTA of this grid has started; they stop at this same wait.  Both are no-ops in a launch without the attribute.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     // plane index i of this CTA's march = own plane z0 - 1 + i: periodic inside a whole lattice, running into the ghost planes of a slab
     auto plane_of = [&](int i) {
@@ -471,14 +478,23 @@ int launch_cfg(const FieldPtrs<T>& f, int N, const ZRange& zr, const GhostPtrs<T
     memset(&gh, 0, sizeof(gh));
     if (ghosts) gh = *ghosts;
     StepCoefT<T> k = { (T)c.c1, (T)c.c2, (T)c.c3, (T)c.d1, (T)c.d2, (T)c.d3, (T)c.dt, (T)c.sigma2 };
-    if (maps && opt.staging == AHS_STAGING_TENSOR) {
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, gh, N, zr, nchunks, k, maps->stage, maps->th2, maps->wstage, maps->wth2, 1);
-    } else {
-        StepMaps none;
-        memset(&none, 0, sizeof(none));
-        kern<<<(unsigned)blocks, C::NTHREADS, C::SMEM, st>>>(f, gh, N, zr, nchunks, k, none.stage, none.th2, none.wstage, none.wth2, 0);
-    }
-    return cudaGetLastError() == cudaSuccess ? 1 : AHS_ERR_CUDA;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(C::NTHREADS);
+    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.stream = st;
+    cudaLaunchAttribute pdl[1];
+    pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // this launch may begin before the stream's previous kernel has drained
+    pdl[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = pdl;
+    cfg.numAttrs = opt.step_pdl ? 1 : 0;
+    StepMaps none;
+    memset(&none, 0, sizeof(none));
+    const bool tma = maps && opt.staging == AHS_STAGING_TENSOR;
+    const StepMaps& mp = tma ? *maps : none;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, f, gh, N, zr, nchunks, k, mp.stage, mp.th2, mp.wstage, mp.wth2, tma ? 1 : 0);
+    return (e == cudaSuccess && cudaGetLastError() == cudaSuccess) ? 1 : AHS_ERR_CUDA;
 }
 
 }  // namespace

@@ -698,7 +698,8 @@ def test_options_change_the_launch_shape_not_the_result(ahs, prec, N):
         want, dref = ref.get_fields_native(), ref.diagnostics()
     settings = [{ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS}, {ahs.AHS_OPT_STEP_CHUNKS: 1, ahs.AHS_OPT_DIAG_CHUNKS: 1},
                 {ahs.AHS_OPT_STEP_CHUNKS: 100, ahs.AHS_OPT_DIAG_CHUNKS: 37}, {ahs.AHS_OPT_STEP_CHUNKS: N // 2, ahs.AHS_OPT_DIAG_CHUNKS: N // 4},
-                {ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS, ahs.AHS_OPT_STEP_CHUNKS: 37, ahs.AHS_OPT_DIAG_CHUNKS: 5}]
+                {ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS, ahs.AHS_OPT_STEP_CHUNKS: 37, ahs.AHS_OPT_DIAG_CHUNKS: 5},
+                {ahs.AHS_OPT_STEP_PDL: 1}, {ahs.AHS_OPT_STEP_PDL: 1, ahs.AHS_OPT_STEP_CHUNKS: 100, ahs.AHS_OPT_STAGING: ahs.AHS_STAGING_ROWS}]
     for opts in settings:
         with ahs.Simulation(N=N, precision=prec, seed=21) as sim:
             for k, v in opts.items():
@@ -711,7 +712,7 @@ def test_options_change_the_launch_shape_not_the_result(ahs, prec, N):
                 assert d[key] == pytest.approx(dref[key], rel=1e-11, abs=1e-11 * abs(dref["v2_den"])), (opts, key)
             assert d["gauss_max"] == dref["gauss_max"], opts
     with ahs.Simulation(N=N, precision=prec) as sim:
-        for bad in ((99, 0), (ahs.AHS_OPT_STAGING, 2), (ahs.AHS_OPT_STEP_CHUNKS, N + 1), (ahs.AHS_OPT_DIAG_CHUNKS, -1), (ahs.AHS_OPT_DIAG_TRIG, 2)):
+        for bad in ((99, 0), (ahs.AHS_OPT_STAGING, 2), (ahs.AHS_OPT_STEP_CHUNKS, N + 1), (ahs.AHS_OPT_DIAG_CHUNKS, -1), (ahs.AHS_OPT_DIAG_TRIG, 2), (ahs.AHS_OPT_STEP_PDL, 2)):
             with pytest.raises(ahs.AhsError) as e:
                 sim.set_option(*bad)
             assert e.value.code == ahs.AHS_ERR_INVALID_ARG
